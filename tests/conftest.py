@@ -1,0 +1,20 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on the B200 box)")
+
+
+@pytest.fixture(scope="session")
+def cfg2_oracle_cloud():
+    """Oracle cloud of BASELINE.json configs[1] (monodisperse 5 um, 2 mg/cm^2), built once."""
+    import pdv_workloads as W
+    from oracle import cloud
+    return cloud.build_cloud(W.config(1)["clouds"][0])
