@@ -1,0 +1,210 @@
+/* pdv.h -- C-ABI of the B200-native Monte-Carlo PDV spectrum library (libpdv_b200.so).
+ *
+ * The library computes what arXiv 2012.00963 (Shi et al., "Reconstruction and interpretation of photon
+ * Doppler velocimetry spectrum for ejecta particles from shock-loaded sample in vacuum") section II.B
+ * describes: Monte-Carlo multiple-scattering transport of the PDV probe photons through a cloud of
+ * spherical ejecta particles above a moving free surface, with the Doppler shifts of the photons that
+ * return to the probe histogrammed per time snapshot (steps (1)-(7) at PAPER.md:174-183).
+ *
+ * C99.  No C++ types and no exceptions cross this boundary.  Every pointer is a HOST pointer unless its
+ * comment says "device".  All physical quantities are SI doubles.  Every function returns a pdv_status
+ * (or void / const char*); on any status other than PDV_OK the caller's output buffers are untouched.
+ * There is no CPU fallback: without a CUDA device pdv_cloud_create still builds the host-side optics
+ * (so they can be inspected) but pdv_mc_run returns PDV_E_CUDA.
+ *
+ * Conventions (readings R1-R4): z points from the free surface to the probe; ejecta move in
+ * +z with v = z/t; photons start at the cloud top with direction cosine mu = u_z = -1; the "Doppler
+ * velocity" of a history is  v~ = 1/2 sum_k (mu_k_out - mu_k_in) v_k  = Eq. 4 times
+ * c/(2 w_r); the frequency shift is 2 v~/lambda.  T is the vertical optical depth measured down from the
+ * cloud top (T = 0 top, T = tau_ext at the free surface).
+ */
+#ifndef PDV_H_
+#define PDV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PDV_OK = 0,
+    PDV_E_INVALID = 1,      /* NULL where not allowed, out-of-range value, inconsistent sizes */
+    PDV_E_NOMEM = 2,        /* host or device allocation failed */
+    PDV_E_CUDA = 3,         /* no device, or a CUDA call failed; text in pdv_last_error() */
+    PDV_E_UNSUPPORTED = 4   /* valid request the kernels do not implement (e.g. tables too large for shared memory) */
+} pdv_status;
+
+typedef struct pdv_cloud pdv_cloud;    /* opaque; owned by the library; immutable after creation */
+
+/* ---- cloud definition: PAPER.md section II.C (187-203) ------------------------------------------------ */
+typedef struct {
+    size_t struct_size;          /* = sizeof(pdv_cloud_params); lets the struct grow */
+    double area_mass;            /* m0, total area mass of the ejecta, kg/m^2 (1 mg/cm^2 = 1e-2); >= 0   (Eq. 9)  */
+    double density;              /* rho0 of the particle material, kg/m^3; > 0                          (Eq. 9)  */
+    double v_fs;                 /* free-surface velocity, m/s; > 0                                     (Eq. 20) */
+    int32_t profile_kind;        /* 0: exponential law Eq. 20 truncated to [v_fs, vmax_ratio v_fs] and renormalised;
+                                    1: tabulated cumulative mass prof_cum_mass(prof_v) */
+    double beta;                 /* velocity distribution coefficient of Eq. 20; > 0 (kind 0) */
+    double vmax_ratio;           /* cloud top velocity / v_fs; > 1 */
+    int32_t n_prof;              /* kind 1: number of table points (>= 2) */
+    const double *prof_v;        /* kind 1: [n_prof] strictly increasing velocities, prof_v[0] = v_fs, last = v_max */
+    const double *prof_cum_mass; /* kind 1: [n_prof] non-decreasing cumulative mass below v (any units)  */
+    int32_t n_classes;           /* size distribution as explicit classes (Eq. 21 discretised by the caller, or by
+                                    pdv_lognormal_classes); 1..PDV_MAX_CLASSES */
+    const double *diameter;      /* [n_classes] particle diameters d_c, m; > 0 */
+    const double *number_weight; /* [n_classes] relative NUMBER of particles per class; > 0; normalised internally */
+    double m_re, m_im;           /* complex refractive index of the particles, m = m_re + i m_im, m_im >= 0 absorbs */
+    double wavelength;           /* probe wavelength lambda, m (1550e-9 in the paper) */
+    double surface_reflectivity; /* R in [0,1]: weight kept by a photon reflected at the free surface (R = 1: paper) */
+    int32_t surface_model;       /* 0: paper's "ideal diffuse reflection", polar angle uniform;
+                                    1: Lambertian (mu = sqrt(xi)) */
+    int32_t n_phase_bins;        /* K of the inverse-CDF phase table D_K; a power of two in [16, 4096]; 0 -> 1024 */
+    int32_t n_depth_bins;        /* depth bins uniform in v (= in z at fixed t); [1, 4096]; 0 -> 1024 */
+    int32_t phase_model;         /* 0: Mie, Eq. 12-14; 1: isotropic ("uniform") scattering, Fig. 6 case 2,
+                                    with the Mie efficiencies kept for extinction and albedo */
+} pdv_cloud_params;
+
+#define PDV_MAX_CLASSES 32
+
+/* Discretises the log-normal number distribution of Eq. 21 into n classes: n bins of equal
+ * width in x = ln(d/d_median)/sigma_ln over [-3, 3 + 3 sigma_ln], representative diameter at the bin centre
+ * in x, weight = standard-normal mass of the bin, renormalised to 1 (reading R11).
+ * sigma_ln = 0 gives one class (n is ignored, diameter[0] = d_median, weight[0] = 1) and returns *n_out = 1.
+ * diameter, weight: [n] outputs.  n_out may be NULL. */
+pdv_status pdv_lognormal_classes(double d_median, double sigma_ln, int32_t n, double *diameter, double *weight,
+                                 int32_t *n_out);
+
+/* Builds the optics of one cloud on the host in double precision -- per class the Mie efficiencies K_ext,
+ * K_sca, K_abs (Eq. 12) and the inverse-CDF table of the phase function |S1|^2+|S2|^2 (Eq. 13-14,
+ * PAPER.md:128-135); the class hit probabilities P_c ~ w_c d_c^2 K_ext,c (Eq. 8); the mass-extinction
+ * coefficient kappa = 3 sum w d^2 K_ext / (2 rho0 sum w d^3) and tau_ext = kappa m0 (Eq. 10);
+ * the depth table T_j (Eq. 20) -- and, when a CUDA device is present, copies the fp32 tables to it.
+ * *out receives the new cloud; release it with pdv_cloud_destroy. */
+pdv_status pdv_cloud_create(const pdv_cloud_params *params, pdv_cloud **out);
+
+/* NULL is a no-op.  The cloud must not be in use by a running pdv_mc_run. */
+void pdv_cloud_destroy(pdv_cloud *cloud);
+
+typedef struct {
+    size_t struct_size;
+    int32_t n_classes, n_phase_bins, n_depth_bins, on_device;
+    double tau_ext;              /* vertical extinction optical thickness of the cloud */
+    double kappa;                /* mass-extinction coefficient, m^2/kg */
+    double sauter_diameter;      /* sum w d^3 / sum w d^2 of the class list */
+    double v_fs, v_max;
+    double mean_albedo;          /* sum_c P_c K_sca,c/K_ext,c */
+    double mean_g;               /* scattering-weighted mean asymmetry parameter */
+} pdv_cloud_info;
+
+pdv_status pdv_cloud_get_info(const pdv_cloud *cloud, pdv_cloud_info *out);
+
+/* Copies the host (double) tables of the cloud into caller buffers; any pointer may be NULL to skip it.
+ * k_ext,k_sca,g,p_class: [n_classes].  phase: [n_classes][n_phase_bins+1], M_c[k] = F_c^-1(k/K) in cos(theta).
+ * T_edge: [n_depth_bins+1], T at velocity v_max - j (v_max - v_fs)/n_depth_bins. */
+pdv_status pdv_cloud_get_tables(const pdv_cloud *cloud, double *k_ext, double *k_sca, double *g, double *p_class,
+                                double *phase, double *T_edge);
+
+/* ---- Monte-Carlo run: PAPER.md section II.B steps (1)-(7) (174-183) ---------------------------------- */
+typedef struct {
+    size_t struct_size;
+    int32_t n_bins;              /* velocity bins, 1..PDV_MAX_BINS; bin k = [v_lo + k dv, v_lo + (k+1) dv) */
+    double v_lo, v_hi;           /* m/s; v_hi > v_lo */
+    double aperture_sr;          /* on-axis probe aperture, sr, in (0, 2 pi]: detected iff mu_exit >= 1 - aperture/(2 pi) */
+    int32_t mode;                /* 0: implicit capture (weight *= K_sca/K_ext, Eq. 11 in expectation);
+                                    1: analog (absorbed with probability K_abs/K_ext, the paper's step (4)) */
+    int32_t max_events;          /* Russian roulette once a history has had >= max_events particle events; 0: never */
+    double roulette_survival;    /* p in (0,1]; a photon survives with probability p and weight w/p.  The kernel plays
+                                    only while w/p <= 1 (weights never exceed one photon; reading R20) */
+    int32_t single_scatter_only; /* 1: a history is cut at its second particle event ("truncated" weight) */
+    uint64_t first_photon_id;    /* histories are keyed by id in [first_photon_id, first_photon_id + n_photons) */
+    int32_t output_on_device;    /* 0: hist/hist2/stats are host pointers, the call returns when they are filled;
+                                    1: they are DEVICE pointers, the call only enqueues work on cuda_stream */
+    int32_t blocks_per_sm;       /* launch shape override for tests; 0: library default */
+    int32_t threads_per_block;   /* 0: library default; multiple of 32, <= 512 */
+} pdv_run_opts;
+
+#define PDV_MAX_BINS 8192
+
+typedef struct {                 /* weights in units of photons; identity (exact in the kernel's fixed point):
+                                    detected+underflow+overflow+escaped+absorbed_particles+absorbed_surface
+                                    +roulette_killed-roulette_gained+truncated = histories */
+    double detected;             /* inside the aperture and inside [v_lo, v_hi): = sum of hist */
+    double underflow, overflow;  /* inside the aperture, v~ < v_lo / v~ >= v_hi */
+    double escaped;              /* left through the top outside the aperture */
+    double absorbed_particles;   /* Eq. 11, p_a */
+    double absorbed_surface;     /* (1 - R) at the free surface */
+    double roulette_killed, roulette_gained;
+    double truncated;            /* single_scatter_only */
+    uint64_t histories;
+    uint64_t particle_events;    /* "scattering events": particle interactions (absorbing ones included) */
+    uint64_t surface_reflections;
+    uint64_t max_events_in_history;
+} pdv_run_stats;
+
+/* Runs n_photons histories for every (cloud, snapshot) unit, unit index u = i_cloud * n_snap + i_snap.
+ *   clouds  [n_clouds] clouds created by pdv_cloud_create (n_clouds >= 1)
+ *   t_snap  [n_snap] snapshot times in s, each > 0 (n_snap >= 1).  In vacuum z = v t makes the
+ *           expected spectrum independent of t (reading R16): t selects the unit's random stream.
+ *   hist    [n_clouds][n_snap][n_bins] sum of weights of detected photons per velocity bin (Eq. 19)
+ *   hist2   same shape, sum of squared weights (variance estimate); may be NULL
+ *   stats   [n_clouds][n_snap]; may be NULL
+ *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream), or NULL for the default stream
+ * Reproducibility: the same (clouds, n_snap, n_photons, seed, first_photon_id, opts) give bit-identical
+ * hist/hist2/stats for any launch shape -- tallies are integer fixed point (Q31) and every history draws
+ * from its own Philox4x32-10 counter stream keyed by (seed, photon id, unit).  Runs over id ranges [a,b)
+ * and [b,c) sum to the run over [a,c).  n_photons = 0 is valid and yields zeros. */
+pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const double *t_snap, int32_t n_snap,
+                      uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
+                      double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream);
+
+/* Per-history record of the diagnostic entry point below. */
+typedef struct {
+    float vt;                    /* Doppler velocity v~ at termination, m/s */
+    float weight;                /* final weight */
+    float mu_exit;               /* direction cosine when the history ended */
+    int32_t fate;                /* 0 detected, 1 escaped, 2 absorbed (analog), 3 roulette-killed, 4 truncated,
+                                    5 detected but under/overflow */
+    int32_t n_scatter, n_reflect;
+} pdv_trace_record;
+
+/* Diagnostic: same transport as pdv_mc_run for ONE unit (cloud, unit index `unit`), and additionally one
+ * record per history, records[id - first_photon_id] (HOST, [n_photons]).  Used by the tests to compare
+ * single histories with the oracle run on the same Philox stream. */
+pdv_status pdv_mc_trace(const pdv_cloud *cloud, uint32_t unit, uint64_t n_photons, uint64_t seed,
+                        const pdv_run_opts *opts, double *hist, double *hist2, pdv_run_stats *stats,
+                        pdv_trace_record *records, void *cuda_stream);
+
+/* Stacks per-snapshot histograms into the spectrogram (Fig. 1 items 12-13; Eq. 19):
+ *   scale 0: out = hist / n_photons            (probability per bin)
+ *   scale 1: out = hist / (n_photons dv)       (spectral density per m/s), dv = (v_hi - v_lo)/n_bins
+ *   scale 2: out = 10 log10(hist / n_photons), floor_db where hist = 0
+ * hist [n_snap][n_bins] doubles, out [n_snap][n_bins] floats; both HOST when on_device = 0, both DEVICE when 1
+ * (then the work is enqueued on cuda_stream). */
+pdv_status pdv_spectrogram(const double *hist, int32_t n_snap, int32_t n_bins, uint64_t n_photons,
+                           double v_lo, double v_hi, int32_t scale, float floor_db, float *out,
+                           int32_t on_device, void *cuda_stream);
+
+/* Measures the issue-rate denominators on the current device: a dependent-free FFMA stream and a MUFU
+ * stream, each run for ~`millis` ms on every SM.  Outputs (any may be NULL): thread-instructions/s of each,
+ * the SM clock in MHz observed meanwhile (clock64 over globaltimer), and the SM count. */
+pdv_status pdv_issue_peaks(double millis, double *ffma_thread_inst_per_s, double *mufu_thread_inst_per_s,
+                           double *sm_clock_mhz, int32_t *n_sm, void *cuda_stream);
+
+/* Launch statistics of the last pdv_mc_run / pdv_mc_trace on this thread: kernels launched and the duration of
+ * the transport kernel in ms measured with CUDA events on cuda_stream (0 when output_on_device = 1, where
+ * nothing is synchronised).  Any pointer may be NULL. */
+pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block,
+                                int32_t *smem_bytes);
+
+/* Thread-local message of the last failing call on this thread; "" if none.  Valid until the next call. */
+const char *pdv_last_error(void);
+
+/* Library version string, e.g. "pdv_b200 0.1 (sm_100a)". */
+const char *pdv_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDV_H_ */

@@ -1,0 +1,520 @@
+// pdv_api.cu -- the C-ABI of include/pdv.h: argument checking, cloud upload, workspace, launches, read-back.
+// No arithmetic of the method lives here beyond packing the fp32/fixed-point device tables.
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pdv_device.h"
+#include "pdv_optics.hpp"
+
+using namespace pdv;
+
+struct pdv_cloud {
+    HostCloud host;
+    std::vector<unsigned char> blob;     // device image (host copy)
+    mutable std::mutex mu;
+    mutable unsigned char *d_blob = nullptr;
+    mutable int device = -1;
+};
+
+namespace {
+
+thread_local std::string g_err;
+thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0; } g_last;
+
+struct Workspace {
+    unsigned char *d = nullptr;
+    size_t bytes = 0;
+    int device = -1;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ~Workspace() {
+        // process teardown: the CUDA context may already be gone; leak rather than fault
+    }
+};
+thread_local Workspace g_ws;
+
+pdv_status fail(pdv_status s, const std::string &msg) { g_err = msg; return s; }
+pdv_status cuda_fail(cudaError_t e, const char *what) {
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? PDV_E_NOMEM : PDV_E_CUDA;
+}
+#define CU(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, what); } while (0)
+
+size_t align16(size_t v) { return (v + 15) & ~(size_t)15; }
+uint32_t f2u(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
+float u2f(uint32_t u) { float f; std::memcpy(&f, &u, 4); return f; }
+
+uint32_t to_thr32(double p) {            // smallest integer t with t/2^32 >= p, clamped
+    const double v = std::ceil(p * 4294967296.0);
+    if (v <= 0.0) return 0u;
+    if (v >= 4294967295.0) return 0xFFFFFFFFu;
+    return (uint32_t)v;
+}
+
+void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
+    const int nc = h.n_classes, K = h.K, nd = h.n_depth;
+    int steps = 0;
+    while ((1 << steps) < nc) ++steps;
+    const int n_pad = 1 << steps;
+    // fp32 depth table
+    std::vector<float> Tf(nd + 1);
+    for (int j = 0; j <= nd; ++j) Tf[j] = (float)h.T_edge[j];
+    Tf[0] = 0.f;
+    for (int j = 1; j <= nd; ++j) if (Tf[j] < Tf[j - 1]) Tf[j] = Tf[j - 1];
+    // guide over (float bits >> 16): exponent + 7 mantissa bits, i.e. 128 cells per octave of T
+    float t_min = 0.f;
+    for (int j = 1; j <= nd; ++j) if (Tf[j] > 0.f) { t_min = Tf[j]; break; }
+    uint32_t base = 0, n_guide = 1;
+    if (t_min > 0.f) {
+        const uint32_t top = f2u(Tf[nd]) >> 16;
+        base = f2u(t_min) >> 16;
+        if (top - base + 1 > 8192u) base = top - 8191u;
+        n_guide = top - base + 1;
+    }
+    std::vector<uint16_t> guide(n_guide, 0);
+    {
+        int j = 0;
+        for (uint32_t i = 1; i < n_guide; ++i) {          // guide[0] = 0: cell 0 also serves every T below it
+            const float lo = u2f((base + i) << 16);
+            while (j + 1 <= nd - 1 && Tf[j + 1] <= lo) ++j;
+            guide[i] = (uint16_t)j;
+        }
+    }
+    DevCloudHeader hd;
+    std::memset(&hd, 0, sizeof(hd));
+    size_t off = sizeof(DevCloudHeader);
+    hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * (size_t)nc * (K + 1));
+    hd.off_tedge = (uint32_t)off;  off = align16(off + sizeof(float) * (nd + 2));
+    hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * n_pad);
+    hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
+    hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
+    hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
+    hd.blob_bytes = (uint32_t)off;
+    hd.n_classes = nc; hd.K = K; hd.n_depth = nd; hd.n_guide = n_guide; hd.guide_base = base;
+    hd.log2K = 0;
+    while ((1 << hd.log2K) < K) ++hd.log2K;
+    hd.tau_ext = Tf[nd]; hd.v_fs = (float)h.v_fs; hd.v_max = (float)h.v_max;
+    hd.dv_depth = (float)((h.v_max - h.v_fs) / nd);
+    hd.R_q31 = (uint32_t)std::llround(h.R * 2147483648.0);
+    hd.R_thr = to_thr32(h.R);
+    hd.surface_model = (uint32_t)h.surface_model;
+    blob.assign(off, 0);
+    std::memcpy(blob.data(), &hd, sizeof(hd));
+    float *ph = reinterpret_cast<float *>(blob.data() + hd.off_phase);
+    for (int c = 0; c < nc; ++c) {
+        float prev = -1.f;
+        for (int k = 0; k <= K; ++k) {
+            float v = (float)h.phase[(size_t)c * (K + 1) + k];
+            if (v < prev) v = prev;
+            ph[(size_t)c * (K + 1) + k] = v;
+            prev = v;
+        }
+    }
+    float *te = reinterpret_cast<float *>(blob.data() + hd.off_tedge);
+    for (int j = 0; j <= nd; ++j) te[j] = Tf[j];
+    te[nd + 1] = Tf[nd];
+    uint32_t *thr = reinterpret_cast<uint32_t *>(blob.data() + hd.off_thr);
+    uint32_t *alb = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albedo);
+    uint32_t *albt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albthr);
+    double cum = 0.0;
+    for (int c = 0; c < n_pad; ++c) {
+        if (c < nc - 1) {
+            cum += h.p_class[c];
+            const double v = std::ceil(cum * 4294967296.0 - 0.5);     // x1 + 0.5 >= cum 2^32
+            thr[c] = v <= 0.0 ? 0u : (v >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)v);
+        } else {
+            thr[c] = 0xFFFFFFFFu;
+        }
+        const double om = c < nc ? h.k_sca[c] / h.k_ext[c] : 0.0;
+        alb[c] = (uint32_t)std::llround(std::min(std::max(om, 0.0), 1.0) * 2147483648.0);
+        albt[c] = to_thr32(om);
+    }
+    std::memcpy(blob.data() + hd.off_guide, guide.data(), sizeof(uint16_t) * n_guide);
+}
+
+pdv_status ensure_on_device(const pdv_cloud *c, int device) {
+    std::lock_guard<std::mutex> lk(c->mu);
+    if (c->d_blob && c->device == device) return PDV_OK;
+    if (c->d_blob) return fail(PDV_E_INVALID, "cloud was uploaded to another CUDA device");
+    unsigned char *d = nullptr;
+    CU(cudaMalloc(&d, c->blob.size()), "cudaMalloc(cloud tables)");
+    cudaError_t e = cudaMemcpy(d, c->blob.data(), c->blob.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(cloud tables)"); }
+    c->d_blob = d;
+    c->device = device;
+    return PDV_OK;
+}
+
+pdv_status get_workspace(size_t bytes, int device, unsigned char **out) {
+    Workspace &w = g_ws;
+    if (w.d && (w.device != device || w.bytes < bytes)) {
+        cudaFree(w.d);
+        w.d = nullptr; w.bytes = 0;
+    }
+    if (!w.d) {
+        const size_t want = std::max(bytes, (size_t)1 << 20);
+        CU(cudaMalloc(&w.d, want), "cudaMalloc(workspace)");
+        w.bytes = want; w.device = device;
+    }
+    if (!w.e0) {
+        CU(cudaEventCreate(&w.e0), "cudaEventCreate");
+        CU(cudaEventCreate(&w.e1), "cudaEventCreate");
+    }
+    *out = w.d;
+    return PDV_OK;
+}
+
+struct RunPlan {
+    RunParams rp;
+    LaunchShape shape;
+    bool poly, analog;
+};
+
+pdv_status check_opts(const pdv_run_opts *o) {
+    if (!o) return fail(PDV_E_INVALID, "opts is NULL");
+    if (o->struct_size != sizeof(pdv_run_opts)) return fail(PDV_E_INVALID, "opts->struct_size mismatch");
+    if (o->n_bins < 1 || o->n_bins > PDV_MAX_BINS) return fail(PDV_E_INVALID, "n_bins out of range");
+    if (!(o->v_hi > o->v_lo) || !std::isfinite(o->v_hi) || !std::isfinite(o->v_lo)) return fail(PDV_E_INVALID, "need v_hi > v_lo");
+    if (!(o->aperture_sr > 0.0) || o->aperture_sr > 2.0 * 3.14159265358979323846 * (1 + 1e-12))
+        return fail(PDV_E_INVALID, "aperture_sr not in (0, 2 pi]");
+    if (o->mode != 0 && o->mode != 1) return fail(PDV_E_INVALID, "mode must be 0 or 1");
+    if (o->max_events < 0) return fail(PDV_E_INVALID, "max_events < 0");
+    if (o->max_events > 0 && !(o->roulette_survival > 0.0 && o->roulette_survival <= 1.0))
+        return fail(PDV_E_INVALID, "roulette_survival not in (0,1]");
+    if (o->threads_per_block < 0 || o->threads_per_block > 512 || (o->threads_per_block % 32) != 0)
+        return fail(PDV_E_INVALID, "threads_per_block must be a multiple of 32, <= 512");
+    if (o->blocks_per_sm < 0 || o->blocks_per_sm > 32) return fail(PDV_E_INVALID, "blocks_per_sm out of range");
+    return PDV_OK;
+}
+
+// Fills the run parameters and the launch shape.  `ws` layout: next_id | hist | hist2 | stats | units.
+pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, uint64_t n_photons, uint64_t seed,
+                     const pdv_run_opts *o, bool trace, int device, RunPlan &plan, size_t max_blob) {
+    RunParams &rp = plan.rp;
+    std::memset(&rp, 0, sizeof(rp));
+    rp.n_units = (uint32_t)n_units;
+    rp.n_bins = (uint32_t)o->n_bins;
+    rp.max_events = (uint32_t)o->max_events;
+    rp.single_scatter_only = o->single_scatter_only ? 1u : 0u;
+    const double p = o->max_events > 0 ? o->roulette_survival : 1.0;
+    rp.roulette_thr = to_thr32(p);
+    rp.roulette_wcap = (uint32_t)std::floor(p * 2147483648.0);
+    rp.roulette_inv_p = (float)(1.0 / p);
+    rp.v_lo = (float)o->v_lo;
+    rp.inv_dv = (float)((double)o->n_bins / (o->v_hi - o->v_lo));
+    rp.mu_aperture = (float)(1.0 - o->aperture_sr / (2.0 * 3.14159265358979323846));
+    rp.n_photons = n_photons;
+    rp.first_id = o->first_photon_id;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { rp.key0[r] = k0; rp.key1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+
+    plan.poly = false;
+    for (int i = 0; i < n_clouds; ++i) plan.poly = plan.poly || clouds[i]->host.n_classes > 1;
+    plan.analog = o->mode == 1;
+
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device), "cudaGetDeviceProperties");
+    const int smem = (int)(16 * (size_t)o->n_bins + max_blob);
+    if ((size_t)smem > (size_t)prop.sharedMemPerBlockOptin)
+        return fail(PDV_E_UNSUPPORTED, "cloud tables + histogram exceed the shared memory of one block");
+    int block = o->threads_per_block > 0 ? o->threads_per_block : 512;
+    int per_sm = 0;
+    CU(transport_max_blocks_per_sm(plan.poly, plan.analog, trace, block, smem, &per_sm), "occupancy query");
+    if (per_sm < 1) return fail(PDV_E_UNSUPPORTED, "transport kernel does not fit on an SM with these tables");
+    if (o->blocks_per_sm > 0) per_sm = std::min(per_sm, o->blocks_per_sm);
+    long long grid = (long long)prop.multiProcessorCount * per_sm;
+    const unsigned long long total = n_photons * (unsigned long long)n_units;
+    const long long useful = (long long)((total + block - 1) / block);       // one history per thread at least
+    if (useful < grid) grid = std::max(1LL, useful);
+    plan.shape.grid = (int)grid; plan.shape.block = block; plan.shape.smem = smem;
+    // chunk: ~16 fetches per warp over the run, between 32 and 4096 ids, multiple of 32
+    const unsigned long long warps = (unsigned long long)grid * (block / 32);
+    unsigned long long chunk = total / (warps * 16ull + 1ull);
+    chunk = std::min<unsigned long long>(std::max<unsigned long long>(chunk, 32ull), 4096ull);
+    rp.chunk = (uint32_t)((chunk + 31ull) & ~31ull);
+    return PDV_OK;
+}
+
+pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, const uint32_t *unit_streams,
+                    uint64_t n_photons, uint64_t seed, const pdv_run_opts *o, double *hist, double *hist2,
+                    pdv_run_stats *stats, pdv_trace_record *records, void *cuda_stream) {
+    const int n_units = n_clouds * n_snap;
+    const bool trace = records != nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    int device = 0;
+    CU(cudaGetDevice(&device), "cudaGetDevice");
+    size_t max_blob = 0;
+    for (int i = 0; i < n_clouds; ++i) {
+        pdv_status s = ensure_on_device(clouds[i], device);
+        if (s != PDV_OK) return s;
+        max_blob = std::max(max_blob, clouds[i]->blob.size());
+    }
+    RunPlan plan;
+    pdv_status s = make_plan(clouds, n_clouds, n_units, n_photons, seed, o, trace, device, plan, max_blob);
+    if (s != PDV_OK) return s;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nb = (size_t)o->n_bins;
+    // workspace layout
+    size_t off = 0;
+    const size_t o_next = off;  off = align16(off + 8 * (size_t)n_units);
+    const size_t o_hist = off;  off = align16(off + 8 * nb * n_units);
+    const size_t o_hist2 = off; off = align16(off + 8 * nb * n_units);
+    const size_t o_stats = off; off = align16(off + 8 * (size_t)ST_COUNT * n_units);
+    const size_t zero_bytes = off;
+    const size_t o_units = off; off = align16(off + sizeof(UnitDesc) * (size_t)n_units);
+    const size_t o_oh = off;    off = align16(off + 8 * nb * n_units);
+    const size_t o_oh2 = off;   off = align16(off + 8 * nb * n_units);
+    const size_t o_os = off;    off = align16(off + sizeof(pdv_run_stats) * (size_t)n_units);
+    unsigned char *ws = nullptr;
+    if ((s = get_workspace(off, device, &ws)) != PDV_OK) return s;
+
+    std::vector<UnitDesc> units(n_units);
+    for (int i = 0; i < n_clouds; ++i)
+        for (int j = 0; j < n_snap; ++j) {
+            UnitDesc &u = units[(size_t)i * n_snap + j];
+            u.cloud_blob = clouds[i]->d_blob;
+            u.stream = unit_streams ? unit_streams[(size_t)i * n_snap + j] : (uint32_t)(i * n_snap + j);
+            u.pad = 0;
+        }
+    pdv_trace_record *d_trace = nullptr;
+    if (trace && n_photons) CU(cudaMalloc(&d_trace, sizeof(pdv_trace_record) * n_photons), "cudaMalloc(trace)");
+    auto cleanup = [&]() { if (d_trace) cudaFree(d_trace); };
+#define CUX(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return cuda_fail(e_, what); } } while (0)
+
+    CUX(cudaMemsetAsync(ws, 0, zero_bytes, st), "cudaMemsetAsync(workspace)");
+    CUX(cudaMemcpyAsync(ws + o_units, units.data(), sizeof(UnitDesc) * n_units, cudaMemcpyHostToDevice, st), "copy unit table");
+    RunParams &rp = plan.rp;
+    rp.units = reinterpret_cast<const UnitDesc *>(ws + o_units);
+    rp.next_id = reinterpret_cast<unsigned long long *>(ws + o_next);
+    rp.hist = reinterpret_cast<unsigned long long *>(ws + o_hist);
+    rp.hist2 = reinterpret_cast<unsigned long long *>(ws + o_hist2);
+    rp.stats = reinterpret_cast<unsigned long long *>(ws + o_stats);
+    rp.trace = d_trace;
+
+    g_last.n_kernels = 0; g_last.ms = 0.f;
+    g_last.grid = plan.shape.grid; g_last.block = plan.shape.block; g_last.smem = plan.shape.smem;
+    CUX(cudaEventRecord(g_ws.e0, st), "cudaEventRecord");
+    if (n_photons > 0) {
+        CUX(launch_transport(rp, plan.poly, plan.analog, trace, plan.shape, st), "transport kernel launch");
+        g_last.n_kernels += 1;
+    }
+    CUX(cudaEventRecord(g_ws.e1, st), "cudaEventRecord");
+
+    const bool dev_out = o->output_on_device != 0;
+    double *oh = dev_out ? hist : reinterpret_cast<double *>(ws + o_oh);
+    double *oh2 = hist2 ? (dev_out ? hist2 : reinterpret_cast<double *>(ws + o_oh2)) : nullptr;
+    pdv_run_stats *os = stats ? (dev_out ? stats : reinterpret_cast<pdv_run_stats *>(ws + o_os)) : nullptr;
+    CUX(launch_finalize(rp.hist, rp.hist2, rp.stats, (uint32_t)n_units, (uint32_t)nb, oh, oh2, os, st), "finalize kernel launch");
+    g_last.n_kernels += 1;
+    if (!dev_out) {
+        // stage into host temporaries first so that the caller's buffers stay untouched on failure
+        std::vector<double> th(nb * n_units), th2(hist2 ? nb * n_units : 0);
+        std::vector<pdv_run_stats> ts(stats ? n_units : 0);
+        std::vector<pdv_trace_record> tr;
+        CUX(cudaMemcpyAsync(th.data(), oh, 8 * nb * n_units, cudaMemcpyDeviceToHost, st), "read back hist");
+        if (hist2) CUX(cudaMemcpyAsync(th2.data(), oh2, 8 * nb * n_units, cudaMemcpyDeviceToHost, st), "read back hist2");
+        if (stats) CUX(cudaMemcpyAsync(ts.data(), os, sizeof(pdv_run_stats) * n_units, cudaMemcpyDeviceToHost, st), "read back stats");
+        CUX(cudaStreamSynchronize(st), "transport kernel execution");
+        if (trace && n_photons) CUX(cudaMemcpy(records, d_trace, sizeof(pdv_trace_record) * n_photons, cudaMemcpyDeviceToHost), "read back trace");
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, g_ws.e0, g_ws.e1) == cudaSuccess) g_last.ms = ms;
+        std::memcpy(hist, th.data(), 8 * nb * n_units);
+        if (hist2) std::memcpy(hist2, th2.data(), 8 * nb * n_units);
+        if (stats) std::memcpy(stats, ts.data(), sizeof(pdv_run_stats) * n_units);
+    } else if (trace) {
+        CUX(cudaStreamSynchronize(st), "transport kernel execution");
+        if (n_photons) CUX(cudaMemcpy(records, d_trace, sizeof(pdv_trace_record) * n_photons, cudaMemcpyDeviceToHost), "read back trace");
+    }
+    cleanup();
+#undef CUX
+    return PDV_OK;
+}
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+const char *pdv_last_error(void) { return g_err.c_str(); }
+const char *pdv_version(void) { return "pdv_b200 0.1 (sm_100a)"; }
+
+pdv_status pdv_lognormal_classes(double d_median, double sigma_ln, int32_t n, double *diameter, double *weight,
+                                 int32_t *n_out) {
+    g_err.clear();
+    int no = 0;
+    pdv_status s = lognormal_classes(d_median, sigma_ln, n, diameter, weight, &no);
+    if (s != PDV_OK) return fail(s, "pdv_lognormal_classes: need d_median > 0, sigma_ln >= 0, n >= 1, non-NULL outputs");
+    if (n_out) *n_out = no;
+    return PDV_OK;
+}
+
+pdv_status pdv_cloud_create(const pdv_cloud_params *params, pdv_cloud **out) {
+    g_err.clear();
+    if (!params || !out) return fail(PDV_E_INVALID, "params / out is NULL");
+    if (params->struct_size != sizeof(pdv_cloud_params)) return fail(PDV_E_INVALID, "params->struct_size mismatch");
+    pdv_cloud *c = new (std::nothrow) pdv_cloud;
+    if (!c) return fail(PDV_E_NOMEM, "out of host memory");
+    std::string err;
+    pdv_status s;
+    try {
+        s = build_host_cloud(*params, c->host, err);
+        if (s == PDV_OK) build_blob(c->host, c->blob);
+    } catch (const std::bad_alloc &) {
+        delete c;
+        return fail(PDV_E_NOMEM, "out of host memory");
+    }
+    if (s != PDV_OK) { delete c; return fail(s, err); }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
+        int device = 0;
+        if (cudaGetDevice(&device) == cudaSuccess) {
+            s = ensure_on_device(c, device);
+            if (s != PDV_OK) { delete c; return s; }
+        }
+    } else {
+        cudaGetLastError();          // host-only cloud: tables can be inspected, pdv_mc_run will refuse
+    }
+    *out = c;
+    return PDV_OK;
+}
+
+void pdv_cloud_destroy(pdv_cloud *c) {
+    if (!c) return;
+    if (c->d_blob) cudaFree(c->d_blob);
+    delete c;
+}
+
+pdv_status pdv_cloud_get_info(const pdv_cloud *c, pdv_cloud_info *out) {
+    g_err.clear();
+    if (!c || !out) return fail(PDV_E_INVALID, "cloud / out is NULL");
+    if (out->struct_size != sizeof(pdv_cloud_info)) return fail(PDV_E_INVALID, "out->struct_size mismatch");
+    const HostCloud &h = c->host;
+    out->n_classes = h.n_classes; out->n_phase_bins = h.K; out->n_depth_bins = h.n_depth;
+    out->on_device = c->d_blob ? 1 : 0;
+    out->tau_ext = h.tau_ext; out->kappa = h.kappa; out->sauter_diameter = h.sauter; out->v_fs = h.v_fs; out->v_max = h.v_max;
+    double om = 0.0, gs = 0.0;
+    for (int i = 0; i < h.n_classes; ++i) {
+        const double a = h.k_sca[i] / h.k_ext[i];
+        om += h.p_class[i] * a;
+        gs += h.p_class[i] * a * h.g[i];
+    }
+    out->mean_albedo = om;
+    out->mean_g = om > 0.0 ? gs / om : 0.0;
+    return PDV_OK;
+}
+
+pdv_status pdv_cloud_get_tables(const pdv_cloud *c, double *k_ext, double *k_sca, double *g, double *p_class,
+                                double *phase, double *T_edge) {
+    g_err.clear();
+    if (!c) return fail(PDV_E_INVALID, "cloud is NULL");
+    const HostCloud &h = c->host;
+    const size_t n = (size_t)h.n_classes;
+    if (k_ext) std::memcpy(k_ext, h.k_ext.data(), 8 * n);
+    if (k_sca) std::memcpy(k_sca, h.k_sca.data(), 8 * n);
+    if (g) std::memcpy(g, h.g.data(), 8 * n);
+    if (p_class) std::memcpy(p_class, h.p_class.data(), 8 * n);
+    if (phase) std::memcpy(phase, h.phase.data(), 8 * h.phase.size());
+    if (T_edge) std::memcpy(T_edge, h.T_edge.data(), 8 * h.T_edge.size());
+    return PDV_OK;
+}
+
+pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const double *t_snap, int32_t n_snap,
+                      uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
+                      double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream) {
+    g_err.clear();
+    if (!clouds || n_clouds < 1) return fail(PDV_E_INVALID, "need at least one cloud");
+    if (!t_snap || n_snap < 1) return fail(PDV_E_INVALID, "need at least one snapshot time");
+    if (!hist) return fail(PDV_E_INVALID, "hist is NULL");
+    pdv_status s = check_opts(opts);
+    if (s != PDV_OK) return s;
+    for (int i = 0; i < n_clouds; ++i) if (!clouds[i]) return fail(PDV_E_INVALID, "clouds[i] is NULL");
+    for (int j = 0; j < n_snap; ++j) if (!(t_snap[j] > 0.0) || !std::isfinite(t_snap[j])) return fail(PDV_E_INVALID, "snapshot times must be > 0");
+    if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
+    if (n_photons > (1ull << 62) || opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
+    return run_impl(clouds, n_clouds, n_snap, nullptr, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
+}
+
+pdv_status pdv_mc_trace(const pdv_cloud *cloud, uint32_t unit, uint64_t n_photons, uint64_t seed,
+                        const pdv_run_opts *opts, double *hist, double *hist2, pdv_run_stats *stats,
+                        pdv_trace_record *records, void *cuda_stream) {
+    g_err.clear();
+    if (!cloud || !hist || !records) return fail(PDV_E_INVALID, "cloud / hist / records is NULL");
+    pdv_status s = check_opts(opts);
+    if (s != PDV_OK) return s;
+    if (opts->output_on_device) return fail(PDV_E_INVALID, "pdv_mc_trace writes host buffers only");
+    if (n_photons > (1ull << 28)) return fail(PDV_E_INVALID, "pdv_mc_trace: at most 2^28 histories");
+    const pdv_cloud *cl[1] = {cloud};
+    return run_impl(cl, 1, 1, &unit, n_photons, seed, opts, hist, hist2, stats, records, cuda_stream);
+}
+
+pdv_status pdv_spectrogram(const double *hist, int32_t n_snap, int32_t n_bins, uint64_t n_photons,
+                           double v_lo, double v_hi, int32_t scale, float floor_db, float *out,
+                           int32_t on_device, void *cuda_stream) {
+    g_err.clear();
+    if (!hist || !out) return fail(PDV_E_INVALID, "hist / out is NULL");
+    if (n_snap < 0 || n_bins < 1 || n_photons == 0) return fail(PDV_E_INVALID, "need n_snap >= 0, n_bins >= 1, n_photons > 0");
+    if (!(v_hi > v_lo)) return fail(PDV_E_INVALID, "need v_hi > v_lo");
+    if (scale < 0 || scale > 2) return fail(PDV_E_INVALID, "scale must be 0, 1 or 2");
+    if (n_snap == 0) return PDV_OK;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)n_snap * n_bins;
+    const double inv_n = 1.0 / (double)n_photons, inv_dv = (double)n_bins / (v_hi - v_lo);
+    if (on_device) {
+        CU(launch_spectrogram(hist, n_snap, n_bins, inv_n, inv_dv, scale, floor_db, out, st), "spectrogram kernel launch");
+        return PDV_OK;
+    }
+    int device = 0;
+    CU(cudaGetDevice(&device), "cudaGetDevice");
+    unsigned char *ws = nullptr;
+    pdv_status s = get_workspace(align16(8 * n) + 4 * n, device, &ws);
+    if (s != PDV_OK) return s;
+    double *dh = reinterpret_cast<double *>(ws);
+    float *dout = reinterpret_cast<float *>(ws + align16(8 * n));
+    std::vector<float> tmp(n);
+    CU(cudaMemcpyAsync(dh, hist, 8 * n, cudaMemcpyHostToDevice, st), "copy hist");
+    CU(launch_spectrogram(dh, n_snap, n_bins, inv_n, inv_dv, scale, floor_db, dout, st), "spectrogram kernel launch");
+    CU(cudaMemcpyAsync(tmp.data(), dout, 4 * n, cudaMemcpyDeviceToHost, st), "read back spectrogram");
+    CU(cudaStreamSynchronize(st), "spectrogram kernel execution");
+    std::memcpy(out, tmp.data(), 4 * n);
+    return PDV_OK;
+}
+
+pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mhz, int32_t *n_sm, void *cuda_stream) {
+    g_err.clear();
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available");
+    }
+    if (!(millis > 0.0) || millis > 5000.0) return fail(PDV_E_INVALID, "millis must be in (0, 5000]");
+    int device = 0;
+    CU(cudaGetDevice(&device), "cudaGetDevice");
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device), "cudaGetDeviceProperties");
+    if (n_sm) *n_sm = prop.multiProcessorCount;
+    CU(launch_issue_peaks(millis, ffma, mufu, mhz, prop.multiProcessorCount, (cudaStream_t)cuda_stream), "issue-peak kernels");
+    return PDV_OK;
+}
+
+pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes) {
+    if (n_kernels) *n_kernels = g_last.n_kernels;
+    if (transport_ms) *transport_ms = g_last.ms;
+    if (grid) *grid = g_last.grid;
+    if (block) *block = g_last.block;
+    if (smem_bytes) *smem_bytes = g_last.smem;
+    return PDV_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,73 @@
+// pdv_device.h -- structures shared by the C-ABI layer (pdv_api.cu) and the kernels (pdv_kernels.cu).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/pdv.h"
+
+namespace pdv {
+
+// Fixed point of every weight and tally: Q31, one photon = 2^31.
+constexpr uint32_t kWOne = 0x80000000u;
+constexpr double kWScale = 1.0 / 2147483648.0;
+
+// Per-unit statistics slots (u64 each) in the device workspace.
+enum StatSlot {
+    ST_DETECTED = 0, ST_UNDER, ST_OVER, ST_ESCAPED, ST_ABS_PART, ST_ABS_SURF, ST_KILLED, ST_GAINED, ST_TRUNC,
+    ST_HISTORIES, ST_EVENTS, ST_REFLECT, ST_MAXEV, ST_COUNT = 16
+};
+
+// Device image of one cloud: one contiguous blob [DevCloudHeader | phase | T_edge | class thr | albedo Q31 | albedo thr | guide],
+// every section 16-byte aligned, copied verbatim into shared memory by each block.
+struct DevCloudHeader {
+    uint32_t blob_bytes;       // multiple of 16
+    uint32_t n_classes, K, log2K, n_depth, n_guide;
+    uint32_t off_phase, off_tedge, off_thr, off_albedo, off_albthr, off_guide;   // byte offsets from the blob start
+    uint32_t guide_base;       // (float bits of T) >> 16 of guide cell 0
+    float tau_ext, v_fs, v_max, dv_depth;
+    uint32_t R_q31;            // surface reflectivity, Q31
+    uint32_t R_thr;            // analog mode: reflected iff y1 < R_thr
+    uint32_t surface_model;
+    uint32_t pad[8];
+};
+static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
+
+struct UnitDesc {
+    const unsigned char *cloud_blob;   // device pointer
+    uint32_t stream;                   // Philox counter word 2 (unit index)
+    uint32_t pad;
+};
+
+struct RunParams {
+    const UnitDesc *units;
+    unsigned long long *next_id;       // [n_units] photons handed out so far (relative to first_id)
+    unsigned long long *hist;          // [n_units][n_bins] Q31 sum w
+    unsigned long long *hist2;         // [n_units][n_bins] Q31 sum w^2
+    unsigned long long *stats;         // [n_units][ST_COUNT]
+    pdv_trace_record *trace;           // TRACE only: [n_photons]
+    uint32_t n_units;
+    uint32_t n_bins;
+    uint32_t chunk;                    // photon ids a warp claims per fetch
+    uint32_t max_events;               // 0: no roulette
+    uint32_t single_scatter_only;
+    uint32_t roulette_thr;             // survive iff y0 < roulette_thr
+    uint32_t roulette_wcap;            // play only while w <= wcap (= floor(p 2^31))
+    float roulette_inv_p;
+    float v_lo, inv_dv, mu_aperture;
+    unsigned long long n_photons, first_id;
+    uint32_t key0[10], key1[10];       // Philox round keys
+};
+
+struct LaunchShape { int grid, block, smem; };
+
+// Host wrappers implemented in pdv_kernels.cu.
+cudaError_t launch_transport(const RunParams &rp, bool poly, bool analog, bool trace, LaunchShape shape, cudaStream_t st);
+cudaError_t transport_max_blocks_per_sm(bool poly, bool analog, bool trace, int block, int smem, int *out);
+cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,
+                            uint32_t n_units, uint32_t n_bins, double *out_hist, double *out_hist2, pdv_run_stats *out_stats,
+                            cudaStream_t st);
+cudaError_t launch_spectrogram(const double *hist, int n_snap, int n_bins, double inv_n, double inv_dv, int scale,
+                               float floor_db, float *out, cudaStream_t st);
+cudaError_t launch_issue_peaks(double millis, double *ffma, double *mufu, double *mhz, int n_sm, cudaStream_t st);
+
+}  // namespace pdv

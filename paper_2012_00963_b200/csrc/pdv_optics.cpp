@@ -1,0 +1,264 @@
+// pdv_optics.cpp -- host optics of a cloud (double precision).  See pdv_optics.hpp.
+//
+// Mie theory of a homogeneous sphere as the paper uses it (Eq. 12-14; ref. 33).  The
+// coefficients are the textbook ones for time factor exp(-i w t) (Im m > 0 absorbs), evaluated with
+// Riccati-Bessel recurrences:
+//   psi_n(x) = x j_n(x) upward from psi_-1 = cos x, psi_0 = sin x
+//   chi_n(x) = -x y_n(x) upward from chi_-1 = -sin x, chi_0 = cos x;   xi_n = psi_n - i chi_n
+//   D_n(mx) = psi_n'/psi_n downward from a start well above n_max (stable for absorbing m)
+//   a_n = [(D_n/m + n/x) psi_n - psi_n-1] / [(D_n/m + n/x) xi_n - xi_n-1]
+//   b_n = [(m D_n + n/x) psi_n - psi_n-1] / [(m D_n + n/x) xi_n - xi_n-1]
+#include "pdv_optics.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+
+namespace pdv {
+
+using cplx = std::complex<double>;
+static const double kPi = 3.14159265358979323846;
+
+static int mie_n_max(double x) { return (int)std::ceil(x + 4.0 * std::cbrt(x) + 2.0); }
+
+static void mie_ab(double x, cplx m, std::vector<cplx> &a, std::vector<cplx> &b) {
+    const int n_max = mie_n_max(x);
+    const cplx z = m * x;
+    const int n_start = (int)std::max((double)n_max, std::abs(z)) + 16;
+    std::vector<cplx> D(n_start + 1, cplx(0.0, 0.0));
+    for (int n = n_start; n >= 1; --n) {
+        const cplx nz = (double)n / z;
+        D[n - 1] = nz - 1.0 / (D[n] + nz);
+    }
+    a.assign(n_max, cplx());
+    b.assign(n_max, cplx());
+    double psi_m = std::cos(x), psi_0 = std::sin(x);     // psi_{n-2}, psi_{n-1}
+    double chi_m = -std::sin(x), chi_0 = std::cos(x);
+    for (int n = 1; n <= n_max; ++n) {
+        const double f = (2.0 * n - 1.0) / x;
+        const double psi = f * psi_0 - psi_m;
+        const double chi = f * chi_0 - chi_m;
+        const cplx xi(psi, -chi), xi_0(psi_0, -chi_0);
+        const cplx ta = D[n] / m + (double)n / x;
+        const cplx tb = D[n] * m + (double)n / x;
+        a[n - 1] = (ta * psi - psi_0) / (ta * xi - xi_0);
+        b[n - 1] = (tb * psi - psi_0) / (tb * xi - xi_0);
+        psi_m = psi_0; psi_0 = psi;
+        chi_m = chi_0; chi_0 = chi;
+    }
+}
+
+void mie_coefficients(double x, double m_re, double m_im, std::vector<double> &a_re, std::vector<double> &a_im,
+                      std::vector<double> &b_re, std::vector<double> &b_im) {
+    std::vector<cplx> a, b;
+    mie_ab(x, cplx(m_re, m_im), a, b);
+    const size_t n = a.size();
+    a_re.resize(n); a_im.resize(n); b_re.resize(n); b_im.resize(n);
+    for (size_t i = 0; i < n; ++i) {
+        a_re[i] = a[i].real(); a_im[i] = a[i].imag(); b_re[i] = b[i].real(); b_im[i] = b[i].imag();
+    }
+}
+
+void mie_efficiencies(double x, double m_re, double m_im, double *k_ext, double *k_sca, double *g) {
+    std::vector<cplx> a, b;
+    mie_ab(x, cplx(m_re, m_im), a, b);
+    const int N = (int)a.size();
+    double se = 0.0, ss = 0.0, sg = 0.0;
+    for (int n = 1; n <= N; ++n) {
+        const cplx an = a[n - 1], bn = b[n - 1];
+        se += (2.0 * n + 1.0) * (an + bn).real();                             // Eq. 12, K_ext
+        ss += (2.0 * n + 1.0) * (std::norm(an) + std::norm(bn));               // Eq. 12, K_sca
+        sg += (2.0 * n + 1.0) / (n * (n + 1.0)) * (an * std::conj(bn)).real();
+        if (n < N)
+            sg += n * (n + 2.0) / (n + 1.0) * (an * std::conj(a[n]) + bn * std::conj(b[n])).real();
+    }
+    const double c = 2.0 / (x * x);
+    if (k_ext) *k_ext = c * se;
+    if (k_sca) *k_sca = c * ss;
+    if (g) *g = (ss > 0.0) ? 2.0 * sg / ss : 0.0;      // g = (4/(x^2 K_sca)) sg with K_sca = c ss
+}
+
+// |S1|^2 + |S2|^2 at mu (Eq. 13-14) with pi_n, tau_n by upward recurrence.
+static double mie_intensity(const std::vector<cplx> &a, const std::vector<cplx> &b, double mu) {
+    double pi_prev = 0.0, pi_cur = 1.0;                 // pi_0, pi_1
+    cplx s1(0.0, 0.0), s2(0.0, 0.0);
+    const int N = (int)a.size();
+    for (int n = 1; n <= N; ++n) {
+        const double tau = n * mu * pi_cur - (n + 1.0) * pi_prev;
+        const double f = (2.0 * n + 1.0) / (n * (n + 1.0));
+        s1 += f * (a[n - 1] * pi_cur + b[n - 1] * tau);
+        s2 += f * (a[n - 1] * tau + b[n - 1] * pi_cur);
+        const double pi_next = ((2.0 * n + 1.0) * mu * pi_cur - (n + 1.0) * pi_prev) / n;
+        pi_prev = pi_cur; pi_cur = pi_next;
+    }
+    return std::norm(s1) + std::norm(s2);
+}
+
+void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M) {
+    std::vector<cplx> a, b;
+    mie_ab(x, cplx(m_re, m_im), a, b);
+    // psi = pi - theta in [0, pi]; mu = -cos(psi) increases with psi; density in psi: I(mu) sin(psi).
+    const int n_panel = std::max(16384, (int)std::ceil(300.0 * x));   // Simpson panels of two intervals
+    const int N = 2 * n_panel;
+    const double h = kPi / N;
+    std::vector<double> gv(N + 1);
+    for (int i = 0; i <= N; ++i) {
+        const double psi = i * h;
+        gv[i] = mie_intensity(a, b, -std::cos(psi)) * std::sin(psi);
+    }
+    std::vector<double> C(n_panel + 1);                 // cumulative integral at even nodes
+    C[0] = 0.0;
+    for (int p = 0; p < n_panel; ++p)
+        C[p + 1] = C[p] + (h / 3.0) * (gv[2 * p] + 4.0 * gv[2 * p + 1] + gv[2 * p + 2]);
+    const double total = C[n_panel];
+    M[0] = -1.0;
+    M[K] = 1.0;
+    int p = 0;
+    for (int k = 1; k < K; ++k) {
+        const double target = total * (double)k / (double)K;
+        while (p + 1 < n_panel && C[p + 1] <= target) ++p;
+        // inside panel p the integrand is the parabola through its three nodes; Q(s) is its exact integral
+        const double g0 = gv[2 * p], g1 = gv[2 * p + 1], g2 = gv[2 * p + 2];
+        const double c1 = (-3.0 * g0 + 4.0 * g1 - g2) / (2.0 * h), c2 = (g0 - 2.0 * g1 + g2) / (2.0 * h * h);
+        const double want = target - C[p];
+        double lo = 0.0, hi = 2.0 * h, s = hi * want / std::max(C[p + 1] - C[p], 1e-300);
+        for (int it = 0; it < 60; ++it) {
+            const double Q = s * (g0 + s * (c1 / 2.0 + s * c2 / 3.0)) - want;
+            if (Q > 0.0) hi = s; else lo = s;
+            const double dQ = g0 + s * (c1 + s * c2);
+            double sn = (dQ > 0.0) ? s - Q / dQ : 0.5 * (lo + hi);
+            if (!(sn > lo && sn < hi)) sn = 0.5 * (lo + hi);
+            if (std::fabs(sn - s) < 1e-16 * h) { s = sn; break; }
+            s = sn;
+        }
+        M[k] = -std::cos(2 * p * h + s);
+    }
+    for (int k = 1; k <= K; ++k)                        // enforce monotone (guards rounding at sharp lobes)
+        if (M[k] < M[k - 1]) M[k] = M[k - 1];
+}
+
+// Standard normal CDF.
+static double norm_cdf(double x) { return 0.5 * std::erfc(-x / std::sqrt(2.0)); }
+
+pdv_status lognormal_classes(double d_median, double sigma_ln, int n, double *diameter, double *weight, int *n_out) {
+    if (!diameter || !weight || !(d_median > 0.0) || !(sigma_ln >= 0.0)) return PDV_E_INVALID;
+    if (sigma_ln == 0.0) {
+        diameter[0] = d_median; weight[0] = 1.0;
+        if (n_out) *n_out = 1;
+        return PDV_OK;
+    }
+    if (n < 1) return PDV_E_INVALID;
+    const double lo = -3.0, hi = 3.0 + 3.0 * sigma_ln, w = (hi - lo) / n;
+    double sum = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const double e0 = lo + i * w, e1 = lo + (i + 1) * w;
+        diameter[i] = d_median * std::exp(sigma_ln * 0.5 * (e0 + e1));
+        weight[i] = norm_cdf(e1) - norm_cdf(e0);
+        sum += weight[i];
+    }
+    for (int i = 0; i < n; ++i) weight[i] /= sum;
+    if (n_out) *n_out = n;
+    return PDV_OK;
+}
+
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::string &err) {
+    auto bad = [&](const char *msg) { err = msg; return PDV_E_INVALID; };
+    if (!(p.area_mass >= 0.0) || !std::isfinite(p.area_mass)) return bad("area_mass must be >= 0");
+    if (!(p.density > 0.0)) return bad("density must be > 0");
+    if (!(p.v_fs > 0.0)) return bad("v_fs must be > 0");
+    if (!(p.vmax_ratio > 1.0) || !std::isfinite(p.vmax_ratio)) return bad("vmax_ratio must be > 1");
+    if (p.profile_kind != 0 && p.profile_kind != 1) return bad("profile_kind must be 0 or 1");
+    if (p.profile_kind == 0 && !(p.beta > 0.0)) return bad("beta must be > 0");
+    if (p.n_classes < 1 || p.n_classes > PDV_MAX_CLASSES) return bad("n_classes out of range");
+    if (!p.diameter || !p.number_weight) return bad("diameter / number_weight is NULL");
+    if (!(p.wavelength > 0.0)) return bad("wavelength must be > 0");
+    if (!(p.m_im >= 0.0) || !(p.m_re > 0.0)) return bad("refractive index: m_re > 0, m_im >= 0");
+    if (!(p.surface_reflectivity >= 0.0 && p.surface_reflectivity <= 1.0)) return bad("surface_reflectivity not in [0,1]");
+    if (p.surface_model != 0 && p.surface_model != 1) return bad("surface_model must be 0 or 1");
+    if (p.phase_model != 0 && p.phase_model != 1) return bad("phase_model must be 0 or 1");
+    const int K = p.n_phase_bins == 0 ? 1024 : p.n_phase_bins;
+    const int nd = p.n_depth_bins == 0 ? 1024 : p.n_depth_bins;
+    if (!is_pow2(K) || K < 16 || K > 4096) return bad("n_phase_bins must be a power of two in [16, 4096]");
+    if (nd < 1 || nd > 4096) return bad("n_depth_bins must be in [1, 4096]");
+    double wsum = 0.0;
+    for (int c = 0; c < p.n_classes; ++c) {
+        if (!(p.diameter[c] > 0.0) || !(p.number_weight[c] > 0.0) || !std::isfinite(p.number_weight[c]))
+            return bad("diameters and number weights must be > 0");
+        if (kPi * p.diameter[c] / p.wavelength > 2000.0) return bad("size parameter above 2000 not supported");
+        wsum += p.number_weight[c];
+    }
+    if (p.profile_kind == 1) {
+        if (p.n_prof < 2 || !p.prof_v || !p.prof_cum_mass) return bad("tabulated profile needs n_prof >= 2 points");
+        for (int i = 1; i < p.n_prof; ++i)
+            if (!(p.prof_v[i] > p.prof_v[i - 1]) || !(p.prof_cum_mass[i] >= p.prof_cum_mass[i - 1]))
+                return bad("profile table must have increasing v and non-decreasing cumulative mass");
+        if (!(p.prof_cum_mass[p.n_prof - 1] > p.prof_cum_mass[0])) return bad("profile table carries no mass");
+    }
+
+    HostCloud h;
+    h.n_classes = p.n_classes; h.K = K; h.n_depth = nd;
+    h.v_fs = p.v_fs; h.v_max = p.vmax_ratio * p.v_fs; h.R = p.surface_reflectivity; h.surface_model = p.surface_model;
+    h.diameter.assign(p.diameter, p.diameter + p.n_classes);
+    h.weight.resize(p.n_classes);
+    for (int c = 0; c < p.n_classes; ++c) h.weight[c] = p.number_weight[c] / wsum;
+    h.k_ext.resize(p.n_classes); h.k_sca.resize(p.n_classes); h.g.resize(p.n_classes); h.p_class.resize(p.n_classes);
+    h.phase.resize((size_t)p.n_classes * (K + 1));
+    double s_ext = 0.0, s_d3 = 0.0, s_d2 = 0.0;
+    for (int c = 0; c < p.n_classes; ++c) {
+        const double d = h.diameter[c], x = kPi * d / p.wavelength;
+        int same = -1;                                   // identical diameters share a table
+        for (int e = 0; e < c; ++e) if (h.diameter[e] == d) { same = e; break; }
+        if (same >= 0) {
+            h.k_ext[c] = h.k_ext[same]; h.k_sca[c] = h.k_sca[same]; h.g[c] = h.g[same];
+            std::copy(h.phase.begin() + (size_t)same * (K + 1), h.phase.begin() + (size_t)(same + 1) * (K + 1),
+                      h.phase.begin() + (size_t)c * (K + 1));
+        } else {
+            mie_efficiencies(x, p.m_re, p.m_im, &h.k_ext[c], &h.k_sca[c], &h.g[c]);
+            double *M = &h.phase[(size_t)c * (K + 1)];
+            if (p.phase_model == 1) {
+                for (int k = 0; k <= K; ++k) M[k] = -1.0 + 2.0 * (double)k / (double)K;
+                h.g[c] = 0.0;
+            } else {
+                mie_phase_quantiles(x, p.m_re, p.m_im, K, M);
+            }
+        }
+        if (!(h.k_ext[c] > 0.0) || !std::isfinite(h.k_ext[c])) return bad("Mie series failed (K_ext not positive)");
+        s_ext += h.weight[c] * d * d * h.k_ext[c];
+        s_d3 += h.weight[c] * d * d * d;
+        s_d2 += h.weight[c] * d * d;
+    }
+    for (int c = 0; c < p.n_classes; ++c)
+        h.p_class[c] = h.weight[c] * h.diameter[c] * h.diameter[c] * h.k_ext[c] / s_ext;       // Eq. 8 sums
+    h.kappa = 3.0 * s_ext / (2.0 * p.density * s_d3);                                         // Eq. 10
+    h.tau_ext = h.kappa * p.area_mass;
+    h.sauter = s_d3 / s_d2;
+
+    // depth table: fraction of the mass above v_j = v_max - j dv
+    h.T_edge.resize(nd + 1);
+    const double dv = (h.v_max - h.v_fs) / nd;
+    if (p.profile_kind == 0) {
+        const double bv = p.beta / p.v_fs;
+        const double span = std::expm1(bv * (h.v_max - h.v_fs));   // (e^{-b(v-vfs)} - E)/(1-E) = expm1(b(vmax-v))/expm1(b(vmax-vfs))
+        for (int j = 0; j <= nd; ++j) h.T_edge[j] = h.tau_ext * std::expm1(bv * (j * dv)) / span;
+    } else {
+        const double m_lo = p.prof_cum_mass[0], m_hi = p.prof_cum_mass[p.n_prof - 1];
+        int seg = p.n_prof - 2;
+        for (int j = 0; j <= nd; ++j) {
+            double v = h.v_max - j * dv;
+            v = std::min(std::max(v, p.prof_v[0]), p.prof_v[p.n_prof - 1]);
+            while (seg > 0 && p.prof_v[seg] > v) --seg;
+            const double f = (v - p.prof_v[seg]) / (p.prof_v[seg + 1] - p.prof_v[seg]);
+            const double cm = p.prof_cum_mass[seg] + f * (p.prof_cum_mass[seg + 1] - p.prof_cum_mass[seg]);
+            h.T_edge[j] = h.tau_ext * (m_hi - cm) / (m_hi - m_lo);
+        }
+    }
+    h.T_edge[0] = 0.0;
+    h.T_edge[nd] = h.tau_ext;
+    for (int j = 1; j <= nd; ++j) if (h.T_edge[j] < h.T_edge[j - 1]) h.T_edge[j] = h.T_edge[j - 1];
+    out = std::move(h);
+    return PDV_OK;
+}
+
+}  // namespace pdv
