@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Monte-Carlo PDV hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl b200|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one
+pdv_mc_run of BASELINE.json configs[I] (default I = 1: 2 mg/cm^2 tin cloud, 1e8 photons, 512 bins, t = 3 us)
+followed by pdv_spectrogram.  Every step uses a new seed.  Rank 0 prints ONE JSON line.
+
+  value      scattering events/s (particle interactions, BASELINE.json "metric"), whole job, cloud tables resident in
+             HBM and outputs left in HBM, timed with CUDA events on the launching stream (max over ranks)
+  e2e        the same metric through the host-buffer C-ABI calls a user makes: pdv_cloud_create (host Mie tables + H2D)
+             + pdv_mc_run into host arrays (D2H inside) + pdv_spectrogram on host arrays, wall clock
+  roofline   transport kernel against the instruction-issue peak (bound "alu": no HBM traffic, no contraction)
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores, bounded sample of the same workload
+
+--impl reference times the oracle itself (there is no reference code).
+N > 1: weak scaling, rank r runs the same number of histories on photon ids [r n, (r+1) n); one all-reduce of the
+tallies per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import pdv_workloads as W  # noqa: E402
+
+METRIC = "scattering events/s"
+UNIT = "events/s"
+N_SM_B200 = 148
+
+# Algorithmic thread-instructions of ONE flight (one Philox block + free flight + interaction / reflection / exit) on the
+# common path, counted from the method's operations, not from what the compiler emitted (DESIGN.md "Roofline",
+# table "algorithmic instructions per flight").  A particle event, a surface reflection and the final exit flight are
+# one flight each.
+ALG_INST_PER_FLIGHT = {"scatter": 96, "reflect": 70, "exit": 64}
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+# ---------------------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU with NVML every 50 ms while the timed region runs."""
+
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int, uuid: str | None = None):
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            try:
+                self._h = pynvml.nvmlDeviceGetHandleByUUID(uuid if uuid.startswith("GPU-") else "GPU-" + uuid)
+            except Exception:
+                self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(n for b, n in self.REASONS.items() if self.reason_bits & b),
+                "samples": len(self.samples), "power_w_max": max(self.power) if self.power else None}
+
+
+# ------------------------------------------------------------------------------------------------------ CPU oracle
+def oracle_timed(cfg: dict, seconds: float, seed: int):
+    """Times the oracle, as it stands, on all host cores for about `seconds` of work on unit 0 of `cfg`."""
+    from oracle import cloud as ocloud
+    from oracle import mc as omc
+    omc.build()
+    oc = ocloud.build_cloud(cfg["clouds"][0])
+    cores = os.cpu_count() or 1
+    run = dict(cfg["run"], seed=seed)
+    n0 = 200_000
+    t = time.perf_counter()
+    omc.run(oc, run, n_photons=n0, n_threads=cores)
+    dt = max(time.perf_counter() - t, 1e-3)
+    n = int(min(max(n0, seconds * n0 / dt), cfg["run"]["n_photons"]))
+    t = time.perf_counter()
+    r = omc.run(oc, run, n_photons=n, n_threads=cores, first_id=n0)
+    dt = time.perf_counter() - t
+    return dict(n=n, seconds=dt, events=int(r.stats["particle_events"]), cores=cores)
+
+
+def run_reference(args):
+    """`--impl reference`: the oracle timed on the host cores, each step a bounded sample of the workload."""
+    rank = _env_int("RANK", 0)
+    if rank != 0:
+        return
+    from oracle import cloud as ocloud
+    from oracle import mc as omc
+    omc.build()
+    cfg = W.config(args.config)
+    oc = ocloud.build_cloud(cfg["clouds"][0])
+    cores = os.cpu_count() or 1
+    n = int(min(args.ref_photons, cfg["run"]["n_photons"]))
+    ev = 0
+    for i in range(args.warmup):
+        omc.run(oc, dict(cfg["run"], seed=1000 + i), n_photons=n, n_threads=cores)
+    t = time.perf_counter()
+    for i in range(args.steps):
+        ev += int(omc.run(oc, dict(cfg["run"], seed=2000 + i), n_photons=n, n_threads=cores).stats["particle_events"])
+    dt = time.perf_counter() - t
+    val = ev / dt
+    sample = f"unit 0 of {cfg['name']}: {n} histories per step (of {cfg['run']['n_photons']}), {args.steps} steps"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "histories_per_step": n, "n_bins": cfg["run"]["n_bins"]},
+        "histories_per_s": n * args.steps / dt,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ------------------------------------------------------------------------------------------------------- GPU arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1 = headline)")
+    ap.add_argument("--photons", type=int, default=0, help="override histories per unit (debugging; invalidates the number)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--ref-photons", type=int, default=2_000_000, help="--impl reference: histories per step")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work of the cpu_baseline leg (0: skip)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-buffer leg (0: same as --steps)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2012_00963_b200 as P
+    from paper_2012_00963_b200._shard import allreduce_tallies
+
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    cfg = W.config(args.config)
+    run = dict(cfg["run"])
+    n = int(args.photons or run["n_photons"])
+    run["first_photon_id"] = rank * n                       # weak scaling: disjoint id ranges, same count per rank
+    nb, t_snap = run["n_bins"], cfg["t_snap"]
+    clouds = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
+    nc, ns = len(clouds), len(t_snap)
+    n_units = nc * ns
+    hist = torch.zeros((nc, ns, nb), dtype=torch.float64, device=dev)
+    hist2 = torch.zeros_like(hist)
+    stats = torch.zeros(n_units * P.STATS_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(i):
+        P.pdv_mc_run_device(clouds, t_snap, n, run["seed"] + 7919 * i, run, hist, hist2, stats, stream=stream.cuda_stream)
+        if world > 1:
+            allreduce_tallies(hist, hist2)
+        return P.pdv_spectrogram(hist.view(n_units, nb), n * world, run["v_lo"], run["v_hi"], scale=2,
+                                 stream=stream.cuda_stream)
+
+    def read_stats():
+        return np.frombuffer(stats.cpu().numpy().tobytes(), dtype=P.STATS_DTYPE)
+
+    for i in range(args.warmup):
+        flush.zero_()
+        step(i)
+    barrier()
+
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    tot = dict(particle_events=0, surface_reflections=0, histories=0)
+    transport_ms = []
+    with ClockSampler(local, str(getattr(torch.cuda.get_device_properties(local), "uuid", ""))) as clk:
+        barrier()
+        for i in range(args.steps):
+            flush.zero_()                                    # L2 flush between timed iterations (outside the events)
+            ev0[i].record(stream)
+            step(args.warmup + i)
+            ev1[i].record(stream)
+            transport_ms.append(P.pdv_last_launch_info()["transport_ms"])      # waits for this step's kernel
+            s = read_stats()
+            for k in tot:
+                tot[k] += int(s[k].sum())
+        barrier()
+    step_ms = sum(a.elapsed_time(b) for a, b in zip(ev0, ev1))
+    info = P.pdv_last_launch_info()
+    t_all = torch.tensor([step_ms, sum(transport_ms)], dtype=torch.float64, device=dev)
+    cnt = torch.tensor([tot["particle_events"], tot["surface_reflections"], tot["histories"]], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    step_ms, tr_ms = (float(x) for x in t_all.cpu())
+    events, reflections, histories = (float(x) for x in cnt.cpu())
+    value = events / (step_ms * 1e-3)
+
+    # ---- end to end through the host-buffer API (every step: host Mie tables + H2D, run, D2H, spectrogram) -------------
+    k_e2e = args.e2e_steps or args.steps
+    e2e_events = 0
+
+    def e2e_step(i):
+        cl = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
+        r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run)
+        sp = P.pdv_spectrogram(r.hist.reshape(n_units, nb), n, run["v_lo"], run["v_hi"], scale=2)
+        for c in cl:
+            c.destroy()
+        return int(r.stats["particle_events"].sum()), sp
+
+    for i in range(2):
+        e2e_step(-1 - i)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(k_e2e):
+        e2e_events += e2e_step(i)[0]
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    e2e_c = torch.tensor([float(e2e_events)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(e2e_c, op=dist.ReduceOp.SUM)
+    blob_bytes = info["smem_bytes"] - 16 * nb                                   # largest cloud image staged per block
+    h2d = nc * blob_bytes + 16 * n_units + 8 * n_units * nb                     # tables + unit table + hist (spectrogram)
+    d2h = 2 * 8 * n_units * nb + n_units * P.STATS_DTYPE.itemsize + 4 * n_units * nb
+
+    # ---- roofline of the transport kernel: instruction issue ---------------------------------------------------------
+    peaks = P.pdv_issue_peaks(30.0) if rank == 0 else None
+    out = None
+    if rank == 0:
+        clocks = clk.summary()
+        sm_max = clocks["sm_max_mhz"] or 1965.0
+        n_sm = peaks["n_sm"]
+        issue_peak = n_sm * 4 * 32 * sm_max * 1e6                               # 1 warp-instruction / clk / sub-partition
+        a = ALG_INST_PER_FLIGHT
+        alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
+        achieved = alg / (tr_ms * 1e-3)
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "transport_thread_inst.json")     # written by hand from the ncu capture
+        if os.path.exists(tpath):
+            with open(tpath) as f:
+                tj = json.load(f)
+            if tj.get("workload") == cfg["name"] and tj.get("histories_per_launch") == n:
+                traffic = tj.get("thread_inst_executed_per_launch")
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units,
+                       "n_bins": nb, "parallelism": f"photon-id ranges x{world}", "l2": "flushed between steps (256 MiB write)",
+                       "events_per_history": events / histories, "reflections_per_history": reflections / histories},
+            "histories_per_s": histories / (step_ms * 1e-3),
+            "events_incl_surface_per_s": (events + reflections) / (step_ms * 1e-3),
+            "gpu_launches": 3 * args.steps,                 # transport + finalize + spectrogram kernels per step
+            "launch": {"grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
+                       "transport_ms_per_step": tr_ms / args.steps},
+            "clocks": clocks,
+            "e2e": {"value": float(e2e_c) / float(e2e_t), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": k_e2e, "ms_per_step": 1e3 * float(e2e_t) / k_e2e,
+                    "includes": "pdv_cloud_create (host Mie + tables + H2D), pdv_mc_run (host outputs), pdv_spectrogram"},
+            "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12, "unit": "Tthread-inst/s",
+                         "frac": achieved / issue_peak, "traffic": traffic,
+                         "peak_is": f"{n_sm} SMs x 4 sub-partitions x 32 lanes x {sm_max:.0f} MHz (DESIGN.md), not in MEASURED_PEAKS.json",
+                         "kernel": "pdv::transport_kernel",
+                         "alg_inst_per_flight": a,
+                         "measured_ffma_Tinst_s": peaks["ffma_thread_inst_per_s"] / 1e12,
+                         "measured_mufu_Tinst_s": peaks["mufu_thread_inst_per_s"] / 1e12,
+                         "frac_of_measured_ffma": achieved / peaks["ffma_thread_inst_per_s"],
+                         "sm_clock_mhz_in_microbench": peaks["sm_clock_mhz"]},
+        }
+        if args.cpu_seconds > 0:
+            o = oracle_timed(cfg, args.cpu_seconds, seed=97)
+            out["cpu_baseline"] = {"value": o["events"] / o["seconds"], "unit": UNIT, "cores": o["cores"], "kind": "oracle",
+                                   "histories_per_s": o["n"] / o["seconds"],
+                                   "sample": f"unit 0 of {cfg['name']}: {o['n']} histories in {o['seconds']:.1f} s"}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if out is not None:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

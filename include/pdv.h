@@ -193,8 +193,8 @@ pdv_status pdv_issue_peaks(double millis, double *ffma_thread_inst_per_s, double
                            double *sm_clock_mhz, int32_t *n_sm, void *cuda_stream);
 
 /* Launch statistics of the last pdv_mc_run / pdv_mc_trace on this thread: kernels launched and the duration of
- * the transport kernel in ms measured with CUDA events on cuda_stream (0 when output_on_device = 1, where
- * nothing is synchronised).  Any pointer may be NULL. */
+ * the transport kernel in ms measured with CUDA events on cuda_stream.  After an output_on_device = 1 run this
+ * call waits (cudaEventSynchronize) for that run's transport kernel to finish.  Any pointer may be NULL. */
 pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block,
                                 int32_t *smem_bytes);
 

@@ -23,7 +23,7 @@ struct pdv_cloud {
 namespace {
 
 thread_local std::string g_err;
-thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0; } g_last;
+thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0; bool pending = false; } g_last;
 
 struct Workspace {
     unsigned char *d = nullptr;
@@ -298,7 +298,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     rp.stats = reinterpret_cast<unsigned long long *>(ws + o_stats);
     rp.trace = d_trace;
 
-    g_last.n_kernels = 0; g_last.ms = 0.f;
+    g_last.n_kernels = 0; g_last.ms = 0.f; g_last.pending = false;
     g_last.grid = plan.shape.grid; g_last.block = plan.shape.block; g_last.smem = plan.shape.smem;
     CUX(cudaEventRecord(g_ws.e0, st), "cudaEventRecord");
     if (n_photons > 0) {
@@ -306,6 +306,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
         g_last.n_kernels += 1;
     }
     CUX(cudaEventRecord(g_ws.e1, st), "cudaEventRecord");
+    g_last.pending = true;               // elapsed time is read when the events have completed
 
     const bool dev_out = o->output_on_device != 0;
     double *oh = dev_out ? hist : reinterpret_cast<double *>(ws + o_oh);
@@ -325,6 +326,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
         if (trace && n_photons) CUX(cudaMemcpy(records, d_trace, sizeof(pdv_trace_record) * n_photons, cudaMemcpyDeviceToHost), "read back trace");
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, g_ws.e0, g_ws.e1) == cudaSuccess) g_last.ms = ms;
+        g_last.pending = false;
         std::memcpy(hist, th.data(), 8 * nb * n_units);
         if (hist2) std::memcpy(hist2, th2.data(), 8 * nb * n_units);
         if (stats) std::memcpy(stats, ts.data(), sizeof(pdv_run_stats) * n_units);
@@ -509,6 +511,14 @@ pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mh
 }
 
 pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes) {
+    if (g_last.pending && g_ws.e0 && g_ws.e1) {      // output_on_device run: wait for its transport kernel only
+        float ms = 0.f;
+        if (cudaEventSynchronize(g_ws.e1) == cudaSuccess && cudaEventElapsedTime(&ms, g_ws.e0, g_ws.e1) == cudaSuccess)
+            g_last.ms = ms;
+        else
+            cudaGetLastError();
+        g_last.pending = false;
+    }
     if (n_kernels) *n_kernels = g_last.n_kernels;
     if (transport_ms) *transport_ms = g_last.ms;
     if (grid) *grid = g_last.grid;
