@@ -59,45 +59,66 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     int steps = 0;
     while ((1 << steps) < nc) ++steps;
     const int n_pad = 1 << steps;
-    // fp32 depth table
+    // fp32 depth edges, T_0 = 0 at the cloud top ... T_nd = tau_ext at the free surface, non-decreasing
     std::vector<float> Tf(nd + 1);
     for (int j = 0; j <= nd; ++j) Tf[j] = (float)h.T_edge[j];
     Tf[0] = 0.f;
     for (int j = 1; j <= nd; ++j) if (Tf[j] < Tf[j - 1]) Tf[j] = Tf[j - 1];
-    // guide over (float bits >> 16): exponent + 7 mantissa bits, i.e. 128 cells per octave of T
+    // depth rows (layout: pdv_device.h).  Half velocities: the Doppler update is  v~ += (mu' - mu) v/2  (Eq. 4).
+    const double dv = (h.v_max - h.v_fs) / nd;
+    std::vector<float> slope(nd + 1, 0.f);                    // d(v/2)/dT inside bin j; 0 for an empty bin
+    for (int j = 0; j < nd; ++j) {
+        const double dT = (double)Tf[j + 1] - (double)Tf[j];
+        slope[j] = dT > 0.0 ? (float)(-0.5 * dv / dT) : 0.f;
+    }
+    // guide over (float bits >> shift): the coarsest shift for which no cell straddles two bin edges
     float t_min = 0.f;
     for (int j = 1; j <= nd; ++j) if (Tf[j] > 0.f) { t_min = Tf[j]; break; }
-    uint32_t base = 0, n_guide = 1;
+    uint32_t base = 0, n_guide = 1, shift = 16, bisect = 0;
+    std::vector<uint16_t> guide(1, (uint16_t)(nd - 1));       // tau_ext = 0: every lookup is at the surface
     if (t_min > 0.f) {
-        const uint32_t top = f2u(Tf[nd]) >> 16;
-        base = f2u(t_min) >> 16;
-        if (top - base + 1 > 8192u) base = top - 8191u;
-        n_guide = top - base + 1;
-    }
-    std::vector<uint16_t> guide(n_guide, 0);
-    {
-        int j = 0;
-        for (uint32_t i = 1; i < n_guide; ++i) {          // guide[0] = 0: cell 0 also serves every T below it
-            const float lo = u2f((base + i) << 16);
-            while (j + 1 <= nd - 1 && Tf[j + 1] <= lo) ++j;
-            guide[i] = (uint16_t)j;
+        bool ok = false;
+        for (shift = 16; shift >= 10 && !ok; --shift) {
+            const uint32_t top = f2u(Tf[nd]) >> shift;
+            base = f2u(t_min) >> shift;
+            n_guide = top - base + 1;
+            if (n_guide > 16384u) break;
+            guide.assign(n_guide, 0);
+            int j = 0;
+            ok = true;
+            for (uint32_t i = 0; i < n_guide; ++i) {
+                if (i > 0) {                                  // cell 0 also serves every T below it: j = 0
+                    const float lo = u2f((base + i) << shift);
+                    while (j + 1 <= nd - 1 && Tf[j + 1] <= lo) ++j;
+                }
+                guide[i] = (uint16_t)j;
+                const float hi = u2f(((base + i + 1) << shift) - 1u);
+                if (j + 2 < nd && !(Tf[j + 2] > hi)) ok = false;      // a second inner edge inside the cell (T_nd = tau_ext may be)
+            }
+            if (ok) break;
+        }
+        if (!ok) {                                            // pathological table: coarse guide unused, kernel bisects
+            bisect = 1; shift = 16;
+            base = f2u(t_min) >> shift;
+            n_guide = (f2u(Tf[nd]) >> shift) - base + 1;
+            guide.assign(n_guide, 0);
         }
     }
     DevCloudHeader hd;
     std::memset(&hd, 0, sizeof(hd));
     size_t off = sizeof(DevCloudHeader);
     hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * (size_t)nc * (K + 1));
-    hd.off_tedge = (uint32_t)off;  off = align16(off + sizeof(float) * (nd + 2));
+    hd.off_rows = (uint32_t)off;   off = align16(off + sizeof(float) * 4 * (size_t)nd);
     hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
     hd.blob_bytes = (uint32_t)off;
     hd.n_classes = nc; hd.K = K; hd.n_depth = nd; hd.n_guide = n_guide; hd.guide_base = base;
+    hd.guide_shift = shift; hd.depth_bisect = bisect;
     hd.log2K = 0;
     while ((1 << hd.log2K) < K) ++hd.log2K;
-    hd.tau_ext = Tf[nd]; hd.v_fs = (float)h.v_fs; hd.v_max = (float)h.v_max;
-    hd.dv_depth = (float)((h.v_max - h.v_fs) / nd);
+    hd.tau_ext = Tf[nd]; hd.vh_fs = (float)(0.5 * h.v_fs);
     hd.R_q31 = (uint32_t)std::llround(h.R * 2147483648.0);
     hd.R_thr = to_thr32(h.R);
     hd.surface_model = (uint32_t)h.surface_model;
@@ -113,9 +134,13 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
             prev = v;
         }
     }
-    float *te = reinterpret_cast<float *>(blob.data() + hd.off_tedge);
-    for (int j = 0; j <= nd; ++j) te[j] = Tf[j];
-    te[nd + 1] = Tf[nd];
+    float *rows = reinterpret_cast<float *>(blob.data() + hd.off_rows);
+    for (int j = 0; j < nd; ++j) {
+        rows[4 * j + 0] = Tf[j + 1];
+        rows[4 * j + 1] = j + 1 == nd ? hd.vh_fs : (float)(0.5 * (h.v_max - (j + 1) * dv));
+        rows[4 * j + 2] = slope[j];
+        rows[4 * j + 3] = slope[j + 1];
+    }
     uint32_t *thr = reinterpret_cast<uint32_t *>(blob.data() + hd.off_thr);
     uint32_t *alb = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albedo);
     uint32_t *albt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albthr);
@@ -170,8 +195,23 @@ pdv_status get_workspace(size_t bytes, int device, unsigned char **out) {
 struct RunPlan {
     RunParams rp;
     LaunchShape shape;
-    bool poly, analog;
+    KernelVariant variant;
 };
+
+struct DeviceInfo { int n_sm = 0; size_t smem_optin = 0; bool valid = false; };
+const DeviceInfo &device_info(int device) {           // cudaGetDeviceProperties costs milliseconds: ask once per device
+    static std::mutex mu;
+    static DeviceInfo info[64];
+    std::lock_guard<std::mutex> lk(mu);
+    DeviceInfo &d = info[device & 63];
+    if (!d.valid) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device) == cudaSuccess) d.n_sm = v;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) == cudaSuccess) d.smem_optin = (size_t)v;
+        d.valid = d.n_sm > 0;
+    }
+    return d;
+}
 
 pdv_status check_opts(const pdv_run_opts *o) {
     if (!o) return fail(PDV_E_INVALID, "opts is NULL");
@@ -184,8 +224,8 @@ pdv_status check_opts(const pdv_run_opts *o) {
     if (o->max_events < 0) return fail(PDV_E_INVALID, "max_events < 0");
     if (o->max_events > 0 && !(o->roulette_survival > 0.0 && o->roulette_survival <= 1.0))
         return fail(PDV_E_INVALID, "roulette_survival not in (0,1]");
-    if (o->threads_per_block < 0 || o->threads_per_block > 512 || (o->threads_per_block % 32) != 0)
-        return fail(PDV_E_INVALID, "threads_per_block must be a multiple of 32, <= 512");
+    if (o->threads_per_block < 0 || o->threads_per_block > 1024 || (o->threads_per_block % 32) != 0)
+        return fail(PDV_E_INVALID, "threads_per_block must be a multiple of 32, <= 1024");
     if (o->blocks_per_sm < 0 || o->blocks_per_sm > 32) return fail(PDV_E_INVALID, "blocks_per_sm out of range");
     return PDV_OK;
 }
@@ -197,8 +237,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     std::memset(&rp, 0, sizeof(rp));
     rp.n_units = (uint32_t)n_units;
     rp.n_bins = (uint32_t)o->n_bins;
-    rp.max_events = (uint32_t)o->max_events;
-    rp.single_scatter_only = o->single_scatter_only ? 1u : 0u;
+    rp.max_events = o->max_events > 0 ? (uint32_t)o->max_events : 0xFFFFFFFFu;
     const double p = o->max_events > 0 ? o->roulette_survival : 1.0;
     rp.roulette_thr = to_thr32(p);
     rp.roulette_wcap = (uint32_t)std::floor(p * 2147483648.0);
@@ -211,30 +250,47 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) { rp.key0[r] = k0; rp.key1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
 
-    plan.poly = false;
-    for (int i = 0; i < n_clouds; ++i) plan.poly = plan.poly || clouds[i]->host.n_classes > 1;
-    plan.analog = o->mode == 1;
+    KernelVariant &kv = plan.variant;
+    kv.poly = false;
+    for (int i = 0; i < n_clouds; ++i) kv.poly = kv.poly || clouds[i]->host.n_classes > 1;
+    kv.analog = o->mode == 1;
+    kv.sso = o->single_scatter_only != 0;
+    kv.trace = trace;
 
-    cudaDeviceProp prop;
-    CU(cudaGetDeviceProperties(&prop, device), "cudaGetDeviceProperties");
+    const DeviceInfo &di = device_info(device);
+    if (!di.valid) return fail(PDV_E_CUDA, "cannot query the CUDA device");
     const int smem = (int)(16 * (size_t)o->n_bins + max_blob);
-    if ((size_t)smem > (size_t)prop.sharedMemPerBlockOptin)
+    if ((size_t)smem > di.smem_optin)
         return fail(PDV_E_UNSUPPORTED, "cloud tables + histogram exceed the shared memory of one block");
-    int block = o->threads_per_block > 0 ? o->threads_per_block : 512;
-    int per_sm = 0;
-    CU(transport_max_blocks_per_sm(plan.poly, plan.analog, trace, block, smem, &per_sm), "occupancy query");
+    // 1024 resident threads per SM (64 registers each): two blocks of 512 when their shared memory fits twice, else one of 1024
+    int block = o->threads_per_block, per_sm = 0;
+    if (block == 0) block = 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024 ? 512 : 1024;
+    {
+        struct Key { KernelVariant v; int block, smem, device; };
+        static std::mutex mu;
+        static std::vector<std::pair<Key, int>> cache;       // occupancy queries are not free either
+        std::lock_guard<std::mutex> lk(mu);
+        for (const auto &e : cache)
+            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace &&
+                e.first.block == block && e.first.smem == smem && e.first.device == device) { per_sm = e.second; break; }
+        if (per_sm == 0) {
+            CU(transport_max_blocks_per_sm(kv, block, smem, &per_sm), "occupancy query");
+            if (per_sm >= 1) cache.push_back({Key{kv, block, smem, device}, per_sm});
+        }
+    }
     if (per_sm < 1) return fail(PDV_E_UNSUPPORTED, "transport kernel does not fit on an SM with these tables");
     if (o->blocks_per_sm > 0) per_sm = std::min(per_sm, o->blocks_per_sm);
-    long long grid = (long long)prop.multiProcessorCount * per_sm;
+    long long grid = (long long)di.n_sm * per_sm;
     const unsigned long long total = n_photons * (unsigned long long)n_units;
     const long long useful = (long long)((total + block - 1) / block);       // one history per thread at least
     if (useful < grid) grid = std::max(1LL, useful);
     plan.shape.grid = (int)grid; plan.shape.block = block; plan.shape.smem = smem;
-    // chunk: ~16 fetches per warp over the run, between 32 and 4096 ids, multiple of 32
-    const unsigned long long warps = (unsigned long long)grid * (block / 32);
-    unsigned long long chunk = total / (warps * 16ull + 1ull);
-    chunk = std::min<unsigned long long>(std::max<unsigned long long>(chunk, 32ull), 4096ull);
-    rp.chunk = (uint32_t)((chunk + 31ull) & ~31ull);
+    // Guided self-scheduling of photon ids: a lane claims clamp(remaining / (2 * threads on the unit), 1, chunk) ids
+    const double threads = (double)grid * block / std::min<double>((double)n_units, (double)grid);
+    double chunk = std::floor((double)n_photons / (threads * 4.0));
+    chunk = std::min(std::max(chunk, 1.0), 128.0);
+    rp.chunk = (uint32_t)chunk;
+    rp.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
     return PDV_OK;
 }
 
@@ -302,7 +358,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     g_last.grid = plan.shape.grid; g_last.block = plan.shape.block; g_last.smem = plan.shape.smem;
     CUX(cudaEventRecord(g_ws.e0, st), "cudaEventRecord");
     if (n_photons > 0) {
-        CUX(launch_transport(rp, plan.poly, plan.analog, trace, plan.shape, st), "transport kernel launch");
+        CUX(launch_transport(rp, plan.variant, plan.shape, st), "transport kernel launch");
         g_last.n_kernels += 1;
     }
     CUX(cudaEventRecord(g_ws.e1, st), "cudaEventRecord");

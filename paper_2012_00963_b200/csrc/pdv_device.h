@@ -17,14 +17,27 @@ enum StatSlot {
     ST_HISTORIES, ST_EVENTS, ST_REFLECT, ST_MAXEV, ST_COUNT = 16
 };
 
-// Device image of one cloud: one contiguous blob [DevCloudHeader | phase | T_edge | class thr | albedo Q31 | albedo thr | guide],
+// Device image of one cloud: one contiguous blob [DevCloudHeader | phase | depth rows | class thr | albedo Q31 | albedo thr | guide],
 // every section 16-byte aligned, copied verbatim into shared memory by each block.
+//
+// Depth rows (one float4 per depth bin j, bins uniform in v, j = 0 at the cloud top):
+//   x = T_{j+1}                      vertical optical depth of the LOWER edge of bin j
+//   y = v(T_{j+1}) / 2               half the particle velocity at that edge (the Doppler update uses v/2)
+//   z = d(v/2)/dT inside bin j       (0 for an empty bin)
+//   w = d(v/2)/dT inside bin j+1     (0 past the last bin)
+// so that for T_j <= T < T_{j+2}:  v(T)/2 = y + (T - x) * (T < x ? z : w)   -- T linear in v inside each bin
+// (the canonical depth discretisation), one branch-free probe.
+// Guide: cell = (float bits of T) >> guide_shift, minus guide_base; guide[cell] = largest j with T_j <= every T of the
+// cell.  The host picks guide_shift so that no cell straddles two bin edges (then one probe is exact); if it cannot,
+// depth_bisect = 1 and the kernel bisects the rows instead.
 struct DevCloudHeader {
     uint32_t blob_bytes;       // multiple of 16
     uint32_t n_classes, K, log2K, n_depth, n_guide;
-    uint32_t off_phase, off_tedge, off_thr, off_albedo, off_albthr, off_guide;   // byte offsets from the blob start
-    uint32_t guide_base;       // (float bits of T) >> 16 of guide cell 0
-    float tau_ext, v_fs, v_max, dv_depth;
+    uint32_t off_phase, off_rows, off_thr, off_albedo, off_albthr, off_guide;   // byte offsets from the blob start
+    uint32_t guide_base;       // (float bits of T) >> guide_shift of guide cell 0
+    uint32_t guide_shift;
+    uint32_t depth_bisect;
+    float tau_ext, vh_fs;      // vh_fs = v_fs / 2
     uint32_t R_q31;            // surface reflectivity, Q31
     uint32_t R_thr;            // analog mode: reflected iff y1 < R_thr
     uint32_t surface_model;
@@ -47,9 +60,9 @@ struct RunParams {
     pdv_trace_record *trace;           // TRACE only: [n_photons]
     uint32_t n_units;
     uint32_t n_bins;
-    uint32_t chunk;                    // photon ids a warp claims per fetch
-    uint32_t max_events;               // 0: no roulette
-    uint32_t single_scatter_only;
+    uint32_t chunk;                    // photon ids a lane claims per fetch at the start of a unit (guided: shrinks
+    float chunk_per_remaining;         //   to clamp(remaining * chunk_per_remaining, 1, chunk) as the unit drains)
+    uint32_t max_events;               // roulette once n_scatter >= max_events; 0xffffffff: never
     uint32_t roulette_thr;             // survive iff y0 < roulette_thr
     uint32_t roulette_wcap;            // play only while w <= wcap (= floor(p 2^31))
     float roulette_inv_p;
@@ -61,8 +74,9 @@ struct RunParams {
 struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
-cudaError_t launch_transport(const RunParams &rp, bool poly, bool analog, bool trace, LaunchShape shape, cudaStream_t st);
-cudaError_t transport_max_blocks_per_sm(bool poly, bool analog, bool trace, int block, int smem, int *out);
+struct KernelVariant { bool poly, analog, sso, trace; };   // template instantiation of transport_kernel
+cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
+cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,
                             uint32_t n_units, uint32_t n_bins, double *out_hist, double *out_hist2, pdv_run_stats *out_stats,
                             cudaStream_t st);

@@ -1,15 +1,20 @@
 // pdv_kernels.cu -- CUDA kernels of the PDV Monte-Carlo transport for sm_100a (B200).
 //
 // transport_kernel: persistent-thread photon transport, section II.B steps (1)-(7) (174-183):
-//   * one lane = one photon history at a time; dead lanes are re-filled ("photon regeneration") from a chunk of
-//     photon ids the warp claims with one global atomic, so lanes stay busy whatever the history lengths are;
+//   * one lane = one photon history at a time; a lane whose photon left the cloud starts its next history in the
+//     same branch ("photon regeneration"), taking ids from a private chunk it claims from the unit's global counter
+//     (guided chunk sizes: large at the start, 1 at the end), so all 32 lanes of a warp fly a photon in every
+//     iteration until the unit is drained;
 //   * every history draws from its own Philox4x32-10 counter stream, counter = (id_lo, id_hi, unit, 2*flight+sub),
 //     key = seed: results do not depend on which lane, warp or block runs a history (D1/D2);
-//   * the cloud tables (inverse-CDF phase tables, depth table + its guide, class thresholds) live in shared memory;
-//   * free flight in vertical optical depth T (exact sampling of Eq. 7/10), interaction (Eq. 11), scattering angle
-//     from the discretised phase function D_K (Eq. 13-14), azimuth (Eq. 15), direction update (z row of Eq. 16 /
-//     Eq. 17 -- only mu = u_z matters in slab geometry, reading R7), Doppler update (Eq. 4);
-//   * tallies are Q31 integers in a shared-memory histogram, warp-aggregated, flushed once per block and unit.
+//   * the cloud tables (inverse-CDF phase tables, depth rows + guide, class thresholds) live in shared memory;
+//   * one loop iteration = one flight: free flight in vertical optical depth T (exact sampling of Eq. 7/10), then
+//     either the photon leaves through the top (tally, Eq. 19) or it interacts.  Particle scattering (Eq. 11,
+//     13-17) and free-surface reflection run through ONE branch-free instruction stream with
+//     selects: a reflection is "a scatter with albedo R, velocity v_fs and an absolute new direction";
+//   * only mu = u_z is tracked (z row of Eq. 16 / Eq. 17; exact in slab geometry, reading R7);
+//   * Doppler update Eq. 4 with half velocities from the depth rows; weights and tallies are Q31 integers;
+//     the block's private shared-memory histogram is flushed once per block and unit.
 #include "pdv_device.h"
 
 namespace pdv {
@@ -41,6 +46,11 @@ __device__ __forceinline__ float fast_sqrt(float x) {
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+__device__ __forceinline__ float fast_lg2(float x) {       // x is a normal number here: no denormal fix-up needed
+    float r;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 
 // w * q (q in Q31, 0..2^31) -> Q31, truncated.
 __device__ __forceinline__ uint32_t mul_q31(uint32_t w, uint32_t q) {
@@ -48,49 +58,40 @@ __device__ __forceinline__ uint32_t mul_q31(uint32_t w, uint32_t q) {
 }
 
 struct CloudView {               // per-unit scalars and shared-memory table pointers
-    const float *phase, *T_edge;
+    const float *phase;
+    const float4 *rows;
     const uint32_t *thr, *albedo;
     const uint16_t *guide;
-    uint32_t n_classes, K1, shiftK, n_depth, n_guide, guide_base, cls_steps;
-    float frac_scale, tau_ext, v_fs, v_max, dv_depth;
+    uint32_t n_classes, K1, shiftK, n_depth, guide_base, guide_shift, cls_steps, depth_bisect;
+    float frac_scale, tau_ext, vh_fs;
     uint32_t R_q31, R_thr, surface_model;
 };
 
-// particle velocity at vertical optical depth Tn, 0 <= Tn < tau_ext: piecewise-linear T(v) table, bins uniform in v.
-__device__ __forceinline__ float depth_velocity(const CloudView &cv, float Tn) {
-    int gi = (int)(__float_as_uint(Tn) >> 16) - (int)cv.guide_base;
-    gi = max(gi, 0);
-    gi = min(gi, (int)cv.n_guide - 1);
-    uint32_t j = cv.guide[gi];
-    float Tj1 = cv.T_edge[j + 1];
-    int steps = 0;
-    while (Tj1 <= Tn && j + 1 < cv.n_depth) {
-        if (++steps > 4) {                               // pathological table: finish by bisection
-            uint32_t lo = j, hi = cv.n_depth;            // T_edge[lo] <= Tn < T_edge[hi]
-            while (hi - lo > 1) {
-                const uint32_t mid = (lo + hi) >> 1;
-                if (cv.T_edge[mid] <= Tn) lo = mid; else hi = mid;
-            }
-            j = lo;
-            Tj1 = cv.T_edge[j + 1];
-            break;
+// half the particle velocity at vertical optical depth Tc, 0 <= Tc <= tau_ext (depth rows: see pdv_device.h).
+__device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float Tc) {
+    uint32_t j;
+    if (cv.depth_bisect) {                                   // pathological table (unit-uniform branch)
+        uint32_t lo = 0u, hi = cv.n_depth;                   // T_lo <= Tc < T_hi
+        while (hi - lo > 1u) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (cv.rows[mid - 1u].x <= Tc) lo = mid; else hi = mid;
         }
-        ++j;
-        Tj1 = cv.T_edge[j + 1];
+        j = lo;
+    } else {
+        const uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base) - cv.guide_base;
+        j = cv.guide[cell];
     }
-    const float Tj = cv.T_edge[j];
-    const float frac = __fdividef(Tn - Tj, Tj1 - Tj);
-    return fmaf(-((float)j + frac), cv.dv_depth, cv.v_max);
+    const float4 r = cv.rows[j];
+    return fmaf(Tc - r.x, Tc < r.x ? r.z : r.w, r.y);
 }
 
-template <bool POLY, bool ANALOG, bool TRACE>
-__global__ void __launch_bounds__(512, 2) transport_kernel(const __grid_constant__ RunParams P) {
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
+__global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned long long s_stats[ST_COUNT];
     __shared__ int s_go;
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u;
-    const uint32_t lanemask_lt = (1u << lane) - 1u;
     unsigned long long *s_hist = reinterpret_cast<unsigned long long *>(smem);
     unsigned long long *s_hist2 = s_hist + P.n_bins;
     unsigned char *s_blob = smem + 16u * (size_t)P.n_bins;
@@ -118,66 +119,87 @@ __global__ void __launch_bounds__(512, 2) transport_kernel(const __grid_constant
         {
             const DevCloudHeader *h = reinterpret_cast<const DevCloudHeader *>(s_blob);
             cv.phase = reinterpret_cast<const float *>(s_blob + h->off_phase);
-            cv.T_edge = reinterpret_cast<const float *>(s_blob + h->off_tedge);
+            cv.rows = reinterpret_cast<const float4 *>(s_blob + h->off_rows);
             cv.thr = reinterpret_cast<const uint32_t *>(s_blob + h->off_thr);
             cv.albedo = reinterpret_cast<const uint32_t *>(s_blob + (ANALOG ? h->off_albthr : h->off_albedo));
             cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide);
             cv.n_classes = h->n_classes; cv.K1 = h->K + 1u; cv.shiftK = 32u - h->log2K;
-            cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base;
+            cv.n_depth = h->n_depth; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
+            cv.depth_bisect = h->depth_bisect;
             cv.cls_steps = 0;
             while ((1u << cv.cls_steps) < cv.n_classes) ++cv.cls_steps;
             cv.frac_scale = __uint_as_float((127u - cv.shiftK) << 23);       // 2^-(32-log2K)
-            cv.tau_ext = h->tau_ext; cv.v_fs = h->v_fs; cv.v_max = h->v_max; cv.dv_depth = h->dv_depth;
+            cv.tau_ext = h->tau_ext; cv.vh_fs = h->vh_fs;
             cv.R_q31 = h->R_q31; cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
         const uint32_t albedo0 = cv.albedo[0];            // monodisperse: the only class
 
         // ---- per-thread accumulators (flushed once per unit) ------------------------------------------------
-        unsigned long long acc_esc = 0ull, acc_absp = 0ull, acc_abss = 0ull;
+        // acc_lost = sum over finished histories of (1 - final weight) + roulette gains: all weight that went into
+        // particles or the surface; absorbed_particles = acc_lost - acc_abss (same integers as a per-event sum).
+        unsigned long long acc_esc = 0ull, acc_lost = 0ull, acc_abss = 0ull;
         uint32_t cnt_hist = 0u, cnt_ev = 0u, cnt_refl = 0u, max_ev = 0u;
 
-        // ---- warp-uniform work-queue state ------------------------------------------------------------------
-        unsigned long long chunk_base = 0ull;
-        uint32_t chunk_pos = 0u, chunk_len = 0u;
-        bool exhausted = false;
-
-        // ---- lane state: one photon history (step (1)) -----------------------------------------
-        bool alive = false;
+        // ---- lane state: one photon history (step (1)) + the lane's private id chunk -------------
+        bool alive = true;
         float T = 0.f, mu = -1.f, vt = 0.f;
-        uint32_t w = 0u, n_sc = 0u, n_refl = 0u, flight = 0u, id_lo = 0u, id_hi = 0u;
+        uint32_t w = kWOne, n_sc = 0u, n_refl = 0u, id_lo = 0u, id_hi = 0u, left = 0u, chunk = P.chunk;
 
-        for (;;) {
-            // ---------------- photon regeneration --------------------------------------------------------------
-            const uint32_t need = __ballot_sync(FULL_MASK, !alive);
-            if (need) {
-                if (chunk_pos >= chunk_len && !exhausted) {
-                    unsigned long long b = 0ull;
-                    if (lane == 0) b = atomicAdd(P.next_id + u, (unsigned long long)P.chunk);
-                    b = __shfl_sync(FULL_MASK, b, 0);
-                    if (b >= P.n_photons) {
-                        exhausted = true;
-                    } else {
-                        const unsigned long long left = P.n_photons - b;
-                        chunk_base = b; chunk_pos = 0u;
-                        chunk_len = left < (unsigned long long)P.chunk ? (uint32_t)left : P.chunk;
-                    }
-                }
-                const uint32_t avail = chunk_len - chunk_pos;
-                const uint32_t rank = __popc(need & lanemask_lt);
-                if (!alive && rank < avail) {
-                    const unsigned long long id = P.first_id + chunk_base + chunk_pos + rank;
+        // next photon of this lane (or alive = false when the unit is drained); resets the history state
+        auto regenerate = [&]() {
+            if (left) {
+                --left;
+                if (++id_lo == 0u) ++id_hi;
+            } else {
+                const unsigned long long b = atomicAdd(P.next_id + u, (unsigned long long)chunk);
+                if (b >= P.n_photons) {
+                    alive = false;
+                } else {
+                    const unsigned long long rem = P.n_photons - b;
+                    const uint32_t len = rem < (unsigned long long)chunk ? (uint32_t)rem : chunk;
+                    const unsigned long long id = P.first_id + b;
                     id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32);
-                    alive = true; T = 0.f; mu = -1.f; vt = 0.f; w = kWOne; n_sc = 0u; n_refl = 0u; flight = 0u;
-                    ++cnt_hist;
+                    left = len - 1u;
+                    cnt_hist += len;
+                    chunk = min(max(__float2uint_rd(__ull2float_rd(rem) * P.chunk_per_remaining), 1u), P.chunk);
                 }
-                chunk_pos += min((uint32_t)__popc(need), avail);
-                if (exhausted && !__any_sync(FULL_MASK, alive)) break;
             }
+            T = 0.f; mu = -1.f; vt = 0.f; w = kWOne; n_sc = 0u; n_refl = 0u;
+        };
+        // end of a history (step (7)): per-history bookkeeping, then the lane's next photon
+        auto finish = [&](int fate) {
+            acc_lost += kWOne - w;
+            cnt_ev += n_sc; cnt_refl += n_refl;
+            max_ev = max(max_ev, n_sc + n_refl);
+            if (TRACE) {
+                const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
+                pdv_trace_record r;
+                r.vt = vt; r.weight = (float)((double)w * kWScale); r.mu_exit = mu; r.fate = fate;
+                r.n_scatter = (int)n_sc; r.n_reflect = (int)n_refl;
+                P.trace[idx] = r;
+            }
+            regenerate();
+        };
 
-            int tally_bin = -1;                            // >= 0: this lane tallies w into that bin this iteration
-            uint32_t tally_w = 0u;
+        {   // initial fill: one atomic per warp hands every lane its first chunk
+            unsigned long long b = 0ull;
+            if (lane == 0) b = atomicAdd(P.next_id + u, 32ull * chunk);
+            b = __shfl_sync(FULL_MASK, b, 0) + (unsigned long long)lane * chunk;
+            if (b >= P.n_photons) {
+                alive = false;
+            } else {
+                const unsigned long long rem = P.n_photons - b;
+                const uint32_t len = rem < (unsigned long long)chunk ? (uint32_t)rem : chunk;
+                const unsigned long long id = P.first_id + b;
+                id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32);
+                left = len - 1u;
+                cnt_hist += len;
+            }
+        }
+        while (__any_sync(FULL_MASK, alive)) {
             if (alive) {
                 // ---------------- random numbers of this flight (step (3)) -------------------------------------
+                const uint32_t flight = n_sc + n_refl;
                 uint32_t x0, x1, x2, x3;
                 philox4x32_10(id_lo, id_hi, ud.stream, 2u * flight, P.key0, P.key1, x0, x1, x2, x3);
                 uint32_t y0 = 0u, y1 = 0u;
@@ -187,45 +209,37 @@ __global__ void __launch_bounds__(512, 2) transport_kernel(const __grid_constant
                 }
                 // ---------------- free flight: s = -ln(xi), xi in (0,1]; T' = T - mu s (Eq. 7/10) --------------
                 const float xi = 2.0f - __uint_as_float(0x3F800000u | (x0 >> 9));
-                const float s = __log2f(xi) * -0.69314718056f;
+                const float s = fast_lg2(xi) * -0.69314718056f;
                 const float Tn = fmaf(-mu, s, T);
-                int fate = -1;
                 if (Tn < 0.f) {
                     // ------------ leaves through the top (step (6)); Eq. 19 tally inside the aperture ----------
+                    int fate = 1;
                     if (mu >= P.mu_aperture) {
                         const float fb = (vt - P.v_lo) * P.inv_dv;
                         fate = 5;
-                        if (fb < 0.f) {
+                        if (!(fb >= 0.f)) {
                             atomicAdd(&s_stats[ST_UNDER], (unsigned long long)w);
                         } else if (fb >= (float)P.n_bins) {
                             atomicAdd(&s_stats[ST_OVER], (unsigned long long)w);
                         } else {
-                            tally_bin = (int)fb; tally_w = w; fate = 0;
+                            const int bin = (int)fb;
+                            atomicAdd(&s_hist[bin], (unsigned long long)w);
+                            atomicAdd(&s_hist2[bin], ((unsigned long long)w * w) >> 31);
+                            fate = 0;
                         }
                     } else {
-                        acc_esc += w; fate = 1;
+                        acc_esc += w;
                     }
+                    finish(fate);
                 } else {
-                    float mu_new, v_here;
-                    if (Tn >= cv.tau_ext) {
-                        // -------- free surface: "ideal diffuse reflection", Doppler event at v_fs
-                        v_here = cv.v_fs;
-                        if (ANALOG) {
-                            if (y1 >= cv.R_thr) { acc_abss += w; fate = 2; }
-                        } else {
-                            const uint32_t wn = mul_q31(w, cv.R_q31);
-                            acc_abss += w - wn; w = wn;
-                        }
-                        const float xc = __uint2float_rn(x2) * 2.3283064365386963e-10f;
-                        mu_new = cv.surface_model ? fast_sqrt(xc) : __cosf(1.57079632679f * xc);
-                        T = cv.tau_ext;
-                        if (fate < 0) { ++n_refl; ++cnt_refl; }
-                    } else if (P.single_scatter_only && n_sc >= 1u) {
+                    const bool surf = Tn >= cv.tau_ext;           // reaches the free surface
+                    if (SSO && !surf && n_sc >= 1u) {             // single-scatter-only mode: cut at the 2nd particle event
                         atomicAdd(&s_stats[ST_TRUNC], (unsigned long long)w);
-                        fate = 4; mu_new = mu; v_here = 0.f;
+                        finish(4);
                     } else {
-                        // -------- particle interaction at depth Tn (steps (4)-(5)) ------------------------------
-                        v_here = depth_velocity(cv, Tn);
+                        // -------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ----
+                        T = fminf(Tn, cv.tau_ext);
+                        const float vh = depth_half_velocity(cv, T);           // = v_fs / 2 at the surface
                         uint32_t c = 0u, alb = albedo0;
                         if (POLY) {
                             for (uint32_t stp = 1u << cv.cls_steps; stp > 1u;) {     // thr padded with 0xffffffff
@@ -235,79 +249,61 @@ __global__ void __launch_bounds__(512, 2) transport_kernel(const __grid_constant
                             c = min(c, cv.n_classes - 1u);
                             alb = cv.albedo[c];
                         }
-                        ++cnt_ev;
-                        if (ANALOG) {
-                            if (y1 >= alb) { acc_absp += w; fate = 2; }          // alb = albedo threshold in analog mode
+                        bool absorbed = false;
+                        if (ANALOG) {                             // Eq. 11 literally: absorbed with probability 1 - albedo
+                            absorbed = y1 >= (surf ? cv.R_thr : alb);
+                        } else {                                  // implicit capture: Eq. 11 in expectation
+                            const uint32_t wn = mul_q31(w, surf ? cv.R_q31 : alb);
+                            if (surf) acc_abss += w - wn;
+                            w = wn;
+                        }
+                        if (ANALOG && absorbed) {
+                            if (surf) acc_abss += w; else ++cnt_ev;           // an absorbing interaction is a particle event
+                            w = 0u;
+                            finish(2);
                         } else {
-                            const uint32_t wn = mul_q31(w, alb);                 // Eq. 11 in expectation
-                            acc_absp += w - wn; w = wn;
-                        }
-                        const float *M = cv.phase + c * cv.K1;
-                        const uint32_t k = x2 >> cv.shiftK;
-                        const float frac = __uint2float_rn(x2 - (k << cv.shiftK)) * cv.frac_scale;
-                        const float m0 = M[k], m1 = M[k + 1u];
-                        const float ct = fmaf(m1 - m0, frac, m0);                   // cos(theta) from D_K
-                        const float cphi = __cosf(__int2float_rn((int)x3) * 1.46291807927e-9f);   // phi = 2 pi x3/2^32
-                        const float sq = fast_sqrt(fmaxf((1.f - ct) * (1.f + ct) * (1.f - mu) * (1.f + mu), 0.f));
-                        mu_new = fmaf(mu, ct, -cphi * sq);                           // z row of Eq. 16 (Eq. 17 at |mu| = 1)
-                        mu_new = fminf(fmaxf(mu_new, -1.f), 1.f);
-                        T = Tn;
-                        if (fate < 0) ++n_sc;
-                    }
-                    if (fate < 0) {
-                        vt = fmaf(0.5f * (mu_new - mu), v_here, vt);                 // Eq. 4
-                        mu = mu_new;
-                        ++flight;
-                        if (P.max_events && n_sc >= P.max_events && w <= P.roulette_wcap) {   // Russian roulette
-                            if (!ANALOG) {
-                                uint32_t y2, y3;
-                                philox4x32_10(id_lo, id_hi, ud.stream, 2u * flight - 1u, P.key0, P.key1, y0, y1, y2, y3);
+                            // cos(theta) from D_K (Eq. 13-14), azimuth (Eq. 15); surface: polar angle uniform in [0, pi/2]
+                            const float *M = cv.phase + c * cv.K1;
+                            const uint32_t k = x2 >> cv.shiftK;
+                            const float frac = __uint2float_rn(x2 - (k << cv.shiftK)) * cv.frac_scale;
+                            const float m0 = M[k], m1 = M[k + 1u];
+                            const float ct = fmaf(m1 - m0, frac, m0);
+                            // one cosine serves both: cos(phi), phi = 2 pi x3 / 2^32, or cos(theta'), theta' = (pi/2) x2 / 2^32
+                            const float cosv = __cosf(__uint2float_rn(surf ? x2 : x3) *
+                                                      (surf ? 3.65729519818e-10f : 1.46291807927e-9f));
+                            const float sq = fast_sqrt(fmaxf(fmaf(-ct, ct, 1.f) * fmaf(-mu, mu, 1.f), 0.f));
+                            float mu_s = fmaf(mu, ct, -cosv * sq);                    // z row of Eq. 16 (Eq. 17 at |mu| = 1)
+                            mu_s = fminf(fmaxf(mu_s, -1.f), 1.f);
+                            float mu_r = cosv;
+                            if (cv.surface_model) mu_r = fast_sqrt(__uint2float_rn(x2) * 2.3283064365386963e-10f);   // Lambertian
+                            const float mu_new = surf ? mu_r : mu_s;
+                            vt = fmaf(mu_new - mu, vh, vt);                            // Eq. 4 (vh = v/2)
+                            mu = mu_new;
+                            if (surf) ++n_refl; else ++n_sc;
+                            if (n_sc >= P.max_events && w <= P.roulette_wcap) {      // Russian roulette (rare path)
+                                if (!ANALOG) {
+                                    uint32_t y2, y3;
+                                    philox4x32_10(id_lo, id_hi, ud.stream, 2u * flight + 1u, P.key0, P.key1, y0, y1, y2, y3);
+                                }
+                                if (y0 < P.roulette_thr) {
+                                    uint32_t wn = (uint32_t)__float2uint_rd(__uint2float_rd(w) * P.roulette_inv_p);
+                                    wn = max(min(wn, kWOne), w);
+                                    atomicAdd(&s_stats[ST_GAINED], (unsigned long long)(wn - w));
+                                    acc_lost += wn - w;
+                                    w = wn;
+                                } else {
+                                    atomicAdd(&s_stats[ST_KILLED], (unsigned long long)w);
+                                    finish(3);
+                                }
                             }
-                            if (y0 < P.roulette_thr) {
-                                uint32_t wn = (uint32_t)__float2uint_rd(__uint2float_rd(w) * P.roulette_inv_p);
-                                wn = max(min(wn, kWOne), w);
-                                atomicAdd(&s_stats[ST_GAINED], (unsigned long long)(wn - w));
-                                w = wn;
-                            } else {
-                                atomicAdd(&s_stats[ST_KILLED], (unsigned long long)w);
-                                fate = 3;
-                            }
                         }
-                    }
-                }
-                if (fate >= 0) {                            // history over (step (7))
-                    alive = false;
-                    max_ev = max(max_ev, n_sc + n_refl);
-                    if (TRACE) {
-                        const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
-                        pdv_trace_record r;
-                        r.vt = vt; r.weight = (float)((double)w * kWScale); r.mu_exit = mu; r.fate = fate;
-                        r.n_scatter = (int)n_sc; r.n_reflect = (int)n_refl;
-                        P.trace[idx] = r;
-                    }
-                }
-            }
-
-            // ---------------- warp-aggregated tally into the block's private histogram (Eq. 19) ----------------
-            const uint32_t tm = __ballot_sync(FULL_MASK, tally_bin >= 0);
-            if (tm) {
-                if (tally_bin >= 0) {
-                    const uint32_t peers = __match_any_sync(tm, tally_bin);
-                    unsigned long long sw = 0ull, sw2 = 0ull;
-                    for (uint32_t m = peers; m; m &= m - 1u) {            // sum the weights of the lanes in my bin
-                        const uint32_t wl = __shfl_sync(peers, tally_w, __ffs(m) - 1);
-                        sw += wl;
-                        sw2 += ((unsigned long long)wl * wl) >> 31;
-                    }
-                    if (lane == (uint32_t)(__ffs(peers) - 1)) {
-                        atomicAdd(&s_hist[tally_bin], sw);
-                        atomicAdd(&s_hist2[tally_bin], sw2);
                     }
                 }
             }
         }
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
+        unsigned long long acc_absp = acc_lost - acc_abss;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             acc_esc += __shfl_xor_sync(FULL_MASK, acc_esc, o);
@@ -350,39 +346,45 @@ __global__ void __launch_bounds__(512, 2) transport_kernel(const __grid_constant
 }
 
 // ------------------------------------------------------------------------------------------------------------
-template <bool POLY, bool ANALOG, bool TRACE>
+// The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
+static cudaError_t ensure_smem(int smem) {
+    static int smem_set = 48 * 1024;
+    if (smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    return cudaSuccess;
+}
+
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
 static cudaError_t launch_t(const RunParams &rp, LaunchShape s, cudaStream_t st) {
-    auto k = transport_kernel<POLY, ANALOG, TRACE>;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, s.smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE>(s.smem);
     if (e != cudaSuccess) return e;
-    k<<<s.grid, s.block, s.smem, st>>>(rp);
+    transport_kernel<POLY, ANALOG, SSO, TRACE><<<s.grid, s.block, s.smem, st>>>(rp);
     return cudaGetLastError();
 }
 
-template <bool POLY, bool ANALOG, bool TRACE>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
 static cudaError_t occ_t(int block, int smem, int *out) {
-    auto k = transport_kernel<POLY, ANALOG, TRACE>;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE>(smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k, block, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE>, block, smem);
 }
 
-#define PDV_DISPATCH(FN, ...)                                                      \
-    do {                                                                           \
-        if (trace) {                                                               \
-            if (poly) return analog ? FN<true, true, true>(__VA_ARGS__) : FN<true, false, true>(__VA_ARGS__);    \
-            return analog ? FN<false, true, true>(__VA_ARGS__) : FN<false, false, true>(__VA_ARGS__);            \
-        }                                                                          \
-        if (poly) return analog ? FN<true, true, false>(__VA_ARGS__) : FN<true, false, false>(__VA_ARGS__);      \
-        return analog ? FN<false, true, false>(__VA_ARGS__) : FN<false, false, false>(__VA_ARGS__);              \
-    } while (0)
+#define PDV_D1(FN, A, B, C, ...) (v.trace ? FN<A, B, C, true>(__VA_ARGS__) : FN<A, B, C, false>(__VA_ARGS__))
+#define PDV_D2(FN, A, B, ...) (v.sso ? PDV_D1(FN, A, B, true, __VA_ARGS__) : PDV_D1(FN, A, B, false, __VA_ARGS__))
+#define PDV_D3(FN, A, ...) (v.analog ? PDV_D2(FN, A, true, __VA_ARGS__) : PDV_D2(FN, A, false, __VA_ARGS__))
+#define PDV_DISPATCH(FN, ...) (v.poly ? PDV_D3(FN, true, __VA_ARGS__) : PDV_D3(FN, false, __VA_ARGS__))
 
-cudaError_t launch_transport(const RunParams &rp, bool poly, bool analog, bool trace, LaunchShape shape, cudaStream_t st) {
-    PDV_DISPATCH(launch_t, rp, shape, st);
+cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st) {
+    return PDV_DISPATCH(launch_t, rp, shape, st);
 }
 
-cudaError_t transport_max_blocks_per_sm(bool poly, bool analog, bool trace, int block, int smem, int *out) {
-    PDV_DISPATCH(occ_t, block, smem, out);
+cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out) {
+    return PDV_DISPATCH(occ_t, block, smem, out);
 }
 
 // ---- finalize: Q31 integers -> doubles (H12 input; stats) ------------------------------------------------------
