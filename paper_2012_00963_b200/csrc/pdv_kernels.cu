@@ -17,6 +17,15 @@
 //     the block's private shared-memory histogram is flushed once per block and unit.
 #include "pdv_device.h"
 
+#ifdef PDV_DEBUG_BOUNDS
+#include <cstdio>
+// debug build: clamp every data-dependent shared-memory index and count the violations per category (reported at the flush)
+#define PDV_BOUND(cat, idx, limit) do { if ((uint32_t)(idx) >= (uint32_t)(limit)) { atomicAdd(&s_dbg[cat], 1u); s_dbg[4 + cat] = (uint32_t)(idx); idx = 0; } } while (0)
+__shared__ unsigned int s_dbg[8];
+#else
+#define PDV_BOUND(cat, idx, limit) do { } while (0)
+#endif
+
 namespace pdv {
 
 #define FULL_MASK 0xffffffffu
@@ -57,12 +66,20 @@ __device__ __forceinline__ uint32_t mul_q31(uint32_t w, uint32_t q) {
     return (uint32_t)(((unsigned long long)w * q) >> 31);
 }
 
+// 64-bit shared-memory tally += 32-bit value with two native 32-bit atomics (low word, carry into the high word)
+// instead of the compare-and-swap spin loop a 64-bit shared atomicAdd compiles to.
+__device__ __forceinline__ void smem_add64(unsigned long long *p, uint32_t v) {
+    uint32_t *q = reinterpret_cast<uint32_t *>(p);
+    const uint32_t old = atomicAdd(q, v);
+    if (old + v < old) atomicAdd(q + 1, 1u);
+}
+
 struct CloudView {               // per-unit scalars and shared-memory table pointers
     const float *phase;
     const float4 *rows;
     const uint32_t *thr, *albedo;
     const uint16_t *guide;
-    uint32_t n_classes, K1, shiftK, n_depth, guide_base, guide_shift, cls_steps, depth_bisect;
+    uint32_t n_classes, K1, shiftK, n_depth, n_guide, guide_base, guide_shift, cls_steps, depth_bisect;
     float frac_scale, tau_ext, vh_fs;
     uint32_t R_q31, R_thr, surface_model;
 };
@@ -78,9 +95,11 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
         }
         j = lo;
     } else {
-        const uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base) - cv.guide_base;
+        uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base) - cv.guide_base;
+        PDV_BOUND(0, cell, cv.n_guide);
         j = cv.guide[cell];
     }
+    PDV_BOUND(1, j, cv.n_depth);
     const float4 r = cv.rows[j];
     return fmaf(Tc - r.x, Tc < r.x ? r.z : r.w, r.y);
 }
@@ -113,6 +132,9 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
             for (uint32_t i = tid; i < n16; i += blockDim.x) dst[i] = __ldg(src + i);
             for (uint32_t i = tid; i < 2u * P.n_bins; i += blockDim.x) s_hist[i] = 0ull;
             if (tid < ST_COUNT) s_stats[tid] = 0ull;
+#ifdef PDV_DEBUG_BOUNDS
+            if (tid < 8) s_dbg[tid] = 0u;
+#endif
         }
         __syncthreads();
         CloudView cv;
@@ -124,7 +146,7 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
             cv.albedo = reinterpret_cast<const uint32_t *>(s_blob + (ANALOG ? h->off_albthr : h->off_albedo));
             cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide);
             cv.n_classes = h->n_classes; cv.K1 = h->K + 1u; cv.shiftK = 32u - h->log2K;
-            cv.n_depth = h->n_depth; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
+            cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
             cv.depth_bisect = h->depth_bisect;
             cv.cls_steps = 0;
             while ((1u << cv.cls_steps) < cv.n_classes) ++cv.cls_steps;
@@ -211,31 +233,32 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                 const float xi = 2.0f - __uint_as_float(0x3F800000u | (x0 >> 9));
                 const float s = fast_lg2(xi) * -0.69314718056f;
                 const float Tn = fmaf(-mu, s, T);
+                int fate = -1;                                    // >= 0: the history ends in this iteration
                 if (Tn < 0.f) {
                     // ------------ leaves through the top (step (6)); Eq. 19 tally inside the aperture ----------
-                    int fate = 1;
+                    fate = 1;
                     if (mu >= P.mu_aperture) {
                         const float fb = (vt - P.v_lo) * P.inv_dv;
                         fate = 5;
                         if (!(fb >= 0.f)) {
-                            atomicAdd(&s_stats[ST_UNDER], (unsigned long long)w);
+                            smem_add64(&s_stats[ST_UNDER], w);
                         } else if (fb >= (float)P.n_bins) {
-                            atomicAdd(&s_stats[ST_OVER], (unsigned long long)w);
+                            smem_add64(&s_stats[ST_OVER], w);
                         } else {
-                            const int bin = (int)fb;
-                            atomicAdd(&s_hist[bin], (unsigned long long)w);
-                            atomicAdd(&s_hist2[bin], ((unsigned long long)w * w) >> 31);
+                            int bin = (int)fb;
+                            PDV_BOUND(2, bin, P.n_bins);
+                            smem_add64(&s_hist[bin], w);
+                            smem_add64(&s_hist2[bin], mul_q31(w, w));
                             fate = 0;
                         }
                     } else {
                         acc_esc += w;
                     }
-                    finish(fate);
                 } else {
                     const bool surf = Tn >= cv.tau_ext;           // reaches the free surface
                     if (SSO && !surf && n_sc >= 1u) {             // single-scatter-only mode: cut at the 2nd particle event
-                        atomicAdd(&s_stats[ST_TRUNC], (unsigned long long)w);
-                        finish(4);
+                        smem_add64(&s_stats[ST_TRUNC], w);
+                        fate = 4;
                     } else {
                         // -------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ----
                         T = fminf(Tn, cv.tau_ext);
@@ -260,11 +283,12 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                         if (ANALOG && absorbed) {
                             if (surf) acc_abss += w; else ++cnt_ev;           // an absorbing interaction is a particle event
                             w = 0u;
-                            finish(2);
+                            fate = 2;
                         } else {
                             // cos(theta) from D_K (Eq. 13-14), azimuth (Eq. 15); surface: polar angle uniform in [0, pi/2]
                             const float *M = cv.phase + c * cv.K1;
-                            const uint32_t k = x2 >> cv.shiftK;
+                            uint32_t k = x2 >> cv.shiftK;
+                            PDV_BOUND(3, k, cv.K1 - 1u);
                             const float frac = __uint2float_rn(x2 - (k << cv.shiftK)) * cv.frac_scale;
                             const float m0 = M[k], m1 = M[k + 1u];
                             const float ct = fmaf(m1 - m0, frac, m0);
@@ -288,17 +312,18 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                                 if (y0 < P.roulette_thr) {
                                     uint32_t wn = (uint32_t)__float2uint_rd(__uint2float_rd(w) * P.roulette_inv_p);
                                     wn = max(min(wn, kWOne), w);
-                                    atomicAdd(&s_stats[ST_GAINED], (unsigned long long)(wn - w));
+                                    smem_add64(&s_stats[ST_GAINED], wn - w);
                                     acc_lost += wn - w;
                                     w = wn;
                                 } else {
-                                    atomicAdd(&s_stats[ST_KILLED], (unsigned long long)w);
-                                    finish(3);
+                                    smem_add64(&s_stats[ST_KILLED], w);
+                                    fate = 3;
                                 }
                             }
                         }
                     }
                 }
+                if (fate >= 0) finish(fate);                      // the one place where a lane moves on to its next photon
             }
         }
 
@@ -324,6 +349,11 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
             atomicMax(&s_stats[ST_MAXEV], (unsigned long long)max_ev);
         }
         __syncthreads();
+#ifdef PDV_DEBUG_BOUNDS
+        if (tid == 0 && (s_dbg[0] | s_dbg[1] | s_dbg[2] | s_dbg[3]))
+            printf("PDV_BOUND block %u: guide %u (%u) rows %u (%u) bin %u (%u) phase %u (%u)\n", blockIdx.x, s_dbg[0], s_dbg[4],
+                   s_dbg[1], s_dbg[5], s_dbg[2], s_dbg[6], s_dbg[3], s_dbg[7]);
+#endif
         {
             unsigned long long *gh = P.hist + (size_t)u * P.n_bins, *gh2 = P.hist2 + (size_t)u * P.n_bins;
             unsigned long long det = 0ull;

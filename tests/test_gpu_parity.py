@@ -44,15 +44,18 @@ def _assert_hist_parity(g_hist, g_hist2, n_g, o, min_ndf=5):
     return res
 
 
-def _assert_stats_parity(gs, n_g, o):
-    """Weights leaving / absorbed per photon agree within 5 sigma of a conservative variance bound (w <= 1)."""
+def _assert_stats_parity(gs, n_g, o, same_game=True):
+    """Weights leaving / absorbed per photon agree within 5 sigma of a conservative variance bound (w <= 1).
+    same_game=False: the two sides play Russian roulette under different rules (the kernel only while w/p <= 1,
+    DESIGN.md reading R20), so the number of events per history is not comparable, only the expectations are."""
     for key in ("detected", "escaped", "absorbed_particles", "absorbed_surface", "truncated"):
         a, b = float(gs[key]) / n_g, o.stats[key] / o.n_photons
         sig = math.sqrt(max(a, 1e-12) / n_g + max(b, 1e-12) / o.n_photons)
         assert abs(a - b) < 5 * sig, (key, a, b, sig)
-    a = float(gs["particle_events"]) / n_g
-    b = o.stats["particle_events"] / o.n_photons
-    assert a == pytest.approx(b, rel=0.02)
+    if same_game:
+        a = float(gs["particle_events"]) / n_g
+        b = o.stats["particle_events"] / o.n_photons
+        assert a == pytest.approx(b, rel=0.02)
 
 
 # -------------------------------------------------------------------------------------------------- configs
@@ -214,7 +217,7 @@ def test_variants_match_oracle(P, kw, ckw):
     else:
         o = _oracle(params, run, n)
     _assert_hist_parity(r.hist[0, 0], r.hist2[0, 0], n, o, min_ndf=3)
-    _assert_stats_parity(r.stats[0, 0], n, o)
+    _assert_stats_parity(r.stats[0, 0], n, o, same_game="max_events" not in kw)
     for key in ("underflow", "overflow"):
         a, b = float(r.stats[0, 0][key]) / n, o.stats[key] / n
         assert abs(a - b) < 5 * math.sqrt((a + b + 1e-9) / n)
@@ -329,3 +332,23 @@ def test_full_size_config2_in_bench_launch_configuration(P):
     a, b = s["detected"] / n, o.stats["detected"] / n_o
     assert abs(a - b) < 5 * math.sqrt(a / n + b / n_o)
     assert s["particle_events"] / n == pytest.approx(o.stats["particle_events"] / n_o, rel=2e-3)
+
+
+def test_rare_paths_stress_many_short_runs(P):
+    """Short runs that spend most of their time in the rare paths (roulette kill / survive, analog absorption,
+    single-scatter truncation, drained-queue lanes) in varying order: every run must complete, conserve weight
+    exactly and be bit-reproducible.  (A first version of the kernel faulted intermittently here.)"""
+    cfg = W.config(1)
+    kws = [dict(max_events=3, roulette_survival=0.5), dict(), dict(mode=1), dict(single_scatter_only=1),
+           dict(mode=1, max_events=2, roulette_survival=0.3), dict(max_events=1, roulette_survival=0.1)]
+    ref = {}
+    for rep in range(6):
+        for i in (np.arange(len(kws)) + rep) % len(kws):
+            c = P.pdv_cloud_create(cfg["clouds"][0])
+            n = 200_000 + 1000 * int(i)
+            r = P.pdv_mc_run([c], cfg["t_snap"], n, 77, dict(cfg["run"], **kws[i]))
+            assert r.stats[0, 0]["histories"] == n and r.conservation_residual()[0, 0] == 0.0
+            key = int(i)
+            if key in ref:
+                assert np.array_equal(ref[key], r.hist)
+            ref[key] = r.hist
