@@ -25,7 +25,7 @@
  * Random numbers: rng_mode 0 = xoshiro256** seeded per photon by splitmix64 (53-bit uniforms),
  * unrelated to the GPU generator.  rng_mode 1 = the shared counter-based stream of DESIGN.md
  * ("each side implements the same counter-based generator"): Philox4x32-10, key = seed,
- * counter = (id_lo, id_hi, stream, 2*flight + sub), with the word->uniform maps of DESIGN.md D2.
+ * counter = (id_lo, id_hi, stream, 2*draw + sub), with the word->uniform maps of DESIGN.md D2.
  * Mode 1 exists so that single histories can be compared with the GPU; it is pinned by the
  * published known-answer vectors of Philox4x32-10 (tests/golden/philox4x32_10_kat.txt).
  *
@@ -138,22 +138,40 @@ static inline double rng_u53(rng_t *r) {           /* uniform in [0,1), 53 bits 
 /* the uniforms one flight needs */
 typedef struct { double xi_path, xi_class, xi_cos, xi_phi, xi_roulette, xi_absorb; } flight_draws;
 
-static void draw_flight(rng_t *r, uint32_t flight, flight_draws *d) {
+static void draw_flight(rng_t *r, const oracle_params *p, uint32_t flight, flight_draws *d) {
     if (r->mode == 0) {
         d->xi_path = 1.0 - rng_u53(r);             /* (0,1] */
         d->xi_class = rng_u53(r); d->xi_cos = rng_u53(r); d->xi_phi = rng_u53(r);
         d->xi_roulette = rng_u53(r); d->xi_absorb = rng_u53(r);
-    } else {                                       /* DESIGN.md D1/D2 */
-        uint32_t c[4] = { r->id_lo, r->id_hi, r->stream, 2u * flight }, x[4], y[4];
+    } else {                                       /* DESIGN.md D1/D2: the shared counter-based stream */
+        /* D1: block index `draw` = flight (several size classes: one block per flight) or flight/2 (one class: one
+         * block feeds two flights, words (x0,x1) then (x2,x3)); counter word 3 = 2 draw, and 2 draw + 1 for the
+         * second block (absorption / roulette words). */
+        int mono = p->n_classes == 1;
+        uint32_t draw = mono ? flight >> 1 : flight, half = mono ? (flight & 1u) : 0u;
+        uint32_t c[4] = { r->id_lo, r->id_hi, r->stream, 2u * draw }, x[4], y[4];
         oracle_philox4x32_10(c, r->key, x);
-        c[3] = 2u * flight + 1u;
+        c[3] = 2u * draw + 1u;
         oracle_philox4x32_10(c, r->key, y);
-        d->xi_path = 1.0 - (double)(x[0] >> 9) * (1.0 / 8388608.0);      /* (0,1], 23 bits */
-        d->xi_class = ((double)x[1] + 0.5) * (1.0 / 4294967296.0);
-        d->xi_cos = (double)x[2] * (1.0 / 4294967296.0);
-        d->xi_phi = (double)x[3] * (1.0 / 4294967296.0);
-        d->xi_roulette = (double)y[0] * (1.0 / 4294967296.0);
-        d->xi_absorb = (double)y[1] * (1.0 / 4294967296.0);
+        uint32_t a, b, pw;
+        if (mono) {
+            a = x[2 * half]; b = x[2 * half + 1];
+            /* azimuth word of a two-word flight: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top */
+            pw = ((a & 0xFFu) << 24) | ((b & 0xFFu) << 16) | (((a >> 8) & 0xFFu) << 8) | ((a >> 16) & 0xFFu);
+            d->xi_class = 0.0;
+        } else {
+            a = x[0]; b = x[2]; pw = x[3];
+            d->xi_class = ((double)x[1] + 0.5) * (1.0 / 4294967296.0);
+        }
+        /* D2: path = top 23 bits of a; phase = top (log2 K + 12) bits of b; azimuth = pw */
+        int log2K = 0;
+        while ((1 << log2K) < p->K) ++log2K;
+        uint32_t keep = (uint32_t)(log2K + 12);
+        d->xi_path = 1.0 - (double)(a >> 9) * (1.0 / 8388608.0);         /* (0,1], 23 bits */
+        d->xi_cos = (double)(b >> (32u - keep)) / (double)(1ull << keep);
+        d->xi_phi = (double)pw * (1.0 / 4294967296.0);
+        d->xi_absorb = (double)y[half] * (1.0 / 4294967296.0);
+        d->xi_roulette = (double)y[2 + half] * (1.0 / 4294967296.0);
     }
 }
 
@@ -250,7 +268,7 @@ static void run_history(const oracle_params *p, uint64_t id, tally_t *ty, oracle
     flight_draws d;
     ty->st.histories += 1;
     for (;;) {
-        draw_flight(&rng, flight++, &d);
+        draw_flight(&rng, p, flight++, &d);
         double s = -log(d.xi_path);
         double Tn = T - u[2] * s;
         if (Tn < 0.0) {                            /* leaves through the top (step 6) */
@@ -270,8 +288,9 @@ static void run_history(const oracle_params *p, uint64_t id, tally_t *ty, oracle
             if (p->mode == 1) {                    /* analog: absorbed with probability 1-R */
                 if (d.xi_absorb >= p->R) { ty->st.absorbed_surface += w; fate = 2; w = 0.0; break; }
             } else { ty->st.absorbed_surface += w * (1.0 - p->R); w *= p->R; }
-            double mu_new = (p->surface_model == 1) ? sqrt(d.xi_cos) : cos(0.5 * M_PI * d.xi_cos);
-            double sn = sqrt(fmax(0.0, 1.0 - mu_new * mu_new)), ph = 2.0 * M_PI * d.xi_phi;
+            /* two independent uniforms: xi_phi drives the polar angle here, xi_cos the azimuth (D2) */
+            double mu_new = (p->surface_model == 1) ? sqrt(d.xi_phi) : cos(0.5 * M_PI * d.xi_phi);
+            double sn = sqrt(fmax(0.0, 1.0 - mu_new * mu_new)), ph = 2.0 * M_PI * d.xi_cos;
             u[0] = sn * cos(ph); u[1] = sn * sin(ph); u[2] = mu_new;
             T = p->tau_ext;
             n_refl += 1; ty->st.surface_reflections += 1;

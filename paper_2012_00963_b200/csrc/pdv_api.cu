@@ -107,10 +107,10 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     DevCloudHeader hd;
     std::memset(&hd, 0, sizeof(hd));
     size_t off = sizeof(DevCloudHeader);
-    hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * (size_t)nc * (K + 1));
+    hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * 2 * (size_t)nc * K);
     hd.off_rows = (uint32_t)off;   off = align16(off + sizeof(float) * 4 * (size_t)nd);
     hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * n_pad);
-    hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
+    hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * n_pad);
     hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
     hd.blob_bytes = (uint32_t)off;
@@ -119,19 +119,26 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     hd.log2K = 0;
     while ((1 << hd.log2K) < K) ++hd.log2K;
     hd.tau_ext = Tf[nd]; hd.vh_fs = (float)(0.5 * h.v_fs);
-    hd.R_q31 = (uint32_t)std::llround(h.R * 2147483648.0);
+    hd.R_f = (float)h.R;
     hd.R_thr = to_thr32(h.R);
     hd.surface_model = (uint32_t)h.surface_model;
+    const uint32_t shiftK = 32u - hd.log2K;                   // K <= 4096: shiftK >= 20
+    hd.frac_mask = 0xFFFu << (shiftK - 12u);
     blob.assign(off, 0);
     std::memcpy(blob.data(), &hd, sizeof(hd));
     float *ph = reinterpret_cast<float *>(blob.data() + hd.off_phase);
+    std::vector<float> Mf(K + 1);
     for (int c = 0; c < nc; ++c) {
         float prev = -1.f;
         for (int k = 0; k <= K; ++k) {
             float v = (float)h.phase[(size_t)c * (K + 1) + k];
             if (v < prev) v = prev;
-            ph[(size_t)c * (K + 1) + k] = v;
+            Mf[k] = v;
             prev = v;
+        }
+        for (int k = 0; k < K; ++k) {                         // (M[k], (M[k+1] - M[k]) 2^-shiftK): layout in pdv_device.h
+            ph[2 * ((size_t)c * K + k) + 0] = Mf[k];
+            ph[2 * ((size_t)c * K + k) + 1] = (float)std::ldexp((double)Mf[k + 1] - (double)Mf[k], -(int)shiftK);
         }
     }
     float *rows = reinterpret_cast<float *>(blob.data() + hd.off_rows);
@@ -142,7 +149,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
         rows[4 * j + 3] = slope[j + 1];
     }
     uint32_t *thr = reinterpret_cast<uint32_t *>(blob.data() + hd.off_thr);
-    uint32_t *alb = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albedo);
+    float *alb = reinterpret_cast<float *>(blob.data() + hd.off_albedo);
     uint32_t *albt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albthr);
     double cum = 0.0;
     for (int c = 0; c < n_pad; ++c) {
@@ -154,7 +161,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
             thr[c] = 0xFFFFFFFFu;
         }
         const double om = c < nc ? h.k_sca[c] / h.k_ext[c] : 0.0;
-        alb[c] = (uint32_t)std::llround(std::min(std::max(om, 0.0), 1.0) * 2147483648.0);
+        alb[c] = (float)std::min(std::max(om, 0.0), 1.0);
         albt[c] = to_thr32(om);
     }
     std::memcpy(blob.data() + hd.off_guide, guide.data(), sizeof(uint16_t) * n_guide);
@@ -240,7 +247,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     rp.max_events = o->max_events > 0 ? (uint32_t)o->max_events : 0xFFFFFFFFu;
     const double p = o->max_events > 0 ? o->roulette_survival : 1.0;
     rp.roulette_thr = to_thr32(p);
-    rp.roulette_wcap = (uint32_t)std::floor(p * 2147483648.0);
+    rp.roulette_p = (float)p;
     rp.roulette_inv_p = (float)(1.0 / p);
     rp.v_lo = (float)o->v_lo;
     rp.inv_dv = (float)((double)o->n_bins / (o->v_hi - o->v_lo));

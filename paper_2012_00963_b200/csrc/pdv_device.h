@@ -7,8 +7,10 @@
 
 namespace pdv {
 
-// Fixed point of every weight and tally: Q31, one photon = 2^31.
+// Fixed point of every tally: Q31, one photon = 2^31.  A history carries its weight in fp32 (a product of albedos in
+// event order: the same bits for any launch shape) and converts it once, when the history ends.
 constexpr uint32_t kWOne = 0x80000000u;
+constexpr float kWOneF = 2147483648.0f;
 constexpr double kWScale = 1.0 / 2147483648.0;
 
 // Per-unit statistics slots (u64 each) in the device workspace.
@@ -17,8 +19,13 @@ enum StatSlot {
     ST_HISTORIES, ST_EVENTS, ST_REFLECT, ST_MAXEV, ST_COUNT = 16
 };
 
-// Device image of one cloud: one contiguous blob [DevCloudHeader | phase | depth rows | class thr | albedo Q31 | albedo thr | guide],
+// Device image of one cloud: one contiguous blob [DevCloudHeader | phase | depth rows | class thr | albedo f32 | albedo thr | guide],
 // every section 16-byte aligned, copied verbatim into shared memory by each block.
+//
+// Phase table (one float2 per class c and phase bin k, k = 0..K-1): x = M_c[k], y = (M_c[k+1] - M_c[k]) * 2^-shiftK with
+// shiftK = 32 - log2 K, so that for a 32-bit word b:  k = b >> shiftK,  cos(theta) = x + y * (b & frac_mask)  -- the canonical
+// D_K sample M[k] + (M[k+1]-M[k]) frac with frac = the 12 bits of b below the index bits: one 64-bit load,
+// one FFMA.
 //
 // Depth rows (one float4 per depth bin j, bins uniform in v, j = 0 at the cloud top):
 //   x = T_{j+1}                      vertical optical depth of the LOWER edge of bin j
@@ -38,10 +45,11 @@ struct DevCloudHeader {
     uint32_t guide_shift;
     uint32_t depth_bisect;
     float tau_ext, vh_fs;      // vh_fs = v_fs / 2
-    uint32_t R_q31;            // surface reflectivity, Q31
-    uint32_t R_thr;            // analog mode: reflected iff y1 < R_thr
+    float R_f;                 // surface reflectivity
+    uint32_t R_thr;            // analog mode: reflected iff xi_absorb word < R_thr
     uint32_t surface_model;
-    uint32_t pad[8];
+    uint32_t frac_mask;        // the 12 bits of a phase word below its log2K index bits
+    uint32_t pad[7];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 
@@ -63,8 +71,8 @@ struct RunParams {
     uint32_t chunk;                    // photon ids a lane claims per fetch at the start of a unit (guided: shrinks
     float chunk_per_remaining;         //   to clamp(remaining * chunk_per_remaining, 1, chunk) as the unit drains)
     uint32_t max_events;               // roulette once n_scatter >= max_events; 0xffffffff: never
-    uint32_t roulette_thr;             // survive iff y0 < roulette_thr
-    uint32_t roulette_wcap;            // play only while w <= wcap (= floor(p 2^31))
+    uint32_t roulette_thr;             // survive iff the roulette word < roulette_thr
+    float roulette_p;                  // play only while w <= p (then w / p <= 1)
     float roulette_inv_p;
     float v_lo, inv_dv, mu_aperture;
     unsigned long long n_photons, first_id;

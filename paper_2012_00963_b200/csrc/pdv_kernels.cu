@@ -61,7 +61,7 @@ __device__ __forceinline__ float fast_lg2(float x) {       // x is a normal numb
     return r;
 }
 
-// w * q (q in Q31, 0..2^31) -> Q31, truncated.
+// Q31 * Q31 -> Q31, truncated (sum of squared weights).
 __device__ __forceinline__ uint32_t mul_q31(uint32_t w, uint32_t q) {
     return (uint32_t)(((unsigned long long)w * q) >> 31);
 }
@@ -75,13 +75,14 @@ __device__ __forceinline__ void smem_add64(unsigned long long *p, uint32_t v) {
 }
 
 struct CloudView {               // per-unit scalars and shared-memory table pointers
-    const float *phase;
+    const float2 *phase;
     const float4 *rows;
-    const uint32_t *thr, *albedo;
+    const uint32_t *thr, *albthr;
+    const float *albedo;
     const uint16_t *guide;
-    uint32_t n_classes, K1, shiftK, n_depth, n_guide, guide_base, guide_shift, cls_steps, depth_bisect;
-    float frac_scale, tau_ext, vh_fs;
-    uint32_t R_q31, R_thr, surface_model;
+    uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, cls_steps, depth_bisect;
+    float tau_ext, R_f, cos_scale_surf;
+    uint32_t R_thr, surface_model;
 };
 
 // half the particle velocity at vertical optical depth Tc, 0 <= Tc <= tau_ext (depth rows: see pdv_device.h).
@@ -103,6 +104,9 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
     const float4 r = cv.rows[j];
     return fmaf(Tc - r.x, Tc < r.x ? r.z : r.w, r.y);
 }
+
+// History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
+enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
 template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
 __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constant__ RunParams P) {
@@ -140,32 +144,34 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
         CloudView cv;
         {
             const DevCloudHeader *h = reinterpret_cast<const DevCloudHeader *>(s_blob);
-            cv.phase = reinterpret_cast<const float *>(s_blob + h->off_phase);
+            cv.phase = reinterpret_cast<const float2 *>(s_blob + h->off_phase);
             cv.rows = reinterpret_cast<const float4 *>(s_blob + h->off_rows);
             cv.thr = reinterpret_cast<const uint32_t *>(s_blob + h->off_thr);
-            cv.albedo = reinterpret_cast<const uint32_t *>(s_blob + (ANALOG ? h->off_albthr : h->off_albedo));
+            cv.albedo = reinterpret_cast<const float *>(s_blob + h->off_albedo);
+            cv.albthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_albthr);
             cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide);
-            cv.n_classes = h->n_classes; cv.K1 = h->K + 1u; cv.shiftK = 32u - h->log2K;
+            cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
             cv.depth_bisect = h->depth_bisect;
             cv.cls_steps = 0;
             while ((1u << cv.cls_steps) < cv.n_classes) ++cv.cls_steps;
-            cv.frac_scale = __uint_as_float((127u - cv.shiftK) << 23);       // 2^-(32-log2K)
-            cv.tau_ext = h->tau_ext; cv.vh_fs = h->vh_fs;
-            cv.R_q31 = h->R_q31; cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
+            cv.tau_ext = h->tau_ext; cv.R_f = h->R_f;
+            cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
-        const uint32_t albedo0 = cv.albedo[0];            // monodisperse: the only class
+        const float albedo0 = cv.albedo[0];               // monodisperse: the only class
+        const uint32_t albthr0 = cv.albthr[0];
 
         // ---- per-thread accumulators (flushed once per unit) ------------------------------------------------
         // acc_lost = sum over finished histories of (1 - final weight) + roulette gains: all weight that went into
-        // particles or the surface; absorbed_particles = acc_lost - acc_abss (same integers as a per-event sum).
+        // particles or the surface; absorbed_particles = acc_lost - acc_abss.
         unsigned long long acc_esc = 0ull, acc_lost = 0ull, acc_abss = 0ull;
         uint32_t cnt_hist = 0u, cnt_ev = 0u, cnt_refl = 0u, max_ev = 0u;
 
         // ---- lane state: one photon history (step (1)) + the lane's private id chunk -------------
+        // nfl = flights flown so far = Philox draw index of the next flight (D1)
         bool alive = true;
-        float T = 0.f, mu = -1.f, vt = 0.f;
-        uint32_t w = kWOne, n_sc = 0u, n_refl = 0u, id_lo = 0u, id_hi = 0u, left = 0u, chunk = P.chunk;
+        float T = 0.f, mu = -1.f, vt = 0.f, w = 1.f, abss = 0.f;
+        uint32_t nfl = 0u, n_refl = 0u, id_lo = 0u, id_hi = 0u, left = 0u, chunk = P.chunk;
 
         // next photon of this lane (or alive = false when the unit is drained); resets the history state
         auto regenerate = [&]() {
@@ -186,21 +192,128 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                     chunk = min(max(__float2uint_rd(__ull2float_rd(rem) * P.chunk_per_remaining), 1u), P.chunk);
                 }
             }
-            T = 0.f; mu = -1.f; vt = 0.f; w = kWOne; n_sc = 0u; n_refl = 0u;
+            T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u; n_refl = 0u;
         };
-        // end of a history (step (7)): per-history bookkeeping, then the lane's next photon
+        // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
         auto finish = [&](int fate) {
-            acc_lost += kWOne - w;
-            cnt_ev += n_sc; cnt_refl += n_refl;
+            const uint32_t wq = __float2uint_rn(w * kWOneF);
+            if (fate == F_EXIT) {
+                if (mu >= P.mu_aperture) {                    // inside the probe aperture: Eq. 19
+                    const float fb = (vt - P.v_lo) * P.inv_dv;
+                    fate = F_DET_OUT;
+                    if (!(fb >= 0.f)) {
+                        smem_add64(&s_stats[ST_UNDER], wq);
+                    } else if (fb >= (float)P.n_bins) {
+                        smem_add64(&s_stats[ST_OVER], wq);
+                    } else {
+                        int bin = (int)fb;
+                        PDV_BOUND(2, bin, P.n_bins);
+                        smem_add64(&s_hist[bin], wq);
+                        smem_add64(&s_hist2[bin], mul_q31(wq, wq));
+                        fate = F_DETECTED;
+                    }
+                } else {
+                    acc_esc += wq;
+                }
+            } else if (fate == F_KILLED) {
+                smem_add64(&s_stats[ST_KILLED], wq);
+            } else if (SSO && fate == F_TRUNC) {
+                smem_add64(&s_stats[ST_TRUNC], wq);
+            }
+            const uint32_t lost = kWOne - wq;
+            acc_lost += lost;
+            acc_abss += min(__float2uint_rn(abss * kWOneF), lost);
+            const uint32_t n_sc = nfl - n_refl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);
+            cnt_ev += nfl - n_refl; cnt_refl += n_refl;       // an absorbing interaction is a particle event too
             max_ev = max(max_ev, n_sc + n_refl);
             if (TRACE) {
                 const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
                 pdv_trace_record r;
-                r.vt = vt; r.weight = (float)((double)w * kWScale); r.mu_exit = mu; r.fate = fate;
+                r.vt = vt; r.weight = w; r.mu_exit = mu; r.fate = fate == F_ABS_PART ? F_ABS_SURF : fate;
                 r.n_scatter = (int)n_sc; r.n_reflect = (int)n_refl;
                 P.trace[idx] = r;
             }
             regenerate();
+        };
+        // One flight (D2): `a` = path word, `cw` = class word (POLY), `b` = phase word, `pw` = azimuth / surface
+        // polar-angle word, `ya` = absorption word (ANALOG), `sub` = which roulette word of the second block.
+        // Returns F_NONE while the history goes on.
+        auto flight = [&](uint32_t a, uint32_t cw, uint32_t b, uint32_t pw, uint32_t ya, uint32_t y_roul, uint32_t sub) -> int {
+            // ---------------- free flight: s = -ln(xi), xi in (0,1]; T' = T - mu s (Eq. 7/10, step (3)) ---------------
+            const float xi = 2.0f - __uint_as_float(0x3F800000u | (a >> 9));
+            const float s = fast_lg2(xi) * -0.69314718056f;
+            const float Tn = fmaf(-mu, s, T);
+            if (Tn < 0.f) return F_EXIT;                      // leaves through the top (step (6))
+            const bool surf = Tn >= cv.tau_ext;               // reaches the free surface
+            if (SSO && !surf && nfl != n_refl) return F_TRUNC;    // single-scatter-only: cut at the 2nd particle event
+            // ---------------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ------
+            T = fminf(Tn, cv.tau_ext);
+            const float vh = depth_half_velocity(cv, T);      // = v_fs / 2 at the surface
+            uint32_t c = 0u;
+            float alb = albedo0;
+            uint32_t albt = albthr0;
+            if (POLY) {
+                for (uint32_t stp = 1u << cv.cls_steps; stp > 1u;) {     // thr padded with 0xffffffff
+                    stp >>= 1;
+                    if (cv.thr[c + stp - 1u] <= cw) c += stp;
+                }
+                c = min(c, cv.n_classes - 1u);
+                if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
+            }
+            if (ANALOG) {                                     // Eq. 11 literally: absorbed with probability 1 - albedo
+                if (ya >= (surf ? cv.R_thr : albt)) {
+                    if (surf) abss = w; else ++nfl;
+                    w = 0.f;
+                    return surf ? F_ABS_SURF : F_ABS_PART;
+                }
+            } else {                                          // implicit capture: Eq. 11 in expectation
+                const float wn = w * (surf ? cv.R_f : alb);
+                if (surf) abss += w - wn;
+                w = wn;
+            }
+            // cos(theta) from D_K (Eq. 13-14): M[k] + (M[k+1] - M[k]) frac in one 64-bit load and one FFMA
+            uint32_t k = b >> cv.shiftK;
+            PDV_BOUND(3, k, cv.K);
+            const float2 m = cv.phase[c * cv.K + k];
+            const float ct = fmaf(m.y, __uint2float_rn(b & cv.frac_mask), m.x);
+            // one cosine serves both: cos(phi), phi = 2 pi pw / 2^32 (Eq. 15), or cos(theta'), theta' = (pi/2) pw / 2^32
+            const float pwf = __uint2float_rn(pw);
+            const float cosv = __cosf(pwf * (surf ? 3.65729519818e-10f : 1.46291807927e-9f));
+            const float sq = fast_sqrt(fabsf(fmaf(-ct, ct, 1.f) * fmaf(-mu, mu, 1.f)));
+            float mu_s = fmaf(mu, ct, -cosv * sq);            // z row of Eq. 16 (Eq. 17 at |mu| = 1)
+            mu_s = fminf(fmaxf(mu_s, -1.f), 1.f);
+            float mu_r = cosv;
+            if (cv.surface_model) mu_r = fast_sqrt(pwf * 2.3283064365386963e-10f);     // Lambertian
+            const float mu_new = surf ? mu_r : mu_s;
+            vt = fmaf(mu_new - mu, vh, vt);                   // Eq. 4 (vh = v/2)
+            mu = mu_new;
+            ++nfl;
+            if (surf) ++n_refl;
+            if (nfl >= P.max_events) {                        // Russian roulette (rare path; nfl >= particle events)
+                if (nfl - n_refl >= P.max_events && w <= P.roulette_p) {
+                    uint32_t yr = y_roul;
+                    if (!ANALOG) {
+                        uint32_t y0, y1, y2, y3;
+                        const uint32_t draw = POLY ? nfl - 1u : (nfl - 1u) >> 1;
+                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, P.key0, P.key1, y0, y1, y2, y3);
+                        yr = sub ? y3 : y2;
+                    }
+                    if (yr < P.roulette_thr) {
+                        const float wn = fminf(w * P.roulette_inv_p, 1.f);
+                        const uint32_t q0 = __float2uint_rn(w * kWOneF), q1 = __float2uint_rn(wn * kWOneF);
+                        const uint32_t gain = q1 > q0 ? q1 - q0 : 0u;
+                        smem_add64(&s_stats[ST_GAINED], gain);
+                        acc_lost += gain;
+                        // surface losses so far go to the tally now: afterwards `abss` again stays below 1 - w
+                        acc_abss += min(__float2uint_rn(abss * kWOneF), kWOne - q0);
+                        abss = 0.f;
+                        w = wn;
+                    } else {
+                        return F_KILLED;
+                    }
+                }
+            }
+            return F_NONE;
         };
 
         {   // initial fill: one atomic per warp hands every lane its first chunk
@@ -220,110 +333,22 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
         }
         while (__any_sync(FULL_MASK, alive)) {
             if (alive) {
-                // ---------------- random numbers of this flight (step (3)) -------------------------------------
-                const uint32_t flight = n_sc + n_refl;
-                uint32_t x0, x1, x2, x3;
-                philox4x32_10(id_lo, id_hi, ud.stream, 2u * flight, P.key0, P.key1, x0, x1, x2, x3);
-                uint32_t y0 = 0u, y1 = 0u;
-                if (ANALOG) {
-                    uint32_t y2, y3;
-                    philox4x32_10(id_lo, id_hi, ud.stream, 2u * flight + 1u, P.key0, P.key1, y0, y1, y2, y3);
-                }
-                // ---------------- free flight: s = -ln(xi), xi in (0,1]; T' = T - mu s (Eq. 7/10) --------------
-                const float xi = 2.0f - __uint_as_float(0x3F800000u | (x0 >> 9));
-                const float s = fast_lg2(xi) * -0.69314718056f;
-                const float Tn = fmaf(-mu, s, T);
-                int fate = -1;                                    // >= 0: the history ends in this iteration
-                if (Tn < 0.f) {
-                    // ------------ leaves through the top (step (6)); Eq. 19 tally inside the aperture ----------
-                    fate = 1;
-                    if (mu >= P.mu_aperture) {
-                        const float fb = (vt - P.v_lo) * P.inv_dv;
-                        fate = 5;
-                        if (!(fb >= 0.f)) {
-                            smem_add64(&s_stats[ST_UNDER], w);
-                        } else if (fb >= (float)P.n_bins) {
-                            smem_add64(&s_stats[ST_OVER], w);
-                        } else {
-                            int bin = (int)fb;
-                            PDV_BOUND(2, bin, P.n_bins);
-                            smem_add64(&s_hist[bin], w);
-                            smem_add64(&s_hist2[bin], mul_q31(w, w));
-                            fate = 0;
-                        }
-                    } else {
-                        acc_esc += w;
-                    }
+                // -------- random numbers (step (3)): one Philox4x32-10 block feeds one flight of a polydisperse cloud
+                // (path, class, phase, azimuth words) or two flights of a monodisperse one (path + phase word each) ------
+                const uint32_t draw = POLY ? nfl : nfl >> 1;
+                uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
+                philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, P.key0, P.key1, x0, x1, x2, x3);
+                if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, P.key0, P.key1, y0, y1, y2, y3);
+                int fate;
+                if (POLY) {
+                    fate = flight(x0, x1, x2, x3, y0, y2, 0u);
                 } else {
-                    const bool surf = Tn >= cv.tau_ext;           // reaches the free surface
-                    if (SSO && !surf && n_sc >= 1u) {             // single-scatter-only mode: cut at the 2nd particle event
-                        smem_add64(&s_stats[ST_TRUNC], w);
-                        fate = 4;
-                    } else {
-                        // -------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ----
-                        T = fminf(Tn, cv.tau_ext);
-                        const float vh = depth_half_velocity(cv, T);           // = v_fs / 2 at the surface
-                        uint32_t c = 0u, alb = albedo0;
-                        if (POLY) {
-                            for (uint32_t stp = 1u << cv.cls_steps; stp > 1u;) {     // thr padded with 0xffffffff
-                                stp >>= 1;
-                                if (cv.thr[c + stp - 1u] <= x1) c += stp;
-                            }
-                            c = min(c, cv.n_classes - 1u);
-                            alb = cv.albedo[c];
-                        }
-                        bool absorbed = false;
-                        if (ANALOG) {                             // Eq. 11 literally: absorbed with probability 1 - albedo
-                            absorbed = y1 >= (surf ? cv.R_thr : alb);
-                        } else {                                  // implicit capture: Eq. 11 in expectation
-                            const uint32_t wn = mul_q31(w, surf ? cv.R_q31 : alb);
-                            if (surf) acc_abss += w - wn;
-                            w = wn;
-                        }
-                        if (ANALOG && absorbed) {
-                            if (surf) acc_abss += w; else ++cnt_ev;           // an absorbing interaction is a particle event
-                            w = 0u;
-                            fate = 2;
-                        } else {
-                            // cos(theta) from D_K (Eq. 13-14), azimuth (Eq. 15); surface: polar angle uniform in [0, pi/2]
-                            const float *M = cv.phase + c * cv.K1;
-                            uint32_t k = x2 >> cv.shiftK;
-                            PDV_BOUND(3, k, cv.K1 - 1u);
-                            const float frac = __uint2float_rn(x2 - (k << cv.shiftK)) * cv.frac_scale;
-                            const float m0 = M[k], m1 = M[k + 1u];
-                            const float ct = fmaf(m1 - m0, frac, m0);
-                            // one cosine serves both: cos(phi), phi = 2 pi x3 / 2^32, or cos(theta'), theta' = (pi/2) x2 / 2^32
-                            const float cosv = __cosf(__uint2float_rn(surf ? x2 : x3) *
-                                                      (surf ? 3.65729519818e-10f : 1.46291807927e-9f));
-                            const float sq = fast_sqrt(fmaxf(fmaf(-ct, ct, 1.f) * fmaf(-mu, mu, 1.f), 0.f));
-                            float mu_s = fmaf(mu, ct, -cosv * sq);                    // z row of Eq. 16 (Eq. 17 at |mu| = 1)
-                            mu_s = fminf(fmaxf(mu_s, -1.f), 1.f);
-                            float mu_r = cosv;
-                            if (cv.surface_model) mu_r = fast_sqrt(__uint2float_rn(x2) * 2.3283064365386963e-10f);   // Lambertian
-                            const float mu_new = surf ? mu_r : mu_s;
-                            vt = fmaf(mu_new - mu, vh, vt);                            // Eq. 4 (vh = v/2)
-                            mu = mu_new;
-                            if (surf) ++n_refl; else ++n_sc;
-                            if (n_sc >= P.max_events && w <= P.roulette_wcap) {      // Russian roulette (rare path)
-                                if (!ANALOG) {
-                                    uint32_t y2, y3;
-                                    philox4x32_10(id_lo, id_hi, ud.stream, 2u * flight + 1u, P.key0, P.key1, y0, y1, y2, y3);
-                                }
-                                if (y0 < P.roulette_thr) {
-                                    uint32_t wn = (uint32_t)__float2uint_rd(__uint2float_rd(w) * P.roulette_inv_p);
-                                    wn = max(min(wn, kWOne), w);
-                                    smem_add64(&s_stats[ST_GAINED], wn - w);
-                                    acc_lost += wn - w;
-                                    w = wn;
-                                } else {
-                                    smem_add64(&s_stats[ST_KILLED], w);
-                                    fate = 3;
-                                }
-                            }
-                        }
-                    }
+                    // azimuth word of a two-word flight: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top -- neither
+                    // the path (top 23 bits of a) nor the phase lookup (top 22 bits of b) reads the two leading ones
+                    fate = flight(x0, 0u, x1, __byte_perm(x0, x1, 0x0412), y0, y2, 0u);
+                    if (fate == F_NONE) fate = flight(x2, 0u, x3, __byte_perm(x2, x3, 0x0412), y1, y3, 1u);
                 }
-                if (fate >= 0) finish(fate);                      // the one place where a lane moves on to its next photon
+                if (fate != F_NONE) finish(fate);             // the one place where a lane moves on to its next photon
             }
         }
 
