@@ -1,6 +1,8 @@
 // pdv_api.cu -- the C-ABI of include/pdv.h: argument checking, cloud upload, workspace, launches, read-back.
 // No arithmetic of the method lives here beyond packing the fp32/fixed-point device tables.
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -104,6 +106,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
             guide.assign(n_guide, 0);
         }
     }
+    if (std::getenv("PDV_X_DEBUG")) fprintf(stderr, "blob: nd=%d n_guide=%u shift=%u bisect=%u tau=%g\n", nd, n_guide, shift, bisect, (double)Tf[nd]);
     DevCloudHeader hd;
     std::memset(&hd, 0, sizeof(hd));
     size_t off = sizeof(DevCloudHeader);
@@ -263,6 +266,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     kv.analog = o->mode == 1;
     kv.sso = o->single_scatter_only != 0;
     kv.trace = trace;
+    kv.roulette = o->max_events > 0;
 
     const DeviceInfo &di = device_info(device);
     if (!di.valid) return fail(PDV_E_CUDA, "cannot query the CUDA device");
@@ -278,7 +282,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         static std::vector<std::pair<Key, int>> cache;       // occupancy queries are not free either
         std::lock_guard<std::mutex> lk(mu);
         for (const auto &e : cache)
-            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace &&
+            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette &&
                 e.first.block == block && e.first.smem == smem && e.first.device == device) { per_sm = e.second; break; }
         if (per_sm == 0) {
             CU(transport_max_blocks_per_sm(kv, block, smem, &per_sm), "occupancy query");
@@ -298,6 +302,11 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     chunk = std::min(std::max(chunk, 1.0), 128.0);
     rp.chunk = (uint32_t)chunk;
     rp.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
+    rp.chunk_min = 1;
+    if (const char *e = std::getenv("PDV_X_CHUNKMIN")) rp.chunk_min = (uint32_t)std::max(1, atoi(e));
+    if (const char *e = std::getenv("PDV_X_CHUNKDIV")) rp.chunk_per_remaining = (float)(1.0 / (atof(e) * threads));
+    if (const char *e = std::getenv("PDV_X_CHUNKMAX")) rp.chunk = (uint32_t)std::max(1, atoi(e));
+    rp.chunk_min = std::min(rp.chunk_min, rp.chunk);
     return PDV_OK;
 }
 

@@ -5,6 +5,15 @@
 
 #include "../../include/pdv.h"
 
+// transport_kernel is compiled for PDV_LB_THREADS threads per block at most and PDV_LB_BLOCKS resident blocks per SM
+// (its register budget = 65536 / (PDV_LB_THREADS * PDV_LB_BLOCKS)).
+#ifndef PDV_LB_THREADS
+#define PDV_LB_THREADS 1024
+#endif
+#ifndef PDV_LB_BLOCKS
+#define PDV_LB_BLOCKS 1
+#endif
+
 namespace pdv {
 
 // Fixed point of every tally: Q31, one photon = 2^31.  A history carries its weight in fp32 (a product of albedos in
@@ -69,7 +78,8 @@ struct RunParams {
     uint32_t n_units;
     uint32_t n_bins;
     uint32_t chunk;                    // photon ids a lane claims per fetch at the start of a unit (guided: shrinks
-    float chunk_per_remaining;         //   to clamp(remaining * chunk_per_remaining, 1, chunk) as the unit drains)
+    float chunk_per_remaining;         //   to clamp(remaining * chunk_per_remaining, chunk_min, chunk) as the unit drains)
+    uint32_t chunk_min;
     uint32_t max_events;               // roulette once n_scatter >= max_events; 0xffffffff: never
     uint32_t roulette_thr;             // survive iff the roulette word < roulette_thr
     float roulette_p;                  // play only while w <= p (then w / p <= 1)
@@ -82,7 +92,7 @@ struct RunParams {
 struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
-struct KernelVariant { bool poly, analog, sso, trace; };   // template instantiation of transport_kernel
+struct KernelVariant { bool poly, analog, sso, trace, roulette; };   // template instantiation of transport_kernel
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,

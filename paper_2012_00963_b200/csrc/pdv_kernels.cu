@@ -2,8 +2,8 @@
 //
 // transport_kernel: persistent-thread photon transport, section II.B steps (1)-(7) (174-183):
 //   * one lane = one photon history at a time; a lane whose photon left the cloud starts its next history in the
-//     same branch ("photon regeneration"), taking ids from a private chunk it claims from the unit's global counter
-//     (guided chunk sizes: large at the start, 1 at the end), so all 32 lanes of a warp fly a photon in every
+//     same pass ("photon regeneration"), taking the next id of its warp's pool; a warp refills its pool from the unit's
+//     global cursor (guided pool sizes: large at the start, 32 at the end), so all 32 lanes of a warp fly a photon in every
 //     iteration until the unit is drained;
 //   * every history draws from its own Philox4x32-10 counter stream, counter = (id_lo, id_hi, unit, 2*flight+sub),
 //     key = seed: results do not depend on which lane, warp or block runs a history (D1/D2);
@@ -26,26 +26,35 @@ __shared__ unsigned int s_dbg[8];
 #define PDV_BOUND(cat, idx, limit) do { } while (0)
 #endif
 
+// Register budget of transport_kernel: PDV_LB_THREADS x PDV_LB_BLOCKS resident threads per SM (pdv_device.h).
 namespace pdv {
 
 #define FULL_MASK 0xffffffffu
 
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
 
-// Philox4x32-10 block function; round keys precomputed on the host (kernel parameter = constant bank).
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                              const uint32_t (&k0)[10], const uint32_t (&k1)[10],
+// Philox4x32-10 block function.  The 10 round keys (k0_r, k1_r) are precomputed on the host and staged in shared memory,
+// two rounds per uint4: five broadcast LDS.128 per block instead of ten constant-bank loads (the ADU pipe that serves
+// LDC was a third busy with the keys alone).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint4 *keys,
                                               uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3) {
 #pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0;
-        const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c2;
-        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0[r];
-        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1[r];
-        c1 = (uint32_t)p1;
-        c3 = (uint32_t)p0;
-        c0 = n0;
-        c2 = n2;
+    for (int r = 0; r < 10; r += 2) {
+        const uint4 k = keys[r >> 1];
+        {
+            const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0;
+            const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c2;
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k.x;
+            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k.y;
+            c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        }
+        {
+            const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0;
+            const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c2;
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k.z;
+            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k.w;
+            c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        }
     }
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
@@ -81,7 +90,7 @@ struct CloudView {               // per-unit scalars and shared-memory table poi
     const float *albedo;
     const uint16_t *guide;
     uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, cls_steps, depth_bisect;
-    float tau_ext, R_f, cos_scale_surf;
+    float tau_ext, R_f, one_minus_R;
     uint32_t R_thr, surface_model;
 };
 
@@ -105,19 +114,57 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
     return fmaf(Tc - r.x, Tc < r.x ? r.z : r.w, r.y);
 }
 
+// ---- rare paths kept out of line: the flight loop stays small, and the compiler cannot fold their conditions into the
+// ---- per-flight gates or turn them into predicated instructions that every flight would issue ------------------------
+
+// Lambertian surface (surface_model 1): mu = sqrt(xi)
+__device__ __noinline__ float lambert_mu(float pwf) { return fast_sqrt(pwf * 2.3283064365386963e-10f); }
+
+// Russian roulette (reading R20) once a history has had max_events particle events: played only while w <= p, so
+// that w / p <= 1.  `yr` is the roulette word of the flight's second Philox block.  Everything by value: a reference
+// parameter would pin the caller's weight registers to local memory.
+struct RouletteOut { float w, abss; uint32_t add_lost, add_abss, killed; };
+__device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, uint32_t thr, float inv_p, unsigned long long *s_stats) {
+    RouletteOut o;
+    o.w = w; o.abss = abss; o.add_lost = 0u; o.add_abss = 0u; o.killed = yr >= thr ? 1u : 0u;
+    if (o.killed) return o;
+    const float wn = fminf(w * inv_p, 1.f);
+    const uint32_t q0 = __float2uint_rn(w * kWOneF), q1 = __float2uint_rn(wn * kWOneF);
+    const uint32_t gain = q1 > q0 ? q1 - q0 : 0u;
+    smem_add64(&s_stats[ST_GAINED], gain);
+    o.add_lost = gain;
+    // surface losses so far go to the tally now: afterwards `abss` again stays below 1 - w
+    o.add_abss = min(__float2uint_rn(abss * kWOneF), kWOne - q0);
+    o.abss = 0.f;
+    o.w = wn;
+    return o;
+}
+
+// second Philox block of a draw (absorption / roulette words), out of line for the roulette path of the implicit-capture kernels
+__device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t draw, const uint4 *keys,
+                                                      uint32_t sub) {
+    uint32_t y0, y1, y2, y3;
+    philox4x32_10(id_lo, id_hi, stream, 2u * draw + 1u, keys, y0, y1, y2, y3);
+    return sub ? y3 : y2;
+}
+
+
 // History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
 enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
-__global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constant__ RunParams P) {
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
+__global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned long long s_stats[ST_COUNT];
+    __shared__ __align__(16) uint4 s_keys[5];
+    __shared__ uint32_t s_pool_next[32];
     __shared__ int s_go;
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u;
     unsigned long long *s_hist = reinterpret_cast<unsigned long long *>(smem);
     unsigned long long *s_hist2 = s_hist + P.n_bins;
     unsigned char *s_blob = smem + 16u * (size_t)P.n_bins;
+    if (tid < 5) s_keys[tid] = make_uint4(P.key0[2 * tid], P.key1[2 * tid], P.key0[2 * tid + 1], P.key1[2 * tid + 1]);
 
     for (uint32_t visit = 0; visit < P.n_units; ++visit) {
         const uint32_t u = (blockIdx.x + visit) % P.n_units;
@@ -155,7 +202,7 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
             cv.depth_bisect = h->depth_bisect;
             cv.cls_steps = 0;
             while ((1u << cv.cls_steps) < cv.n_classes) ++cv.cls_steps;
-            cv.tau_ext = h->tau_ext; cv.R_f = h->R_f;
+            cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
         const float albedo0 = cv.albedo[0];               // monodisperse: the only class
@@ -167,30 +214,34 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
         unsigned long long acc_esc = 0ull, acc_lost = 0ull, acc_abss = 0ull;
         uint32_t cnt_hist = 0u, cnt_ev = 0u, cnt_refl = 0u, max_ev = 0u;
 
-        // ---- lane state: one photon history (step (1)) + the lane's private id chunk -------------
-        // nfl = flights flown so far = Philox draw index of the next flight (D1)
-        bool alive = true;
+        // ---- lane state: one photon history (step (1)) ---------------------------------------------
+        // nfl = flights flown so far = Philox draw index of the next flight (D1).
+        // run: the lane flies a photon; want: it needs a photon id (neither: the unit is drained, the lane is done).
+        bool run = false, want = true;
         float T = 0.f, mu = -1.f, vt = 0.f, w = 1.f, abss = 0.f;
-        uint32_t nfl = 0u, n_refl = 0u, id_lo = 0u, id_hi = 0u, left = 0u, chunk = P.chunk;
+        uint32_t nfl = 0u, n_refl = 0u, id_lo = 0u, id_hi = 0u;
+        // ---- the warp's pool of photon ids: [pool_lo/hi, + pool_len), warp-uniform registers; the hand-out cursor lives in
+        // shared memory so that a lane can take a slice of ids from inside the divergent end-of-history code with one shared
+        // atomic.  Pools are claimed from the unit's global cursor by lane 0 (guided sizes): ~1e4 times fewer global
+        // atomics than one claim per lane -- the single-address L2 atomic rate was what bounded the drain of a unit.
+        uint32_t pool_lo = 0u, pool_hi = 0u, pool_len = 0u, slice = 1u, left = 0u;
+        uint32_t *pool_next = &s_pool_next[tid >> 5];
+        if (lane == 0) *pool_next = 0u;
+        __syncwarp();
 
-        // next photon of this lane (or alive = false when the unit is drained); resets the history state
-        auto regenerate = [&]() {
+        // next photon of this lane: the next id of its private slice, else a new slice of `slice` ids from the warp pool
+        // (want = true if the pool is exhausted); resets the history state
+        auto take_photon = [&]() {
             if (left) {
                 --left;
                 if (++id_lo == 0u) ++id_hi;
             } else {
-                const unsigned long long b = atomicAdd(P.next_id + u, (unsigned long long)chunk);
-                if (b >= P.n_photons) {
-                    alive = false;
-                } else {
-                    const unsigned long long rem = P.n_photons - b;
-                    const uint32_t len = rem < (unsigned long long)chunk ? (uint32_t)rem : chunk;
-                    const unsigned long long id = P.first_id + b;
-                    id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32);
-                    left = len - 1u;
-                    cnt_hist += len;
-                    chunk = min(max(__float2uint_rd(__ull2float_rd(rem) * P.chunk_per_remaining), 1u), P.chunk);
-                }
+                const uint32_t off = atomicAdd(pool_next, slice);
+                run = off < pool_len;
+                want = !run;
+                left = run ? min(slice, pool_len - off) - 1u : 0u;
+                id_lo = pool_lo + off;
+                id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
             }
             T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u; n_refl = 0u;
         };
@@ -200,17 +251,14 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
             if (fate == F_EXIT) {
                 if (mu >= P.mu_aperture) {                    // inside the probe aperture: Eq. 19
                     const float fb = (vt - P.v_lo) * P.inv_dv;
-                    fate = F_DET_OUT;
-                    if (!(fb >= 0.f)) {
-                        smem_add64(&s_stats[ST_UNDER], wq);
-                    } else if (fb >= (float)P.n_bins) {
-                        smem_add64(&s_stats[ST_OVER], wq);
-                    } else {
-                        int bin = (int)fb;
-                        PDV_BOUND(2, bin, P.n_bins);
+                    const uint32_t bin = (uint32_t)__float2int_rd(fb);       // floor; negative -> huge
+                    if (bin < P.n_bins) {
                         smem_add64(&s_hist[bin], wq);
                         smem_add64(&s_hist2[bin], mul_q31(wq, wq));
                         fate = F_DETECTED;
+                    } else {
+                        smem_add64(&s_stats[fb < 0.f ? ST_UNDER : ST_OVER], wq);
+                        fate = F_DET_OUT;
                     }
                 } else {
                     acc_esc += wq;
@@ -233,7 +281,7 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                 r.n_scatter = (int)n_sc; r.n_reflect = (int)n_refl;
                 P.trace[idx] = r;
             }
-            regenerate();
+            take_photon();
         };
         // One flight (D2): `a` = path word, `cw` = class word (POLY), `b` = phase word, `pw` = azimuth / surface
         // polar-angle word, `ya` = absorption word (ANALOG), `sub` = which roulette word of the second block.
@@ -267,9 +315,8 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                     return surf ? F_ABS_SURF : F_ABS_PART;
                 }
             } else {                                          // implicit capture: Eq. 11 in expectation
-                const float wn = w * (surf ? cv.R_f : alb);
-                if (surf) abss += w - wn;
-                w = wn;
+                if (surf) abss = fmaf(w, cv.one_minus_R, abss);
+                w *= surf ? cv.R_f : alb;
             }
             // cos(theta) from D_K (Eq. 13-14): M[k] + (M[k+1] - M[k]) frac in one 64-bit load and one FFMA
             uint32_t k = b >> cv.shiftK;
@@ -280,66 +327,67 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
             const float pwf = __uint2float_rn(pw);
             const float cosv = __cosf(pwf * (surf ? 3.65729519818e-10f : 1.46291807927e-9f));
             const float sq = fast_sqrt(fabsf(fmaf(-ct, ct, 1.f) * fmaf(-mu, mu, 1.f)));
-            float mu_s = fmaf(mu, ct, -cosv * sq);            // z row of Eq. 16 (Eq. 17 at |mu| = 1)
-            mu_s = fminf(fmaxf(mu_s, -1.f), 1.f);
+            // z row of Eq. 16 (Eq. 17 at |mu| = 1).  Rounding may leave |mu| one ulp above 1: harmless, the next square root
+            // takes |(1 - ct^2)(1 - mu^2)|
+            const float mu_s = fmaf(mu, ct, -cosv * sq);
             float mu_r = cosv;
-            if (cv.surface_model) mu_r = fast_sqrt(pwf * 2.3283064365386963e-10f);     // Lambertian
+            if (cv.surface_model) mu_r = lambert_mu(pwf);     // unit-uniform branch
             const float mu_new = surf ? mu_r : mu_s;
             vt = fmaf(mu_new - mu, vh, vt);                   // Eq. 4 (vh = v/2)
             mu = mu_new;
             ++nfl;
-            if (surf) ++n_refl;
-            if (nfl >= P.max_events) {                        // Russian roulette (rare path; nfl >= particle events)
-                if (nfl - n_refl >= P.max_events && w <= P.roulette_p) {
-                    uint32_t yr = y_roul;
-                    if (!ANALOG) {
-                        uint32_t y0, y1, y2, y3;
-                        const uint32_t draw = POLY ? nfl - 1u : (nfl - 1u) >> 1;
-                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, P.key0, P.key1, y0, y1, y2, y3);
-                        yr = sub ? y3 : y2;
-                    }
-                    if (yr < P.roulette_thr) {
-                        const float wn = fminf(w * P.roulette_inv_p, 1.f);
-                        const uint32_t q0 = __float2uint_rn(w * kWOneF), q1 = __float2uint_rn(wn * kWOneF);
-                        const uint32_t gain = q1 > q0 ? q1 - q0 : 0u;
-                        smem_add64(&s_stats[ST_GAINED], gain);
-                        acc_lost += gain;
-                        // surface losses so far go to the tally now: afterwards `abss` again stays below 1 - w
-                        acc_abss += min(__float2uint_rn(abss * kWOneF), kWOne - q0);
-                        abss = 0.f;
-                        w = wn;
-                    } else {
-                        return F_KILLED;
-                    }
-                }
+            n_refl += surf ? 1u : 0u;
+            if (ROUL && nfl - n_refl >= P.max_events && w <= P.roulette_p) {       // Russian roulette (rare path)
+                const uint32_t yr = ANALOG ? y_roul
+                                           : philox_roulette_word(id_lo, id_hi, ud.stream, POLY ? nfl - 1u : (nfl - 1u) >> 1, s_keys, sub);
+                const RouletteOut o = roulette(w, abss, yr, P.roulette_thr, P.roulette_inv_p, s_stats);
+                if (o.killed) return F_KILLED;
+                w = o.w; abss = o.abss; acc_lost += o.add_lost; acc_abss += o.add_abss;
             }
             return F_NONE;
         };
 
-        {   // initial fill: one atomic per warp hands every lane its first chunk
-            unsigned long long b = 0ull;
-            if (lane == 0) b = atomicAdd(P.next_id + u, 32ull * chunk);
-            b = __shfl_sync(FULL_MASK, b, 0) + (unsigned long long)lane * chunk;
-            if (b >= P.n_photons) {
-                alive = false;
-            } else {
-                const unsigned long long rem = P.n_photons - b;
-                const uint32_t len = rem < (unsigned long long)chunk ? (uint32_t)rem : chunk;
-                const unsigned long long id = P.first_id + b;
-                id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32);
-                left = len - 1u;
-                cnt_hist += len;
+        for (;;) {
+            if (__any_sync(FULL_MASK, want)) {
+                // ---- some lane found the warp pool empty: refill it from the unit's cursor (guided self-scheduling: a warp
+                // claims clamp(remaining / (2 warps), 32 chunk_min, 32 chunk) ids, sized from a fresh look at the cursor) and
+                // hand ids to the waiting lanes; lanes still waiting when the unit is drained are done
+                for (;;) {
+                    unsigned long long b = 0ull;
+                    uint32_t len = 0u;
+                    if (lane == 0) {
+                        const unsigned long long seen = *(volatile unsigned long long *)(P.next_id + u);
+                        if (seen < P.n_photons) {
+                            const uint32_t ask = 32u * min(max(__float2uint_rd(__ull2float_rd(P.n_photons - seen) * P.chunk_per_remaining),
+                                                               P.chunk_min), P.chunk);
+                            b = atomicAdd(P.next_id + u, (unsigned long long)ask);
+                            if (b < P.n_photons) {
+                                const unsigned long long rem = P.n_photons - b;
+                                len = rem < (unsigned long long)ask ? (uint32_t)rem : ask;
+                                cnt_hist += len;
+                                *pool_next = 0u;
+                            }
+                        }
+                    }
+                    len = __shfl_sync(FULL_MASK, len, 0);
+                    __syncwarp();                                 // lane 0's cursor reset is visible to the takes below
+                    if (len == 0u) { want = false; break; }
+                    const unsigned long long id0 = P.first_id + __shfl_sync(FULL_MASK, b, 0);
+                    pool_lo = (uint32_t)id0; pool_hi = (uint32_t)(id0 >> 32); pool_len = len;
+                    slice = max(len >> 5, 1u);                    // a lane takes 1/32 of the pool at a time: 1 id from the last pools
+                    if (want) take_photon();
+                    if (!__any_sync(FULL_MASK, want)) break;
+                }
+                if (!__any_sync(FULL_MASK, run)) break;
             }
-        }
-        while (__any_sync(FULL_MASK, alive)) {
-            if (alive) {
+            int fate = F_NONE;
+            if (run) {
                 // -------- random numbers (step (3)): one Philox4x32-10 block feeds one flight of a polydisperse cloud
                 // (path, class, phase, azimuth words) or two flights of a monodisperse one (path + phase word each) ------
                 const uint32_t draw = POLY ? nfl : nfl >> 1;
                 uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
-                philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, P.key0, P.key1, x0, x1, x2, x3);
-                if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, P.key0, P.key1, y0, y1, y2, y3);
-                int fate;
+                philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
+                if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, s_keys, y0, y1, y2, y3);
                 if (POLY) {
                     fate = flight(x0, x1, x2, x3, y0, y2, 0u);
                 } else {
@@ -348,8 +396,9 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
                     fate = flight(x0, 0u, x1, __byte_perm(x0, x1, 0x0412), y0, y2, 0u);
                     if (fate == F_NONE) fate = flight(x2, 0u, x3, __byte_perm(x2, x3, 0x0412), y1, y3, 1u);
                 }
-                if (fate != F_NONE) finish(fate);             // the one place where a lane moves on to its next photon
             }
+            __syncwarp();                                     // histories that ended in either flight are finished in ONE pass
+            if (fate != F_NONE) finish(fate);                 // the one place where a lane moves on to its next photon
         }
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
@@ -402,11 +451,11 @@ __global__ void __launch_bounds__(1024, 1) transport_kernel(const __grid_constan
 
 // ------------------------------------------------------------------------------------------------------------
 // The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
 static cudaError_t ensure_smem(int smem) {
     static int smem_set = 48 * 1024;
     if (smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE>,
+        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         smem_set = smem;
@@ -414,22 +463,23 @@ static cudaError_t ensure_smem(int smem) {
     return cudaSuccess;
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
 static cudaError_t launch_t(const RunParams &rp, LaunchShape s, cudaStream_t st) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE>(s.smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL>(s.smem);
     if (e != cudaSuccess) return e;
-    transport_kernel<POLY, ANALOG, SSO, TRACE><<<s.grid, s.block, s.smem, st>>>(rp);
+    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL><<<s.grid, s.block, s.smem, st>>>(rp);
     return cudaGetLastError();
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
 static cudaError_t occ_t(int block, int smem, int *out) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE>(smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL>(smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE>, block, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL>, block, smem);
 }
 
-#define PDV_D1(FN, A, B, C, ...) (v.trace ? FN<A, B, C, true>(__VA_ARGS__) : FN<A, B, C, false>(__VA_ARGS__))
+#define PDV_D0(FN, A, B, C, D, ...) (v.roulette ? FN<A, B, C, D, true>(__VA_ARGS__) : FN<A, B, C, D, false>(__VA_ARGS__))
+#define PDV_D1(FN, A, B, C, ...) (v.trace ? PDV_D0(FN, A, B, C, true, __VA_ARGS__) : PDV_D0(FN, A, B, C, false, __VA_ARGS__))
 #define PDV_D2(FN, A, B, ...) (v.sso ? PDV_D1(FN, A, B, true, __VA_ARGS__) : PDV_D1(FN, A, B, false, __VA_ARGS__))
 #define PDV_D3(FN, A, ...) (v.analog ? PDV_D2(FN, A, true, __VA_ARGS__) : PDV_D2(FN, A, false, __VA_ARGS__))
 #define PDV_DISPATCH(FN, ...) (v.poly ? PDV_D3(FN, true, __VA_ARGS__) : PDV_D3(FN, false, __VA_ARGS__))
