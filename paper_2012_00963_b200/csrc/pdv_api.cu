@@ -116,6 +116,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * n_pad);
     hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
+    hd.off_cguide = (uint32_t)off; off = align16(off + 256);
     hd.blob_bytes = (uint32_t)off;
     hd.n_classes = nc; hd.K = K; hd.n_depth = nd; hd.n_guide = n_guide; hd.guide_base = base;
     hd.guide_shift = shift; hd.depth_bisect = bisect;
@@ -168,6 +169,16 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
         albt[c] = to_thr32(om);
     }
     std::memcpy(blob.data() + hd.off_guide, guide.data(), sizeof(uint16_t) * n_guide);
+    unsigned char *cg = blob.data() + hd.off_cguide;          // class guide (layout: pdv_device.h)
+    for (uint32_t g = 0; g < 256u; ++g) {
+        const uint32_t first = g << 24, last = first | 0x00FFFFFFu;
+        int below = 0, inside = 0;
+        for (int j = 0; j < nc - 1; ++j) {
+            if (thr[j] <= first) ++below;
+            else if (thr[j] <= last) ++inside;
+        }
+        cg[g] = (unsigned char)(below | (inside > 1 ? 0x80 : 0));
+    }
 }
 
 pdv_status ensure_on_device(const pdv_cloud *c, int device) {

@@ -46,6 +46,10 @@ enum StatSlot {
 // Guide: cell = (float bits of T) >> guide_shift, minus guide_base; guide[cell] = largest j with T_j <= every T of the
 // cell.  The host picks guide_shift so that no cell straddles two bin edges (then one probe is exact); if it cannot,
 // depth_bisect = 1 and the kernel bisects the rows instead.
+// Class guide (polydisperse clouds): the class of a class word cw is  c = #{j < n_classes-1 : thr[j] <= cw}  (cumulative
+// pick probabilities of Eq. 8, R12).  cguide[cw >> 24] holds that count for the first word of the cell in its low
+// 7 bits, and bit 7 is set if more than one threshold lies inside the cell; so  c = low7 + (thr[low7] <= cw)  settles every
+// cell but the flagged ones (tiny classes at the ends of the distribution), which walk on.
 struct DevCloudHeader {
     uint32_t blob_bytes;       // multiple of 16
     uint32_t n_classes, K, log2K, n_depth, n_guide;
@@ -58,7 +62,8 @@ struct DevCloudHeader {
     uint32_t R_thr;            // analog mode: reflected iff xi_absorb word < R_thr
     uint32_t surface_model;
     uint32_t frac_mask;        // the 12 bits of a phase word below its log2K index bits
-    uint32_t pad[7];
+    uint32_t off_cguide;       // class guide: 256 bytes, see below
+    uint32_t pad[6];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 

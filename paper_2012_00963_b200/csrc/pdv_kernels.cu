@@ -89,7 +89,8 @@ struct CloudView {               // per-unit scalars and shared-memory table poi
     const uint32_t *thr, *albthr;
     const float *albedo;
     const uint16_t *guide;
-    uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, cls_steps, depth_bisect;
+    const unsigned char *cguide;
+    uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, depth_bisect;
     float tau_ext, R_f, one_minus_R;
     uint32_t R_thr, surface_model;
 };
@@ -116,6 +117,12 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
 
 // ---- rare paths kept out of line: the flight loop stays small, and the compiler cannot fold their conditions into the
 // ---- per-flight gates or turn them into predicated instructions that every flight would issue ------------------------
+
+// class pick inside a guide cell that holds several thresholds: walk on from c
+__device__ __noinline__ uint32_t class_walk(const uint32_t *thr, uint32_t c, uint32_t last, uint32_t cw) {
+    while (c < last && thr[c] <= cw) ++c;
+    return c;
+}
 
 // Lambertian surface (surface_model 1): mu = sqrt(xi)
 __device__ __noinline__ float lambert_mu(float pwf) { return fast_sqrt(pwf * 2.3283064365386963e-10f); }
@@ -197,11 +204,10 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             cv.albedo = reinterpret_cast<const float *>(s_blob + h->off_albedo);
             cv.albthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_albthr);
             cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide);
+            cv.cguide = s_blob + h->off_cguide;
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
             cv.depth_bisect = h->depth_bisect;
-            cv.cls_steps = 0;
-            while ((1u << cv.cls_steps) < cv.n_classes) ++cv.cls_steps;
             cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
@@ -301,10 +307,11 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             float alb = albedo0;
             uint32_t albt = albthr0;
             if (POLY) {
-                for (uint32_t stp = 1u << cv.cls_steps; stp > 1u;) {     // thr padded with 0xffffffff
-                    stp >>= 1;
-                    if (cv.thr[c + stp - 1u] <= cw) c += stp;
-                }
+                // c = #{j : thr[j] <= cw} through the class guide (pdv_device.h); thr is padded with 0xffffffff
+                const uint32_t e = cv.cguide[cw >> 24];
+                c = e & 0x7Fu;
+                c += cv.thr[c] <= cw ? 1u : 0u;
+                if (e & 0x80u) c = class_walk(cv.thr, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
                 c = min(c, cv.n_classes - 1u);
                 if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
             }
