@@ -36,7 +36,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile the CUDA library if a source is newer than the .so.  Returns the .so path."""
     if force or needs_build():
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        extra = os.environ.get("PDV_NVCC_EXTRA", "").split()          # e.g. -DPDV_BLOCKS_POLY=2 (kernel experiments)
+        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)

@@ -26,6 +26,12 @@ __shared__ unsigned int s_dbg[8];
 #define PDV_BOUND(cat, idx, limit) do { } while (0)
 #endif
 
+#ifndef PDV_BLOCKS_MONO
+#define PDV_BLOCKS_MONO 1
+#endif
+#ifndef PDV_BLOCKS_POLY
+#define PDV_BLOCKS_POLY 4
+#endif
 // Register budget of transport_kernel: PDV_LB_THREADS x PDV_LB_BLOCKS resident threads per SM (pdv_device.h).
 namespace pdv {
 
@@ -390,18 +396,23 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             int fate = F_NONE;
             if (run) {
                 // -------- random numbers (step (3)): one Philox4x32-10 block feeds one flight of a polydisperse cloud
-                // (path, class, phase, azimuth words) or two flights of a monodisperse one (path + phase word each) ------
-                const uint32_t draw = POLY ? nfl : nfl >> 1;
-                uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
-                philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
-                if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, s_keys, y0, y1, y2, y3);
-                if (POLY) {
-                    fate = flight(x0, x1, x2, x3, y0, y2, 0u);
-                } else {
-                    // azimuth word of a two-word flight: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top -- neither
-                    // the path (top 23 bits of a) nor the phase lookup (top 22 bits of b) reads the two leading ones
-                    fate = flight(x0, 0u, x1, __byte_perm(x0, x1, 0x0412), y0, y2, 0u);
-                    if (fate == F_NONE) fate = flight(x2, 0u, x3, __byte_perm(x2, x3, 0x0412), y1, y3, 1u);
+                // (path, class, phase, azimuth words) or two flights of a monodisperse one (path + phase word each).
+                // PDV_BLOCKS_* blocks per pass: the end-of-history code below runs at the few lanes whose history ended, so it
+                // is entered once per several flights; a lane whose history ended waits for the others meanwhile ------
+#pragma unroll 1
+                for (int blk = 0; blk < (POLY ? PDV_BLOCKS_POLY : PDV_BLOCKS_MONO) && fate == F_NONE; ++blk) {
+                    const uint32_t draw = POLY ? nfl : nfl >> 1;
+                    uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
+                    philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
+                    if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, s_keys, y0, y1, y2, y3);
+                    if (POLY) {
+                        fate = flight(x0, x1, x2, x3, y0, y2, 0u);
+                    } else {
+                        // azimuth word of a two-word flight: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top -- neither
+                        // the path (top 23 bits of a) nor the phase lookup (top 22 bits of b) reads the two leading ones
+                        fate = flight(x0, 0u, x1, __byte_perm(x0, x1, 0x0412), y0, y2, 0u);
+                        if (fate == F_NONE) fate = flight(x2, 0u, x3, __byte_perm(x2, x3, 0x0412), y1, y3, 1u);
+                    }
                 }
             }
             __syncwarp();                                     // histories that ended in either flight are finished in ONE pass
