@@ -186,6 +186,43 @@ pdv_status pdv_spectrogram(const double *hist, int32_t n_snap, int32_t n_bins, u
                            double v_lo, double v_hi, int32_t scale, float floor_db, float *out,
                            int32_t on_device, void *cuda_stream);
 
+/* Characteristics of the main peak of each spectrum of a stack (section III.B: the three quantities of Eq. 35,
+ * PAPER.md:356-365, which the paper reads off its MC spectra in Figs. 13-15).  For row i, with x = v/v_fs[i]:
+ *   1. S[k] = hist[i][k] / (n_photons dx), dx = (v_hi - v_lo) / (n_bins v_fs[i]): density of detected weight per unit x;
+ *      bin centre x_k = (v_lo + (k + 1/2) dv) / v_fs[i];
+ *   2. k* = arg-max (first on ties) of S smoothed by `smooth_passes` passes of a centred moving average of half-width
+ *      `smooth_half` bins (mean over the bins that exist at the array ends), over the bins with x_min <= x_k <= x_max
+ *      (x_min > 1 keeps the free-surface peak of thin clouds, out of the search);
+ *   3. unweighted least-squares parabola through the UNSMOOTHED S[k], |k - k*| <= fit_half (bins that exist):
+ *      x_peak = vertex position, i_peak = vertex value, curvature = S''/S at the vertex (per unit x squared).
+ * status: 0 ok; 1 no bin in the search range (k_peak = -1) or fewer than 3 bins in the fit window; 2 the parabola has no
+ * maximum -- then x_peak = x_{k*}, i_peak = smoothed S[k*], curvature = 0.
+ * All arithmetic is fp64.  Steps 1-2 use the same operation order as their definition (sequential sums, no fused
+ * multiply-add), so k* is reproducible bit for bit. */
+typedef struct {
+    size_t struct_size;          /* sizeof(pdv_peak_opts) */
+    int32_t smooth_half;         /* >= 0 */
+    int32_t smooth_passes;       /* >= 0 */
+    int32_t fit_half;            /* >= 1 */
+    int32_t pad;
+    double x_min, x_max;         /* search range in x = v / v_fs; x_max >= x_min */
+} pdv_peak_opts;
+
+typedef struct {
+    double x_peak;               /* v~_peak / v_fs            (Eq. 31) */
+    double i_peak;               /* spectrum value at the peak (Eq. 32), density per unit x */
+    double curvature;            /* I''/I at the peak          (Eq. 34), per unit x squared */
+    int32_t k_peak;              /* arg-max bin k*, -1 if none */
+    int32_t status;
+} pdv_peak;
+
+/* hist [n_units][n_bins] doubles, v_fs [n_units] doubles (m/s, > 0), out [n_units]: all three HOST when on_device = 0,
+ * all three DEVICE when on_device = 1 (then the work is enqueued on cuda_stream and the call does not wait).
+ * n_bins <= PDV_MAX_BINS; n_units = 0 is valid.  Errors: PDV_E_INVALID for NULLs / bad sizes / bad opts, PDV_E_CUDA. */
+pdv_status pdv_spectrum_peaks(const double *hist, int32_t n_units, int32_t n_bins, uint64_t n_photons,
+                              double v_lo, double v_hi, const double *v_fs, const pdv_peak_opts *opts,
+                              pdv_peak *out, int32_t on_device, void *cuda_stream);
+
 /* Measures the issue-rate denominators on the current device: a dependent-free FFMA stream and a MUFU
  * stream, each run for ~`millis` ms on every SM.  Outputs (any may be NULL): thread-instructions/s of each,
  * the SM clock in MHz observed meanwhile (clock64 over globaltimer), and the SM count. */

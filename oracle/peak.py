@@ -33,12 +33,15 @@ import numpy as np
 
 def moving_average(s: np.ndarray, half: int) -> np.ndarray:
     """One pass of R28's centred moving average: out[k] = mean of s[max(0,k-half) .. min(n-1,k+half)]."""
-    s = np.asarray(s, dtype=np.float64)
+    s = [float(v) for v in np.asarray(s, dtype=np.float64)]
     n = len(s)
     out = np.empty(n)
     for k in range(n):
         lo, hi = max(0, k - half), min(n - 1, k + half)
-        out[k] = np.sum(s[lo:hi + 1]) / (hi - lo + 1)
+        acc = 0.0
+        for j in range(lo, hi + 1):                    # in index order: the arg-max of R28 must not depend on a summation trick
+            acc += s[j]
+        out[k] = acc / (hi - lo + 1)
     return out
 
 

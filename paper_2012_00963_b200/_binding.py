@@ -18,7 +18,7 @@ PDV_MAX_CLASSES = 32
 PDV_MAX_BINS = 8192
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
-           "pdv_cloud_get_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_issue_peaks",
+           "pdv_cloud_get_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_issue_peaks",
            "pdv_last_launch_info", "pdv_last_error", "pdv_version")
 
 
@@ -59,6 +59,13 @@ STAT_INTS = ("histories", "particle_events", "surface_reflections", "max_events_
 STATS_DTYPE = np.dtype([(n, "f8") for n in STAT_FLOATS] + [(n, "u8") for n in STAT_INTS])
 TRACE_DTYPE = np.dtype([("vt", "f4"), ("weight", "f4"), ("mu_exit", "f4"), ("fate", "i4"), ("n_scatter", "i4"),
                         ("n_reflect", "i4")])
+PEAK_DTYPE = np.dtype([("x_peak", "f8"), ("i_peak", "f8"), ("curvature", "f8"), ("k_peak", "i4"), ("status", "i4")])
+
+
+class PeakOpts(C.Structure):
+    _fields_ = [("struct_size", C.c_size_t), ("smooth_half", C.c_int32), ("smooth_passes", C.c_int32),
+                ("fit_half", C.c_int32), ("pad", C.c_int32), ("x_min", C.c_double), ("x_max", C.c_double)]
+
 
 _lib = None
 
@@ -83,6 +90,8 @@ def lib() -> C.CDLL:
         L.pdv_mc_trace.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint64, C.POINTER(RunOpts), vp, vp, vp, vp, vp]
         L.pdv_spectrogram.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_double, C.c_double, C.c_int32,
                                       C.c_float, vp, C.c_int32, vp]
+        L.pdv_spectrum_peaks.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_double, C.c_double, vp,
+                                         C.POINTER(PeakOpts), vp, C.c_int32, vp]
         L.pdv_issue_peaks.argtypes = [C.c_double, dp, dp, dp, C.POINTER(C.c_int32), vp]
         L.pdv_last_launch_info.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32),
                                            C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -285,6 +294,37 @@ def pdv_spectrogram(hist, n_photons: int, v_lo: float, v_hi: float, scale: int =
         stream = torch.cuda.current_stream().cuda_stream
     _check(lib().pdv_spectrogram(hist.data_ptr(), hist.shape[0], hist.shape[1], int(n_photons), v_lo, v_hi, scale,
                                  floor_db, out.data_ptr(), 1, C.c_void_p(stream)))
+    return out
+
+
+def pdv_spectrum_peaks(hist, n_photons: int, v_lo: float, v_hi: float, v_fs, *, half: int = 4, n_pass: int = 2,
+                       fit_half: int = 8, x_min: float = 1.02, x_max: float = 1e30, stream: int | None = None):
+    """Main-peak characteristics (Eq. 35) of each row of hist [n_units, n_bins].
+
+    numpy float64 hist + scalar / array v_fs -> numpy structured array of PEAK_DTYPE;
+    CUDA float64 tensors hist [n_units, n_bins] and v_fs [n_units] -> CUDA uint8 tensor of n_units * PEAK_DTYPE.itemsize
+    bytes (enqueued on the stream; `.cpu().numpy().view(PEAK_DTYPE)` reads it)."""
+    o = PeakOpts(C.sizeof(PeakOpts), int(half), int(n_pass), int(fit_half), 0, float(x_min), float(x_max))
+    if isinstance(hist, np.ndarray):
+        h = np.ascontiguousarray(hist, dtype=np.float64)
+        if h.ndim != 2:
+            raise ValueError("hist must be [n_units, n_bins]")
+        v = np.ascontiguousarray(np.broadcast_to(np.asarray(v_fs, dtype=np.float64), (h.shape[0],)))
+        out = np.zeros(h.shape[0], dtype=PEAK_DTYPE)
+        _check(lib().pdv_spectrum_peaks(h.ctypes.data, h.shape[0], h.shape[1], int(n_photons), v_lo, v_hi, v.ctypes.data,
+                                        C.byref(o), out.ctypes.data, 0, C.c_void_p(stream)))
+        return out
+    import torch
+    if not (hist.is_cuda and hist.dtype == torch.float64 and hist.is_contiguous() and hist.dim() == 2):
+        raise ValueError("hist must be a contiguous 2-D CUDA float64 tensor")
+    if not (torch.is_tensor(v_fs) and v_fs.is_cuda and v_fs.dtype == torch.float64 and v_fs.is_contiguous()
+            and v_fs.numel() == hist.shape[0]):
+        raise ValueError("v_fs must be a contiguous CUDA float64 tensor with one value per row of hist")
+    out = torch.empty(hist.shape[0] * PEAK_DTYPE.itemsize, dtype=torch.uint8, device=hist.device)
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    _check(lib().pdv_spectrum_peaks(hist.data_ptr(), hist.shape[0], hist.shape[1], int(n_photons), v_lo, v_hi,
+                                    v_fs.data_ptr(), C.byref(o), out.data_ptr(), 1, C.c_void_p(stream)))
     return out
 
 

@@ -576,6 +576,49 @@ pdv_status pdv_spectrogram(const double *hist, int32_t n_snap, int32_t n_bins, u
     return PDV_OK;
 }
 
+pdv_status pdv_spectrum_peaks(const double *hist, int32_t n_units, int32_t n_bins, uint64_t n_photons, double v_lo, double v_hi,
+                              const double *v_fs, const pdv_peak_opts *opts, pdv_peak *out, int32_t on_device, void *cuda_stream) {
+    g_err.clear();
+    if (!hist || !v_fs || !out || !opts) return fail(PDV_E_INVALID, "hist / v_fs / opts / out is NULL");
+    if (opts->struct_size != sizeof(pdv_peak_opts)) return fail(PDV_E_INVALID, "opts->struct_size mismatch");
+    if (n_units < 0 || n_bins < 1 || n_bins > PDV_MAX_BINS) return fail(PDV_E_INVALID, "need n_units >= 0, 1 <= n_bins <= PDV_MAX_BINS");
+    if (!(v_hi > v_lo) || !std::isfinite(v_hi) || !std::isfinite(v_lo)) return fail(PDV_E_INVALID, "need v_hi > v_lo");
+    if (opts->smooth_half < 0 || opts->smooth_passes < 0 || opts->fit_half < 1 || opts->smooth_half > PDV_MAX_BINS ||
+        opts->smooth_passes > 16 || opts->fit_half > PDV_MAX_BINS)
+        return fail(PDV_E_INVALID, "need 0 <= smooth_half, 0 <= smooth_passes <= 16, 1 <= fit_half (windows at most PDV_MAX_BINS)");
+    if (!(opts->x_max >= opts->x_min)) return fail(PDV_E_INVALID, "need x_max >= x_min");
+    if (n_units == 0) return PDV_OK;
+    if (!on_device)
+        for (int i = 0; i < n_units; ++i)
+            if (!(v_fs[i] > 0.0) || !std::isfinite(v_fs[i])) return fail(PDV_E_INVALID, "v_fs must be > 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (on_device) {
+        CU(launch_peaks(hist, n_units, n_bins, (double)n_photons, v_lo, v_hi, v_fs, *opts, out, st), "peak kernel launch");
+        return PDV_OK;
+    }
+    int device = 0;
+    CU(cudaGetDevice(&device), "cudaGetDevice");
+    const size_t n = (size_t)n_units * n_bins;
+    const size_t off_v = align16(8 * n), off_o = align16(off_v + 8 * (size_t)n_units);
+    unsigned char *ws = nullptr;
+    pdv_status s = get_workspace(off_o + sizeof(pdv_peak) * (size_t)n_units, device, &ws);
+    if (s != PDV_OK) return s;
+    std::vector<pdv_peak> tmp(n_units);
+    CU(cudaMemcpyAsync(ws, hist, 8 * n, cudaMemcpyHostToDevice, st), "copy hist");
+    CU(cudaMemcpyAsync(ws + off_v, v_fs, 8 * (size_t)n_units, cudaMemcpyHostToDevice, st), "copy v_fs");
+    CU(launch_peaks(reinterpret_cast<double *>(ws), n_units, n_bins, (double)n_photons, v_lo, v_hi,
+                    reinterpret_cast<double *>(ws + off_v), *opts, reinterpret_cast<pdv_peak *>(ws + off_o), st), "peak kernel launch");
+    CU(cudaMemcpyAsync(tmp.data(), ws + off_o, sizeof(pdv_peak) * (size_t)n_units, cudaMemcpyDeviceToHost, st), "read back peaks");
+    CU(cudaStreamSynchronize(st), "peak kernel execution");
+    std::memcpy(out, tmp.data(), sizeof(pdv_peak) * (size_t)n_units);
+    return PDV_OK;
+}
+
 pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mhz, int32_t *n_sm, void *cuda_stream) {
     g_err.clear();
     int ndev = 0;

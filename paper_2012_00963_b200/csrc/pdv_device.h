@@ -105,6 +105,8 @@ cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long 
                             cudaStream_t st);
 cudaError_t launch_spectrogram(const double *hist, int n_snap, int n_bins, double inv_n, double inv_dv, int scale,
                                float floor_db, float *out, cudaStream_t st);
+cudaError_t launch_peaks(const double *hist, int n_units, int n_bins, double n_photons, double v_lo, double v_hi,
+                         const double *v_fs, const pdv_peak_opts &o, pdv_peak *out, cudaStream_t st);
 cudaError_t launch_issue_peaks(double millis, double *ffma, double *mufu, double *mhz, int n_sm, cudaStream_t st);
 
 }  // namespace pdv

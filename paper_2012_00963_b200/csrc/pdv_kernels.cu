@@ -569,6 +569,100 @@ cudaError_t launch_spectrogram(const double *hist, int n_snap, int n_bins, doubl
     return cudaGetLastError();
 }
 
+// ---- main-peak characteristics of each spectrum (Eq. 35; steps 1-3 of pdv_spectrum_peaks in include/pdv.h) -----------
+// One block per spectrum.  Steps 1-2 (density, moving averages, arg-max) decide an integer, so they use the operation
+// order of their definition with explicit round-to-nearest adds / multiplies / divides: no fused multiply-add.
+__global__ void __launch_bounds__(256) peak_kernel(const double *hist, int n_bins, double n_photons, double v_lo, double v_hi,
+                                                   const double *v_fs, pdv_peak_opts o, pdv_peak *out) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    double *a = reinterpret_cast<double *>(smem), *b = a + n_bins;
+    __shared__ double red_v[256];
+    __shared__ int red_k[256];
+    const int u = blockIdx.x, tid = threadIdx.x;
+    const double *h = hist + (size_t)u * n_bins;
+    const double vfs = v_fs[u];
+    const double dv = __ddiv_rn(__dsub_rn(v_hi, v_lo), (double)n_bins);
+    const double dx = __ddiv_rn(dv, vfs);
+    const double denom = __dmul_rn(n_photons, dx);
+    auto xk = [&](int k) { return __ddiv_rn(__dadd_rn(v_lo, __dmul_rn(__dadd_rn((double)k, 0.5), dv)), vfs); };
+    auto sk = [&](int k) { return n_photons > 0.0 ? __ddiv_rn(h[k], denom) : 0.0; };
+    for (int k = tid; k < n_bins; k += blockDim.x) a[k] = sk(k);
+    __syncthreads();
+    for (int p = 0; p < o.smooth_passes; ++p) {               // centred moving average, windows cut at the array ends
+        for (int k = tid; k < n_bins; k += blockDim.x) {
+            const int lo = max(0, k - o.smooth_half), hi = min(n_bins - 1, k + o.smooth_half);
+            double sum = 0.0;
+            for (int j = lo; j <= hi; ++j) sum = __dadd_rn(sum, a[j]);
+            b[k] = __ddiv_rn(sum, (double)(hi - lo + 1));
+        }
+        __syncthreads();
+        double *t = a; a = b; b = t;
+    }
+    // arg-max over the search range, first bin on ties
+    double best = -1.0;                                        // S >= 0: any bin in range beats it
+    int kb = -1;
+    for (int k = tid; k < n_bins; k += blockDim.x) {
+        const double x = xk(k);
+        if (x >= o.x_min && x <= o.x_max && a[k] > best) { best = a[k]; kb = k; }
+    }
+    red_v[tid] = best; red_k[tid] = kb;
+    __syncthreads();
+    for (int s = blockDim.x >> 1; s > 0; s >>= 1) {
+        if (tid < s) {
+            const double v2 = red_v[tid + s];
+            const int k2 = red_k[tid + s];
+            const bool take = k2 >= 0 && (red_k[tid] < 0 || v2 > red_v[tid] || (v2 == red_v[tid] && k2 < red_k[tid]));
+            if (take) { red_v[tid] = v2; red_k[tid] = k2; }
+        }
+        __syncthreads();
+    }
+    if (tid != 0) return;
+    pdv_peak r;
+    const int ks = red_k[0];
+    r.k_peak = ks; r.x_peak = 0.0; r.i_peak = 0.0; r.curvature = 0.0; r.status = 1;
+    if (ks >= 0) {
+        r.x_peak = xk(ks); r.i_peak = a[ks];
+        const int lo = max(0, ks - o.fit_half), hi = min(n_bins - 1, ks + o.fit_half);
+        if (hi - lo + 1 >= 3) {
+            // least squares S ~ A + B j + C j^2 in bin units j = k - k*: normal equations, solved by Cramer's rule
+            double s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0, t0 = 0, t1 = 0, t2 = 0;
+            for (int k = lo; k <= hi; ++k) {
+                const double j = (double)(k - ks), y = sk(k), j2 = j * j;
+                s0 += 1.0; s1 += j; s2 += j2; s3 += j2 * j; s4 += j2 * j2;
+                t0 += y; t1 += y * j; t2 += y * j2;
+            }
+            const double det = s0 * (s2 * s4 - s3 * s3) - s1 * (s1 * s4 - s3 * s2) + s2 * (s1 * s3 - s2 * s2);
+            const double A = (t0 * (s2 * s4 - s3 * s3) - s1 * (t1 * s4 - s3 * t2) + s2 * (t1 * s3 - s2 * t2)) / det;
+            const double B = (s0 * (t1 * s4 - t2 * s3) - t0 * (s1 * s4 - s3 * s2) + s2 * (s1 * t2 - s2 * t1)) / det;
+            const double C = (s0 * (s2 * t2 - s3 * t1) - s1 * (s1 * t2 - s2 * t1) + t0 * (s1 * s3 - s2 * s2)) / det;
+            if (C < 0.0) {
+                const double ip = A - B * B / (4.0 * C);
+                r.x_peak = xk(ks) - dx * B / (2.0 * C);
+                r.i_peak = ip;
+                r.curvature = 2.0 * C / (dx * dx * ip);
+                r.status = 0;
+            } else {
+                r.status = 2;
+            }
+        }
+    }
+    out[u] = r;
+}
+
+cudaError_t launch_peaks(const double *hist, int n_units, int n_bins, double n_photons, double v_lo, double v_hi,
+                         const double *v_fs, const pdv_peak_opts &o, pdv_peak *out, cudaStream_t st) {
+    if (n_units == 0) return cudaSuccess;
+    const int smem = 16 * n_bins;
+    static int smem_set = 48 * 1024;
+    if (smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    peak_kernel<<<n_units, 256, smem, st>>>(hist, n_bins, n_photons, v_lo, v_hi, v_fs, o, out);
+    return cudaGetLastError();
+}
+
 // ---- issue-rate microbenchmarks: the FP32/SFU denominators of the roofline ---------------------
 // Each thread runs 8 independent chains so the pipe, not the dependency latency, limits the rate.
 __global__ void __launch_bounds__(512) ffma_peak_kernel(unsigned long long iters, float seed, float *sink,

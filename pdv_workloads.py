@@ -95,3 +95,25 @@ def scaled(cfg: dict, n_photons: int, n_snap: int | None = None, n_clouds: int |
 def paper_base_case(n_photons=1e7, seed=7) -> dict:
     return dict(name="paper_fig4", clouds=[_cloud(20.0, 10.0, 2000.0, lognormal=(1.5, 0.5, 16))],
                 t_snap=[2.0e-6], run=_run(n_photons, seed, 512, 6000.0))
+
+
+# The paper's parameter studies around that base case (section III.A; Figs. 7-10) and the two
+# optical thicknesses of Figs. 13-15 (tau0 = 23.4 <-> m0 = 20 mg/cm^2, d_m = 1.5 um; tau0 = 8.6 <->
+# m0 = 10 mg/cm^2, d_m = 2.0 um; sigma = 0.5) over "a large range of velocity profiles".  The swept values are not
+# printed in the text (they are in the figures); the ones below bracket the base case.  One launch runs a whole sweep.
+PAPER_SWEEPS = {
+    "fig7_beta": [dict(m0=20.0, beta=b, d_m=1.5, sigma=0.5) for b in (6.0, 8.0, 10.0, 12.0, 14.0)],
+    "fig8_m0": [dict(m0=m, beta=10.0, d_m=1.5, sigma=0.5) for m in (2.0, 5.0, 10.0, 20.0, 40.0)],
+    "fig9_dm": [dict(m0=20.0, beta=10.0, d_m=d, sigma=0.5) for d in (0.5, 1.0, 1.5, 2.0, 3.0)],
+    "fig10_sigma": [dict(m0=20.0, beta=10.0, d_m=1.5, sigma=s) for s in (0.3, 0.4, 0.5, 0.6, 0.7)],
+    "fig13_15": [dict(m0=m, beta=b, d_m=d, sigma=0.5) for (m, d) in ((20.0, 1.5), (10.0, 2.0))
+                 for b in (4.0, 6.0, 8.0, 10.0, 12.0, 16.0, 20.0)],
+}
+
+
+def paper_sweep(name: str, n_photons=1e7, seed=11, n_bins=1024, v_fs=2000.0) -> dict:
+    """One of PAPER_SWEEPS as a multi-cloud workload; `points` keeps the swept parameters of each cloud."""
+    pts = PAPER_SWEEPS[name]
+    return dict(name=f"paper_{name}", points=copy.deepcopy(pts),
+                clouds=[_cloud(p["m0"], p["beta"], v_fs, lognormal=(p["d_m"], p["sigma"], 16)) for p in pts],
+                t_snap=[2.0e-6], run=_run(n_photons, seed, n_bins, 3.0 * v_fs))

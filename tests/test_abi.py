@@ -115,6 +115,17 @@ def test_run_argument_validation_and_no_cpu_fallback():
         assert e.value.status == 3 and "no CPU fallback" in str(e.value)
         with pytest.raises(P.PdvError):
             P.pdv_spectrogram(np.ones((2, 4)), 10, 0.0, 1.0)
+        with pytest.raises(P.PdvError) as e:
+            P.pdv_spectrum_peaks(np.ones((2, 64)), 10, 0.0, 6000.0, 2000.0)
+        assert e.value.status == 3 and "no CPU fallback" in str(e.value)
+    for bad in (dict(half=-1), dict(n_pass=17), dict(fit_half=0), dict(x_min=2.0, x_max=1.0)):      # rejected before any CUDA call
+        with pytest.raises(P.PdvError) as e:
+            P.pdv_spectrum_peaks(np.ones((2, 64)), 10, 0.0, 6000.0, 2000.0, **bad)
+        assert e.value.status == 1
+    with pytest.raises(P.PdvError) as e:
+        P.pdv_spectrum_peaks(np.ones((2, 64)), 10, 0.0, 6000.0, [2000.0, 0.0])
+    assert e.value.status == 1
+    assert len(P.pdv_spectrum_peaks(np.ones((0, 64)), 10, 0.0, 6000.0, 2000.0)) == 0                 # n_units = 0 is valid
 
 
 def test_product_does_not_import_oracle():
