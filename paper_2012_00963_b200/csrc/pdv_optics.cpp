@@ -13,6 +13,7 @@
 #include <algorithm>
 #include <cmath>
 #include <complex>
+#include <thread>
 
 namespace pdv {
 
@@ -78,20 +79,44 @@ void mie_efficiencies(double x, double m_re, double m_im, double *k_ext, double 
     if (g) *g = (ss > 0.0) ? 2.0 * sg / ss : 0.0;      // g = (4/(x^2 K_sca)) sg with K_sca = c ss
 }
 
-// |S1|^2 + |S2|^2 at mu (Eq. 13-14) with pi_n, tau_n by upward recurrence.
-static double mie_intensity(const std::vector<cplx> &a, const std::vector<cplx> &b, double mu) {
-    double pi_prev = 0.0, pi_cur = 1.0;                 // pi_0, pi_1
-    cplx s1(0.0, 0.0), s2(0.0, 0.0);
-    const int N = (int)a.size();
-    for (int n = 1; n <= N; ++n) {
-        const double tau = n * mu * pi_cur - (n + 1.0) * pi_prev;
-        const double f = (2.0 * n + 1.0) / (n * (n + 1.0));
-        s1 += f * (a[n - 1] * pi_cur + b[n - 1] * tau);
-        s2 += f * (a[n - 1] * tau + b[n - 1] * pi_cur);
-        const double pi_next = ((2.0 * n + 1.0) * mu * pi_cur - (n + 1.0) * pi_prev) / n;
-        pi_prev = pi_cur; pi_cur = pi_next;
+// |S1|^2 + |S2|^2 (Eq. 13-14) with pi_n, tau_n by upward recurrence:
+// g(psi_i) = (|S1|^2 + |S2|^2)(mu_i) sin(psi_i), mu_i = -cos(psi_i), psi_i = i h, for i0 <= i < i1: the same sums as
+// mie_intensity, 16 nodes abreast so that the compiler turns the inner loops into vector instructions.
+// fa = (2n+1)/(n(n+1)) a_n, fb likewise.
+#define PDV_INTENSITY_NODES_BODY                                                                                     \
+    constexpr int B = 16;                                                                                            \
+    double cj[B], sj[B];                                                                                             \
+    for (int j = 0; j < B; ++j) { cj[j] = std::cos(j * h); sj[j] = std::sin(j * h); }                                \
+    for (int base = i0; base < i1; base += B) {                                                                      \
+        double mu[B], sn[B], pp[B], pc[B], s1r[B], s1i[B], s2r[B], s2i[B];                                           \
+        const double cb = std::cos(base * h), sb = std::sin(base * h);    /* angle addition: 2 libm calls per 16 nodes */ \
+        for (int j = 0; j < B; ++j) {                                                                                \
+            mu[j] = -(cb * cj[j] - sb * sj[j]); sn[j] = sb * cj[j] + cb * sj[j];                                     \
+            pp[j] = 0.0; pc[j] = 1.0; s1r[j] = s1i[j] = s2r[j] = s2i[j] = 0.0;                                       \
+        }                                                                                                            \
+        for (int n = 1; n <= n_terms; ++n) {                                                                         \
+            const double ar = fa_re[n - 1], ai = fa_im[n - 1], br = fb_re[n - 1], bi = fb_im[n - 1];                 \
+            const double dn = (double)n, c1 = (2.0 * n + 1.0) / n, c2 = (n + 1.0) / n;                               \
+            for (int j = 0; j < B; ++j) {                                                                            \
+                const double tau = dn * mu[j] * pc[j] - (dn + 1.0) * pp[j];                                          \
+                s1r[j] += ar * pc[j] + br * tau; s1i[j] += ai * pc[j] + bi * tau;                                    \
+                s2r[j] += ar * tau + br * pc[j]; s2i[j] += ai * tau + bi * pc[j];                                    \
+                const double pn = c1 * mu[j] * pc[j] - c2 * pp[j];                                                   \
+                pp[j] = pc[j]; pc[j] = pn;                                                                           \
+            }                                                                                                        \
+        }                                                                                                            \
+        for (int j = 0; j < B && base + j < i1; ++j)                                                                 \
+            gv[base + j] = (s1r[j] * s1r[j] + s1i[j] * s1i[j] + s2r[j] * s2r[j] + s2i[j] * s2i[j]) * sn[j];          \
     }
-    return std::norm(s1) + std::norm(s2);
+
+static void intensity_nodes_generic(const double *fa_re, const double *fa_im, const double *fb_re, const double *fb_im,
+                                    int n_terms, double h, int i0, int i1, double *gv) {
+    PDV_INTENSITY_NODES_BODY
+}
+__attribute__((target("avx2,fma"))) static void intensity_nodes_avx2(const double *fa_re, const double *fa_im,
+                                                                     const double *fb_re, const double *fb_im, int n_terms,
+                                                                     double h, int i0, int i1, double *gv) {
+    PDV_INTENSITY_NODES_BODY
 }
 
 void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M) {
@@ -102,9 +127,27 @@ void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M) {
     const int N = 2 * n_panel;
     const double h = kPi / N;
     std::vector<double> gv(N + 1);
-    for (int i = 0; i <= N; ++i) {
-        const double psi = i * h;
-        gv[i] = mie_intensity(a, b, -std::cos(psi)) * std::sin(psi);
+    {   // the nodes are independent: contiguous chunks on the host's cores, 16 nodes at a time through the SIMD units
+        std::vector<double> fa_re(a.size()), fa_im(a.size()), fb_re(a.size()), fb_im(a.size());
+        for (size_t n = 1; n <= a.size(); ++n) {
+            const double f = (2.0 * n + 1.0) / (n * (n + 1.0));
+            fa_re[n - 1] = f * a[n - 1].real(); fa_im[n - 1] = f * a[n - 1].imag();
+            fb_re[n - 1] = f * b[n - 1].real(); fb_im[n - 1] = f * b[n - 1].imag();
+        }
+        const bool avx2 = __builtin_cpu_supports("avx2") && __builtin_cpu_supports("fma");
+        const unsigned hw = std::thread::hardware_concurrency();
+        const int n_thr = (int)std::min<unsigned>(std::max(1u, hw), 8u);
+        const int per = ((N + 1 + n_thr - 1) / n_thr + 15) & ~15;
+        auto work = [&](int t) {
+            const int i0 = t * per, i1 = std::min(N + 1, i0 + per);
+            if (i0 >= i1) return;
+            (avx2 ? intensity_nodes_avx2 : intensity_nodes_generic)(fa_re.data(), fa_im.data(), fb_re.data(), fb_im.data(),
+                                                                    (int)a.size(), h, i0, i1, gv.data());
+        };
+        std::vector<std::thread> pool;
+        for (int t = 1; t < n_thr; ++t) pool.emplace_back(work, t);
+        work(0);
+        for (auto &th : pool) th.join();
     }
     std::vector<double> C(n_panel + 1);                 // cumulative integral at even nodes
     C[0] = 0.0;
