@@ -167,6 +167,7 @@ enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED =
 
 template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
 __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
+    constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned long long s_stats[ST_COUNT];
     __shared__ __align__(16) uint4 s_keys[5];
@@ -224,10 +225,12 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
         // acc_lost = sum over finished histories of (1 - final weight) + roulette gains: all weight that went into
         // particles or the surface; absorbed_particles = acc_lost - acc_abss.
         unsigned long long acc_esc = 0ull, acc_lost = 0ull, acc_abss = 0ull;
-        uint32_t cnt_hist = 0u, cnt_ev = 0u, cnt_refl = 0u, max_ev = 0u;
+        // cnt_fl = flights that ended in an interaction (particle events + reflections), cnt_refl = reflections
+        uint32_t cnt_hist = 0u, cnt_fl = 0u, cnt_refl = 0u, max_ev = 0u;
 
         // ---- lane state: one photon history (step (1)) ---------------------------------------------
-        // nfl = flights flown so far = Philox draw index of the next flight (D1).
+        // nfl = flights flown so far = Philox draw index of the next flight (D1); n_refl = reflections of this
+        // history, carried only by the variants that read it (NREFL).
         // run: the lane flies a photon; want: it needs a photon id (neither: the unit is drained, the lane is done).
         bool run = false, want = true;
         float T = 0.f, mu = -1.f, vt = 0.f, w = 1.f, abss = 0.f;
@@ -255,7 +258,8 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
                 id_lo = pool_lo + off;
                 id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
             }
-            T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u; n_refl = 0u;
+            T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u;
+            if (NREFL) n_refl = 0u;
         };
         // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
         auto finish = [&](int fate) {
@@ -283,14 +287,14 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             const uint32_t lost = kWOne - wq;
             acc_lost += lost;
             acc_abss += min(__float2uint_rn(abss * kWOneF), lost);
-            const uint32_t n_sc = nfl - n_refl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);
-            cnt_ev += nfl - n_refl; cnt_refl += n_refl;       // an absorbing interaction is a particle event too
-            max_ev = max(max_ev, n_sc + n_refl);
+            const uint32_t n_int = nfl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);     // scatters + reflections
+            cnt_fl += nfl;                                    // an absorbing interaction is a particle event too
+            max_ev = max(max_ev, n_int);
             if (TRACE) {
                 const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
                 pdv_trace_record r;
                 r.vt = vt; r.weight = w; r.mu_exit = mu; r.fate = fate == F_ABS_PART ? F_ABS_SURF : fate;
-                r.n_scatter = (int)n_sc; r.n_reflect = (int)n_refl;
+                r.n_scatter = (int)(n_int - n_refl); r.n_reflect = (int)n_refl;
                 P.trace[idx] = r;
             }
             take_photon();
@@ -349,7 +353,8 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             vt = fmaf(mu_new - mu, vh, vt);                   // Eq. 4 (vh = v/2)
             mu = mu_new;
             ++nfl;
-            n_refl += surf ? 1u : 0u;
+            cnt_refl += surf ? 1u : 0u;
+            if (NREFL) n_refl += surf ? 1u : 0u;
             if (ROUL && nfl - n_refl >= P.max_events && w <= P.roulette_p) {       // Russian roulette (rare path)
                 const uint32_t yr = ANALOG ? y_roul
                                            : philox_roulette_word(id_lo, id_hi, ud.stream, POLY ? nfl - 1u : (nfl - 1u) >> 1, s_keys, sub);
@@ -421,6 +426,7 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
         unsigned long long acc_absp = acc_lost - acc_abss;
+        uint32_t cnt_ev = cnt_fl - cnt_refl;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             acc_esc += __shfl_xor_sync(FULL_MASK, acc_esc, o);
