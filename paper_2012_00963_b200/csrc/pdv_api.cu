@@ -286,6 +286,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         return fail(PDV_E_UNSUPPORTED, "cloud tables + histogram exceed the shared memory of one block");
     // 1024 resident threads per SM (64 registers each): two blocks of 512 when their shared memory fits twice, else one of 1024
     int block = o->threads_per_block, per_sm = 0;
+    if (const char *e = std::getenv("PDV_X_BLOCK")) block = atoi(e);      // kernel experiments
     if (block == 0) block = 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024 ? 512 : 1024;
     {
         struct Key { KernelVariant v; int block, smem, device; };
