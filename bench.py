@@ -169,6 +169,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1 = headline)")
     ap.add_argument("--photons", type=int, default=0, help="override histories per unit (debugging; invalidates the number)")
+    ap.add_argument("--depth-model", type=int, default=0, choices=[0, 1],
+                    help="0: depth table (the headline design); 1: closed-form v(T), exponential profiles only (variant f2)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--ref-photons", type=int, default=2_000_000, help="--impl reference: histories per step")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work of the cpu_baseline leg (0: skip)")
@@ -195,6 +197,8 @@ def main():
     dev = torch.device("cuda", local)
 
     cfg = W.config(args.config)
+    if args.depth_model:
+        cfg["clouds"] = [dict(c, depth_model=args.depth_model) for c in cfg["clouds"]]
     run = dict(cfg["run"])
     n = int(args.photons or run["n_photons"])
     run["first_photon_id"] = rank * n                       # weak scaling: disjoint id ranges, same count per rank
@@ -296,7 +300,9 @@ def main():
         sm_max = clocks["sm_max_mhz"] or 1965.0
         n_sm = peaks["n_sm"]
         issue_peak = n_sm * 4 * 32 * sm_max * 1e6                               # 1 warp-instruction / clk / sub-partition
-        a = ALG_INST_PER_FLIGHT
+        a = dict(ALG_INST_PER_FLIGHT)
+        if args.depth_model == 1:                      # closed-form v(T): log + 2 FMA (4 with the clamp) instead of the 8 of the table probe
+            a["scatter"] -= 4
         alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
         achieved = alg / (tr_ms * 1e-3)
         traffic = None
@@ -310,7 +316,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units,
+            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units, "depth_model": args.depth_model,
                        "n_bins": nb, "parallelism": f"photon-id ranges x{world}", "l2": "flushed between steps (256 MiB write)",
                        "events_per_history": events / histories, "reflections_per_history": reflections / histories},
             "histories_per_s": histories / (step_ms * 1e-3),

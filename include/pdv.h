@@ -64,6 +64,11 @@ typedef struct {
     int32_t n_depth_bins;        /* depth bins uniform in v (= in z at fixed t); [1, 4096]; 0 -> 1024 */
     int32_t phase_model;         /* 0: Mie, Eq. 12-14; 1: isotropic ("uniform") scattering, Fig. 6 case 2,
                                     with the Mie efficiencies kept for extinction and albedo */
+    int32_t depth_model;         /* how the kernel gets the particle velocity at an optical depth T (counted from the top):
+                                    0: the depth table (n_depth_bins bins uniform in v, T linear in v inside a bin);
+                                    1: the closed form of the truncated Eq. 20,
+                                       v = v_fs - (v_fs/beta) ln(E + (1 - E) T/tau_ext), E = exp(-beta (vmax_ratio - 1))
+                                       (R26) -- profile_kind 0 only; no table error, one logarithm per event */
 } pdv_cloud_params;
 
 #define PDV_MAX_CLASSES 32

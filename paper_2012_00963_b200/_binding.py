@@ -35,7 +35,8 @@ class CloudParams(C.Structure):
                 ("n_classes", C.c_int32), ("diameter", C.POINTER(C.c_double)), ("number_weight", C.POINTER(C.c_double)),
                 ("m_re", C.c_double), ("m_im", C.c_double), ("wavelength", C.c_double),
                 ("surface_reflectivity", C.c_double), ("surface_model", C.c_int32),
-                ("n_phase_bins", C.c_int32), ("n_depth_bins", C.c_int32), ("phase_model", C.c_int32)]
+                ("n_phase_bins", C.c_int32), ("n_depth_bins", C.c_int32), ("phase_model", C.c_int32),
+                ("depth_model", C.c_int32)]
 
 
 class CloudInfo(C.Structure):
@@ -192,6 +193,7 @@ def pdv_cloud_create(params: dict) -> Cloud:
     p.surface_reflectivity, p.surface_model = params["surface_reflectivity"], int(params.get("surface_model", 0))
     p.n_phase_bins, p.n_depth_bins = int(params.get("n_phase_bins", 0)), int(params.get("n_depth_bins", 0))
     p.phase_model = int(params.get("phase_model", 0))
+    p.depth_model = int(params.get("depth_model", 0))
     h = C.c_void_p(None)
     _check(lib().pdv_cloud_create(C.byref(p), C.byref(h)))
     return Cloud(h.value)

@@ -120,6 +120,13 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     hd.blob_bytes = (uint32_t)off;
     hd.n_classes = nc; hd.K = K; hd.n_depth = nd; hd.n_guide = n_guide; hd.guide_base = base;
     hd.guide_shift = shift; hd.depth_bisect = bisect;
+    if (h.depth_model == 1) {              // v/2 = v_fs/2 - (v_fs ln2 / (2 beta)) lg2(E + (1 - E) T / tau_ext)   (R26)
+        const double E = std::exp(-h.beta * (h.v_max / h.v_fs - 1.0));
+        hd.an_c0 = (float)(0.5 * h.v_fs);
+        hd.an_c1 = (float)(-0.5 * h.v_fs * 0.6931471805599453 / h.beta);
+        hd.an_c2 = Tf[nd] > 0.f ? (float)E : 1.f;             // empty cloud: every event is at the surface, v = v_fs
+        hd.an_c3 = Tf[nd] > 0.f ? (float)((1.0 - E) / (double)Tf[nd]) : 0.f;
+    }
     hd.log2K = 0;
     while ((1 << hd.log2K) < K) ++hd.log2K;
     hd.tau_ext = Tf[nd]; hd.vh_fs = (float)(0.5 * h.v_fs);
@@ -278,6 +285,10 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     kv.sso = o->single_scatter_only != 0;
     kv.trace = trace;
     kv.roulette = o->max_events > 0;
+    kv.closed_depth = clouds[0]->host.depth_model == 1;
+    for (int i = 1; i < n_clouds; ++i)
+        if ((clouds[i]->host.depth_model == 1) != kv.closed_depth)
+            return fail(PDV_E_UNSUPPORTED, "all clouds of one launch must use the same depth_model");
 
     const DeviceInfo &di = device_info(device);
     if (!di.valid) return fail(PDV_E_CUDA, "cannot query the CUDA device");
@@ -294,7 +305,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         static std::vector<std::pair<Key, int>> cache;       // occupancy queries are not free either
         std::lock_guard<std::mutex> lk(mu);
         for (const auto &e : cache)
-            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette &&
+            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.closed_depth == kv.closed_depth &&
                 e.first.block == block && e.first.smem == smem && e.first.device == device) { per_sm = e.second; break; }
         if (per_sm == 0) {
             CU(transport_max_blocks_per_sm(kv, block, smem, &per_sm), "occupancy query");

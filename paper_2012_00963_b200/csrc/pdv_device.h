@@ -56,14 +56,15 @@ struct DevCloudHeader {
     uint32_t off_phase, off_rows, off_thr, off_albedo, off_albthr, off_guide;   // byte offsets from the blob start
     uint32_t guide_base;       // (float bits of T) >> guide_shift of guide cell 0
     uint32_t guide_shift;
-    uint32_t depth_bisect;
+    uint32_t depth_bisect;     // 0: one guide probe; 1: bisect the rows
     float tau_ext, vh_fs;      // vh_fs = v_fs / 2
     float R_f;                 // surface reflectivity
     uint32_t R_thr;            // analog mode: reflected iff xi_absorb word < R_thr
     uint32_t surface_model;
     uint32_t frac_mask;        // the 12 bits of a phase word below its log2K index bits
     uint32_t off_cguide;       // class guide: 256 bytes, see below
-    uint32_t pad[6];
+    float an_c0, an_c1, an_c2, an_c3;   // closed-form depth model (pdv_cloud_params.depth_model 1)
+    uint32_t pad[2];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 
@@ -97,7 +98,7 @@ struct RunParams {
 struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
-struct KernelVariant { bool poly, analog, sso, trace, roulette; };   // template instantiation of transport_kernel
+struct KernelVariant { bool poly, analog, sso, trace, roulette, closed_depth; };   // template instantiation of transport_kernel
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,

@@ -165,7 +165,7 @@ __device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t i
 // History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
 enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
 __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     extern __shared__ __align__(16) unsigned char smem[];
@@ -219,6 +219,13 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
         const float albedo0 = cv.albedo[0];               // monodisperse: the only class
+        // CF: closed form of the exponential profile (pdv_cloud_params.depth_model 1) instead of the depth rows:
+        // v/2 = an0 + an1 lg2(an2 + an3 T), exactly v_fs / 2 at T = tau_ext
+        float an0 = 0.f, an1 = 0.f, an2 = 1.f, an3 = 0.f;
+        if (CF) {
+            const DevCloudHeader *h = reinterpret_cast<const DevCloudHeader *>(s_blob);
+            an0 = h->an_c0; an1 = h->an_c1; an2 = h->an_c2; an3 = h->an_c3;
+        }
         const uint32_t albthr0 = cv.albthr[0];
 
         // ---- per-thread accumulators (flushed once per unit) ------------------------------------------------
@@ -312,7 +319,7 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             if (SSO && !surf && nfl != n_refl) return F_TRUNC;    // single-scatter-only: cut at the 2nd particle event
             // ---------------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ------
             T = fminf(Tn, cv.tau_ext);
-            const float vh = depth_half_velocity(cv, T);      // = v_fs / 2 at the surface
+            const float vh = CF ? fmaf(an1, fast_lg2(fmaf(an3, T, an2)), an0) : depth_half_velocity(cv, T);   // = v_fs / 2 at the surface
             uint32_t c = 0u;
             float alb = albedo0;
             uint32_t albt = albthr0;
@@ -475,11 +482,11 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
 
 // ------------------------------------------------------------------------------------------------------------
 // The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
 static cudaError_t ensure_smem(int smem) {
     static int smem_set = 48 * 1024;
     if (smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL>,
+        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, CF>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         smem_set = smem;
@@ -487,22 +494,23 @@ static cudaError_t ensure_smem(int smem) {
     return cudaSuccess;
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
 static cudaError_t launch_t(const RunParams &rp, LaunchShape s, cudaStream_t st) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL>(s.smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, CF>(s.smem);
     if (e != cudaSuccess) return e;
-    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL><<<s.grid, s.block, s.smem, st>>>(rp);
+    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, CF><<<s.grid, s.block, s.smem, st>>>(rp);
     return cudaGetLastError();
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
 static cudaError_t occ_t(int block, int smem, int *out) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL>(smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, CF>(smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL>, block, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, CF>, block, smem);
 }
 
-#define PDV_D0(FN, A, B, C, D, ...) (v.roulette ? FN<A, B, C, D, true>(__VA_ARGS__) : FN<A, B, C, D, false>(__VA_ARGS__))
+#define PDV_DC(FN, A, B, C, D, E, ...) (v.closed_depth ? FN<A, B, C, D, E, true>(__VA_ARGS__) : FN<A, B, C, D, E, false>(__VA_ARGS__))
+#define PDV_D0(FN, A, B, C, D, ...) (v.roulette ? PDV_DC(FN, A, B, C, D, true, __VA_ARGS__) : PDV_DC(FN, A, B, C, D, false, __VA_ARGS__))
 #define PDV_D1(FN, A, B, C, ...) (v.trace ? PDV_D0(FN, A, B, C, true, __VA_ARGS__) : PDV_D0(FN, A, B, C, false, __VA_ARGS__))
 #define PDV_D2(FN, A, B, ...) (v.sso ? PDV_D1(FN, A, B, true, __VA_ARGS__) : PDV_D1(FN, A, B, false, __VA_ARGS__))
 #define PDV_D3(FN, A, ...) (v.analog ? PDV_D2(FN, A, true, __VA_ARGS__) : PDV_D2(FN, A, false, __VA_ARGS__))

@@ -221,6 +221,8 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     if (!(p.surface_reflectivity >= 0.0 && p.surface_reflectivity <= 1.0)) return bad("surface_reflectivity not in [0,1]");
     if (p.surface_model != 0 && p.surface_model != 1) return bad("surface_model must be 0 or 1");
     if (p.phase_model != 0 && p.phase_model != 1) return bad("phase_model must be 0 or 1");
+    if (p.depth_model != 0 && p.depth_model != 1) return bad("depth_model must be 0 or 1");
+    if (p.depth_model == 1 && p.profile_kind != 0) return bad("depth_model 1 (closed form) needs the exponential profile (profile_kind 0)");
     const int K = p.n_phase_bins == 0 ? 1024 : p.n_phase_bins;
     const int nd = p.n_depth_bins == 0 ? 1024 : p.n_depth_bins;
     if (!is_pow2(K) || K < 16 || K > 4096) return bad("n_phase_bins must be a power of two in [16, 4096]");
@@ -243,6 +245,7 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     HostCloud h;
     h.n_classes = p.n_classes; h.K = K; h.n_depth = nd;
     h.v_fs = p.v_fs; h.v_max = p.vmax_ratio * p.v_fs; h.R = p.surface_reflectivity; h.surface_model = p.surface_model;
+    h.depth_model = p.depth_model; h.beta = p.profile_kind == 0 ? p.beta : 0.0;
     h.diameter.assign(p.diameter, p.diameter + p.n_classes);
     h.weight.resize(p.n_classes);
     for (int c = 0; c < p.n_classes; ++c) h.weight[c] = p.number_weight[c] / wsum;

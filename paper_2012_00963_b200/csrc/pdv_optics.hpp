@@ -18,6 +18,8 @@ struct HostCloud {
     std::vector<double> T_edge;                      // [n_depth+1], T at v_max - j dv
     double tau_ext = 0, kappa = 0, sauter = 0, v_fs = 0, v_max = 0, R = 0;
     int surface_model = 0;
+    int depth_model = 0;                             // 1: closed-form v(T) of the exponential profile (then beta > 0)
+    double beta = 0;
 };
 
 // Mie coefficients a_n, b_n (n = 1..n_max) of a homogeneous sphere, size parameter x, relative index m.

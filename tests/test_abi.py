@@ -89,7 +89,8 @@ def test_isotropic_phase_model_and_tabulated_profile():
 @pytest.mark.parametrize("patch", [dict(area_mass=-1.0), dict(density=0.0), dict(v_fs=0.0), dict(beta=0.0),
                                    dict(vmax_ratio=1.0), dict(surface_reflectivity=1.5), dict(n_phase_bins=1000),
                                    dict(n_depth_bins=5000), dict(wavelength=0.0), dict(m_im=-1.0),
-                                   dict(diameters=[0.0], number_weights=[1.0]), dict(surface_model=3),
+                                   dict(diameters=[0.0], number_weights=[1.0]), dict(surface_model=3), dict(depth_model=2),
+                                   dict(depth_model=1, profile_kind=1, prof_v=[2000.0, 6000.0], prof_cum_mass=[0.0, 1.0]),
                                    dict(diameters=[1e-6] * 33, number_weights=[1.0] * 33)])
 def test_cloud_create_rejects_invalid(patch):
     with pytest.raises(P.PdvError) as e:

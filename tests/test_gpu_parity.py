@@ -238,6 +238,38 @@ def test_tabulated_profile_matches_oracle(P):
     _assert_stats_parity(r.stats[0, 0], n, o)
 
 
+@pytest.mark.parametrize("idx", [1, 2])
+def test_closed_form_depth_model_matches_oracle_and_the_table(P, idx):
+    """depth_model 1 (v(T) from the closed form of the truncated Eq. 20, R26) against
+    the oracle's analytic-profile variant, and history by history against the depth table on the same Philox stream:
+    the 1024-bin table is linear in v inside a bin, so the two velocities differ by < 0.01 m/s per event."""
+    cfg = W.config(idx)
+    params = dict(cfg["clouds"][0], depth_model=1)
+    run = cfg["run"]
+    c1 = P.pdv_cloud_create(params)
+    c0 = P.pdv_cloud_create(cfg["clouds"][0])
+    n = 1_000_000
+    r = P.pdv_mc_run([c1], cfg["t_snap"][:1], n, 53, run)
+    assert r.conservation_residual()[0, 0] == 0.0
+    o = _oracle(cfg["clouds"][0], run, n, analytic_profile=True)
+    _assert_hist_parity(r.hist[0, 0], r.hist2[0, 0], n, o, min_ndf=30)
+    _assert_stats_parity(r.stats[0, 0], n, o)
+    m = 200_000
+    _, ta = P.pdv_mc_trace(c1, 0, m, 77, run)
+    _, tb = P.pdv_mc_trace(c0, 0, m, 77, run)
+    same = (ta["fate"] == tb["fate"]) & (ta["n_scatter"] == tb["n_scatter"]) & (ta["n_reflect"] == tb["n_reflect"])
+    assert same.mean() == 1.0                       # the velocity does not steer a history: identical decisions
+    dv = np.abs(ta["vt"].astype(np.float64) - tb["vt"].astype(np.float64))
+    assert np.median(dv) < 0.02 and np.quantile(dv, 0.999) < 0.5
+    # empty cloud: every event is at the surface, v = v_fs exactly
+    ce = P.pdv_cloud_create(dict(params, area_mass=0.0))
+    re_ = P.pdv_mc_run([ce], cfg["t_snap"][:1], 100_000, 7, run)
+    rt = P.pdv_mc_run([P.pdv_cloud_create(dict(cfg["clouds"][0], area_mass=0.0))], cfg["t_snap"][:1], 100_000, 7, run)
+    assert np.array_equal(re_.hist, rt.hist)
+    with pytest.raises(P.PdvError):                 # the closed form exists for the exponential profile only
+        P.pdv_cloud_create(dict(params, profile_kind=1, prof_v=np.array([2000.0, 6000.0]), prof_cum_mass=np.array([0.0, 1.0])))
+
+
 def test_empty_and_tiny_runs_and_empty_cloud(P):
     cfg = W.config(1)
     c = P.pdv_cloud_create(cfg["clouds"][0])
