@@ -1,5 +1,6 @@
 // pdv_api.cu -- the C-ABI of include/pdv.h: argument checking, cloud upload, workspace, launches, read-back.
 // No arithmetic of the method lives here beyond packing the fp32/fixed-point device tables.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -376,8 +377,19 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
             UnitDesc &u = units[(size_t)i * n_snap + j];
             u.cloud_blob = clouds[i]->d_blob;
             u.stream = unit_streams ? unit_streams[(size_t)i * n_snap + j] : (uint32_t)(i * n_snap + j);
-            u.pad = 0;
+            u.visit = 0;
         }
+    {   // visiting order: descending cost.  The cost of a unit grows with the optical thickness of its cloud (events per
+        // history ~ tau^2 for thick clouds); n_photons is the same for all units.  Stable, so equal clouds keep their order.
+        std::vector<uint32_t> ord(n_units);
+        for (int k = 0; k < n_units; ++k) ord[k] = (uint32_t)k;
+        auto tau = [&](uint32_t k) { return clouds[k / n_snap]->host.tau_ext; };
+        std::stable_sort(ord.begin(), ord.end(), [&](uint32_t x, uint32_t y) { return tau(x) > tau(y); });
+        uint32_t n_lead = 0;
+        while (n_lead < (uint32_t)n_units && tau(ord[n_lead]) >= 0.99 * tau(ord[0])) ++n_lead;
+        for (int k = 0; k < n_units; ++k) units[k].visit = ord[k];
+        plan.rp.n_lead = n_lead ? n_lead : 1u;
+    }
     pdv_trace_record *d_trace = nullptr;
     if (trace && n_photons) CU(cudaMalloc(&d_trace, sizeof(pdv_trace_record) * n_photons), "cudaMalloc(trace)");
     auto cleanup = [&]() { if (d_trace) cudaFree(d_trace); };

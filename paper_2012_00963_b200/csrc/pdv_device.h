@@ -71,7 +71,7 @@ static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignm
 struct UnitDesc {
     const unsigned char *cloud_blob;   // device pointer
     uint32_t stream;                   // Philox counter word 2 (unit index)
-    uint32_t pad;
+    uint32_t visit;                    // entry k of the table: the unit a block works on k-th (see RunParams::n_lead)
 };
 
 struct RunParams {
@@ -82,6 +82,9 @@ struct RunParams {
     unsigned long long *stats;         // [n_units][ST_COUNT]
     pdv_trace_record *trace;           // TRACE only: [n_photons]
     uint32_t n_units;
+    uint32_t n_lead;                   // blocks visit the units in descending cost (units[k].visit), so that the long tails of
+                                       // the expensive ones overlap with other work; block b starts at entry b % n_lead, n_lead =
+                                       // number of leading units of equal cost (all of them when the units are alike)
     uint32_t n_bins;
     uint32_t chunk;                    // photon ids a lane claims per fetch at the start of a unit (guided: shrinks
     float chunk_per_remaining;         //   to clamp(remaining * chunk_per_remaining, chunk_min, chunk) as the unit drains)

@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
     if (tid < 5) s_keys[tid] = make_uint4(P.key0[2 * tid], P.key1[2 * tid], P.key0[2 * tid + 1], P.key1[2 * tid + 1]);
 
     for (uint32_t visit = 0; visit < P.n_units; ++visit) {
-        const uint32_t u = (blockIdx.x + visit) % P.n_units;
+        const uint32_t u = P.units[(blockIdx.x % P.n_lead + visit) % P.n_units].visit;
         if (tid == 0) s_go = (*(volatile unsigned long long *)(P.next_id + u) < P.n_photons) ? 1 : 0;
         __syncthreads();
         const bool go = s_go != 0;
