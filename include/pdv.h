@@ -228,6 +228,30 @@ pdv_status pdv_spectrum_peaks(const double *hist, int32_t n_units, int32_t n_bin
                               double v_lo, double v_hi, const double *v_fs, const pdv_peak_opts *opts,
                               pdv_peak *out, int32_t on_device, void *cuda_stream);
 
+/* Scattering-angle sampling check (the paper's own sampler on the device, to report the error of the table): draws
+ * cos(theta) n_samples times for ONE size class of a Mie cloud (phase_model 0) in two ways and histograms both over
+ * n_bins equal bins of [-1, 1]:
+ *   table  the transport kernel's sampler: cos(theta) = M[k] + (M[k+1] - M[k]) frac from one Philox word (Eq. 13-14
+ *          through the inverse-CDF table D_K);
+ *   exact  acceptance-rejection on the exact Mie function, the paper's step (4): mu uniform on [-1, 1],
+ *          accepted if xi i_max <= I(mu), I = |S1|^2 + |S2|^2 summed from the Mie series (Eq. 13-14) in fp32 on the device,
+ *          i_max = 1.02 x the maximum of I over 20001 angles, found on the host.
+ * Sample i draws from Philox4x32-10 streams keyed by (seed, i): same (cloud, class, n_samples, seed) => same counts.
+ * hist_table, hist_exact: HOST [n_bins] counts.  info: HOST, may be NULL.  1 <= n_bins <= 4096.
+ * Errors: PDV_E_INVALID (NULLs, class_index, n_bins), PDV_E_UNSUPPORTED (isotropic cloud; more than 1024 Mie terms),
+ * PDV_E_CUDA. */
+typedef struct {
+    double sum_cos_table;        /* sum of cos(theta) over the table samples (mean = sum / n_samples -> g) */
+    double sum_cos_exact;        /* same over the rejection samples */
+    double i_max;                /* the bound used */
+    uint64_t n_trials;           /* rejection trials in total: n_samples / n_trials = int I dmu / (2 i_max) */
+    uint64_t n_bound_violations; /* trials that found I(mu) > i_max; must be 0 */
+} pdv_phase_check;
+
+pdv_status pdv_phase_sampling_check(const pdv_cloud *cloud, int32_t class_index, uint64_t n_samples, uint64_t seed,
+                                    int32_t n_bins, uint64_t *hist_table, uint64_t *hist_exact, pdv_phase_check *info,
+                                    void *cuda_stream);
+
 /* Measures the issue-rate denominators on the current device: a dependent-free FFMA stream and a MUFU
  * stream, each run for ~`millis` ms on every SM.  Outputs (any may be NULL): thread-instructions/s of each,
  * the SM clock in MHz observed meanwhile (clock64 over globaltimer), and the SM count. */

@@ -18,7 +18,7 @@ PDV_MAX_CLASSES = 32
 PDV_MAX_BINS = 8192
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
-           "pdv_cloud_get_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_issue_peaks",
+           "pdv_cloud_get_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
            "pdv_last_launch_info", "pdv_last_error", "pdv_version")
 
 
@@ -63,6 +63,11 @@ TRACE_DTYPE = np.dtype([("vt", "f4"), ("weight", "f4"), ("mu_exit", "f4"), ("fat
 PEAK_DTYPE = np.dtype([("x_peak", "f8"), ("i_peak", "f8"), ("curvature", "f8"), ("k_peak", "i4"), ("status", "i4")])
 
 
+class PhaseCheck(C.Structure):
+    _fields_ = [("sum_cos_table", C.c_double), ("sum_cos_exact", C.c_double), ("i_max", C.c_double),
+                ("n_trials", C.c_uint64), ("n_bound_violations", C.c_uint64)]
+
+
 class PeakOpts(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("smooth_half", C.c_int32), ("smooth_passes", C.c_int32),
                 ("fit_half", C.c_int32), ("pad", C.c_int32), ("x_min", C.c_double), ("x_max", C.c_double)]
@@ -93,6 +98,7 @@ def lib() -> C.CDLL:
                                       C.c_float, vp, C.c_int32, vp]
         L.pdv_spectrum_peaks.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_double, C.c_double, vp,
                                          C.POINTER(PeakOpts), vp, C.c_int32, vp]
+        L.pdv_phase_sampling_check.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int32, vp, vp, C.POINTER(PhaseCheck), vp]
         L.pdv_issue_peaks.argtypes = [C.c_double, dp, dp, dp, C.POINTER(C.c_int32), vp]
         L.pdv_last_launch_info.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32),
                                            C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -328,6 +334,19 @@ def pdv_spectrum_peaks(hist, n_photons: int, v_lo: float, v_hi: float, v_fs, *, 
     _check(lib().pdv_spectrum_peaks(hist.data_ptr(), hist.shape[0], hist.shape[1], int(n_photons), v_lo, v_hi,
                                     v_fs.data_ptr(), C.byref(o), out.data_ptr(), 1, C.c_void_p(stream)))
     return out
+
+
+def pdv_phase_sampling_check(cloud: Cloud, class_index: int, n_samples: int, seed: int, n_bins: int = 64,
+                             stream: int | None = None) -> dict:
+    """cos(theta) of one size class sampled n_samples times from the table and by rejection on the exact Mie function.
+    -> dict(hist_table, hist_exact: uint64 [n_bins]; mean_cos_table, mean_cos_exact, i_max, n_trials, n_bound_violations)."""
+    ht, he = np.zeros(int(n_bins), dtype=np.uint64), np.zeros(int(n_bins), dtype=np.uint64)
+    info = PhaseCheck()
+    _check(lib().pdv_phase_sampling_check(cloud.handle, int(class_index), int(n_samples), int(seed), int(n_bins),
+                                          ht.ctypes.data, he.ctypes.data, C.byref(info), C.c_void_p(stream)))
+    n = max(int(n_samples), 1)
+    return dict(hist_table=ht, hist_exact=he, mean_cos_table=info.sum_cos_table / n, mean_cos_exact=info.sum_cos_exact / n,
+                i_max=info.i_max, n_trials=int(info.n_trials), n_bound_violations=int(info.n_bound_violations))
 
 
 def pdv_issue_peaks(millis: float = 50.0, stream: int | None = None) -> dict:

@@ -643,6 +643,82 @@ pdv_status pdv_spectrum_peaks(const double *hist, int32_t n_units, int32_t n_bin
     return PDV_OK;
 }
 
+pdv_status pdv_phase_sampling_check(const pdv_cloud *cloud, int32_t class_index, uint64_t n_samples, uint64_t seed, int32_t n_bins,
+                                    uint64_t *hist_table, uint64_t *hist_exact, pdv_phase_check *info, void *cuda_stream) {
+    g_err.clear();
+    if (!cloud || !hist_table || !hist_exact) return fail(PDV_E_INVALID, "cloud / hist_table / hist_exact is NULL");
+    const HostCloud &h = cloud->host;
+    if (class_index < 0 || class_index >= h.n_classes) return fail(PDV_E_INVALID, "class_index out of range");
+    if (n_bins < 1 || n_bins > 4096) return fail(PDV_E_INVALID, "n_bins must be in [1, 4096]");
+    if (h.phase_model != 0) return fail(PDV_E_UNSUPPORTED, "the cloud samples an isotropic phase function: there is no Mie function to reject on");
+    // Mie series of the class (Eq. 12-14), coefficients premultiplied by (2n+1)/(n(n+1))
+    const double x = 3.14159265358979323846 * h.diameter[class_index] / h.wavelength;
+    std::vector<double> a_re, a_im, b_re, b_im;
+    mie_coefficients(x, h.m_re, h.m_im, a_re, a_im, b_re, b_im);
+    const int n_terms = (int)a_re.size();
+    if (n_terms > 1024) return fail(PDV_E_UNSUPPORTED, "more than 1024 Mie terms");
+    std::vector<float> coef(4 * (size_t)n_terms);
+    std::vector<double> fa_re(n_terms), fa_im(n_terms), fb_re(n_terms), fb_im(n_terms);
+    for (int n = 1; n <= n_terms; ++n) {
+        const double f = (2.0 * n + 1.0) / (n * (n + 1.0));
+        fa_re[n - 1] = f * a_re[n - 1]; fa_im[n - 1] = f * a_im[n - 1]; fb_re[n - 1] = f * b_re[n - 1]; fb_im[n - 1] = f * b_im[n - 1];
+        coef[4 * (n - 1) + 0] = (float)fa_re[n - 1]; coef[4 * (n - 1) + 1] = (float)fa_im[n - 1];
+        coef[4 * (n - 1) + 2] = (float)fb_re[n - 1]; coef[4 * (n - 1) + 3] = (float)fb_im[n - 1];
+    }
+    double i_max = 0.0;                                       // bound of the rejection: maximum over 20001 angles, plus 2 %
+    const int n_grid = 20000;
+    for (int i = 0; i <= n_grid; ++i) {
+        const double mu = std::cos(3.14159265358979323846 * i / n_grid);
+        double pp = 0.0, pc = 1.0, s1r = 0, s1i = 0, s2r = 0, s2i = 0;
+        for (int n = 1; n <= n_terms; ++n) {
+            const double tau = n * mu * pc - (n + 1.0) * pp;
+            s1r += fa_re[n - 1] * pc + fb_re[n - 1] * tau; s1i += fa_im[n - 1] * pc + fb_im[n - 1] * tau;
+            s2r += fa_re[n - 1] * tau + fb_re[n - 1] * pc; s2i += fa_im[n - 1] * tau + fb_im[n - 1] * pc;
+            const double pn = ((2.0 * n + 1.0) * mu * pc - (n + 1.0) * pp) / n;
+            pp = pc; pc = pn;
+        }
+        i_max = std::max(i_max, s1r * s1r + s1i * s1i + s2r * s2r + s2i * s2i);
+    }
+    i_max *= 1.02;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    int device = 0;
+    CU(cudaGetDevice(&device), "cudaGetDevice");
+    pdv_status s = ensure_on_device(cloud, device);
+    if (s != PDV_OK) return s;
+    const DeviceInfo &di = device_info(device);
+    if (!di.valid) return fail(PDV_E_CUDA, "cannot query the CUDA device");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t o_hist = align16(16 * (size_t)n_terms), o_sum = align16(o_hist + 16 * (size_t)n_bins), o_cnt = o_sum + 16;
+    unsigned char *ws = nullptr;
+    if ((s = get_workspace(o_cnt + 16, device, &ws)) != PDV_OK) return s;
+    DevCloudHeader hd;
+    std::memcpy(&hd, cloud->blob.data(), sizeof(hd));
+    const float2 *phase = reinterpret_cast<const float2 *>(cloud->d_blob + hd.off_phase) + (size_t)class_index * hd.K;
+    CU(cudaMemcpyAsync(ws, coef.data(), 16 * (size_t)n_terms, cudaMemcpyHostToDevice, st), "copy Mie coefficients");
+    CU(cudaMemsetAsync(ws + o_hist, 0, o_cnt + 16 - o_hist, st), "cudaMemsetAsync(sampling check)");
+    CU(launch_phase_check(phase, hd.K, hd.log2K, hd.frac_mask, reinterpret_cast<const float4 *>(ws), n_terms, (float)i_max,
+                          n_samples, seed, n_bins, reinterpret_cast<unsigned long long *>(ws + o_hist),
+                          reinterpret_cast<double *>(ws + o_sum), reinterpret_cast<unsigned long long *>(ws + o_cnt), di.n_sm, st),
+       "sampling-check kernel launch");
+    std::vector<unsigned long long> hh(2 * (size_t)n_bins);
+    double sums[2];
+    unsigned long long cnts[2];
+    CU(cudaMemcpyAsync(hh.data(), ws + o_hist, 16 * (size_t)n_bins, cudaMemcpyDeviceToHost, st), "read back counts");
+    CU(cudaMemcpyAsync(sums, ws + o_sum, 16, cudaMemcpyDeviceToHost, st), "read back sums");
+    CU(cudaMemcpyAsync(cnts, ws + o_cnt, 16, cudaMemcpyDeviceToHost, st), "read back counters");
+    CU(cudaStreamSynchronize(st), "sampling-check kernel execution");
+    for (int i = 0; i < n_bins; ++i) { hist_table[i] = hh[i]; hist_exact[i] = hh[(size_t)n_bins + i]; }
+    if (info) {
+        info->sum_cos_table = sums[0]; info->sum_cos_exact = sums[1]; info->i_max = (double)(float)i_max;
+        info->n_trials = cnts[0]; info->n_bound_violations = cnts[1];
+    }
+    return PDV_OK;
+}
+
 pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mhz, int32_t *n_sm, void *cuda_stream) {
     g_err.clear();
     int ndev = 0;

@@ -111,6 +111,13 @@ cudaError_t launch_spectrogram(const double *hist, int n_snap, int n_bins, doubl
                                float floor_db, float *out, cudaStream_t st);
 cudaError_t launch_peaks(const double *hist, int n_units, int n_bins, double n_photons, double v_lo, double v_hi,
                          const double *v_fs, const pdv_peak_opts &o, pdv_peak *out, cudaStream_t st);
+// Sampling check of one class (pdv_phase_sampling_check): phase = that class's float2 table in the device blob; coef = device
+// float4 [n_terms] (fa_re, fa_im, fb_re, fb_im), f = (2n+1)/(n(n+1)); out_hist = u64 [2][n_bins] (table, exact);
+// out_sum = double [2]; out_cnt = u64 [2] (trials, bound violations).  All outputs zeroed by the caller.
+cudaError_t launch_phase_check(const float2 *phase, uint32_t K, uint32_t log2K, uint32_t frac_mask, const float4 *coef,
+                               int n_terms, float i_max, unsigned long long n_samples, unsigned long long seed, int n_bins,
+                               unsigned long long *out_hist, double *out_sum, unsigned long long *out_cnt, int n_sm,
+                               cudaStream_t st);
 cudaError_t launch_issue_peaks(double millis, double *ffma, double *mufu, double *mhz, int n_sm, cudaStream_t st);
 
 }  // namespace pdv

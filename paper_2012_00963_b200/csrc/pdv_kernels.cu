@@ -677,6 +677,97 @@ cudaError_t launch_peaks(const double *hist, int n_units, int n_bins, double n_p
     return cudaGetLastError();
 }
 
+// ---- scattering-angle sampling check: inverse-CDF table against acceptance-rejection on the exact Mie function -------
+// (the paper's step (4)).  Sample i: one Philox block (stream word 'tabl') feeds the table sampler exactly
+// as in a flight (word 2); the rejection sampler draws two trials (mu, xi) per block of stream 'reje', block index t.
+__global__ void __launch_bounds__(256) phase_check_kernel(const float2 *__restrict__ phase, uint32_t K, uint32_t log2K,
+                                                          uint32_t frac_mask, const float4 *__restrict__ coef, int n_terms,
+                                                          float i_max, unsigned long long n_samples, unsigned long long seed,
+                                                          int n_bins, unsigned long long *out_hist, double *out_sum,
+                                                          unsigned long long *out_cnt) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    float4 *s_coef = reinterpret_cast<float4 *>(smem);
+    uint32_t *s_ht = reinterpret_cast<uint32_t *>(s_coef + n_terms), *s_he = s_ht + n_bins;
+    __shared__ __align__(16) uint4 s_keys[5];
+    __shared__ double s_sum[2];
+    __shared__ unsigned long long s_cnt[2];
+    const uint32_t tid = threadIdx.x;
+    if (tid < 5) {
+        const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32), r = 2u * tid;
+        s_keys[tid] = make_uint4(k0 + r * 0x9E3779B9u, k1 + r * 0xBB67AE85u, k0 + (r + 1u) * 0x9E3779B9u, k1 + (r + 1u) * 0xBB67AE85u);
+    }
+    if (tid < 2) { s_sum[tid] = 0.0; s_cnt[tid] = 0ull; }
+    for (int i = tid; i < n_terms; i += blockDim.x) s_coef[i] = coef[i];
+    for (int i = tid; i < 2 * n_bins; i += blockDim.x) s_ht[i] = 0u;
+    __syncthreads();
+    // |S1|^2 + |S2|^2 at mu: pi_n, tau_n by upward recurrence (Eq. 13-14)
+    auto intensity = [&](float mu) {
+        float pp = 0.f, pc = 1.f, s1r = 0.f, s1i = 0.f, s2r = 0.f, s2i = 0.f;
+        for (int n = 1; n <= n_terms; ++n) {
+            const float4 c = s_coef[n - 1];
+            const float fn = (float)n, tau = fn * mu * pc - (fn + 1.f) * pp;
+            s1r += c.x * pc + c.z * tau; s1i += c.y * pc + c.w * tau;
+            s2r += c.x * tau + c.z * pc; s2i += c.y * tau + c.w * pc;
+            const float pn = ((2.f * fn + 1.f) * mu * pc - (fn + 1.f) * pp) / fn;
+            pp = pc; pc = pn;
+        }
+        return s1r * s1r + s1i * s1i + s2r * s2r + s2i * s2i;
+    };
+    const float bin_scale = 0.5f * (float)n_bins;
+    auto bin_of = [&](float ct) { return min((uint32_t)max(__float2int_rd((ct + 1.f) * bin_scale), 0), (uint32_t)n_bins - 1u); };
+    const uint32_t shiftK = 32u - log2K;
+    double sum_t = 0.0, sum_e = 0.0;
+    unsigned long long trials = 0ull, viol = 0ull;
+    for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + tid; i < n_samples;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t lo = (uint32_t)i, hi = (uint32_t)(i >> 32);
+        uint32_t x0, x1, x2, x3;
+        philox4x32_10(lo, hi, 0x7461626Cu, 0u, s_keys, x0, x1, x2, x3);
+        const float2 m = phase[x2 >> shiftK];
+        const float ct = fmaf(m.y, __uint2float_rn(x2 & frac_mask), m.x);
+        atomicAdd(&s_ht[bin_of(ct)], 1u);
+        sum_t += (double)ct;
+        for (uint32_t t = 0u;; ++t) {
+            philox4x32_10(lo, hi, 0x72656A65u, t, s_keys, x0, x1, x2, x3);
+            float mu = fmaf((float)(x0 >> 8) + 0.5f, 1.1920928955078125e-7f, -1.f);         // 24 bits over [-1, 1)
+            float I = intensity(mu);
+            ++trials; viol += I > i_max ? 1ull : 0ull;
+            if (((float)(x1 >> 8) + 0.5f) * 5.9604644775390625e-8f * i_max <= I) { atomicAdd(&s_he[bin_of(mu)], 1u); sum_e += (double)mu; break; }
+            mu = fmaf((float)(x2 >> 8) + 0.5f, 1.1920928955078125e-7f, -1.f);
+            I = intensity(mu);
+            ++trials; viol += I > i_max ? 1ull : 0ull;
+            if (((float)(x3 >> 8) + 0.5f) * 5.9604644775390625e-8f * i_max <= I) { atomicAdd(&s_he[bin_of(mu)], 1u); sum_e += (double)mu; break; }
+        }
+    }
+    atomicAdd(&s_sum[0], sum_t); atomicAdd(&s_sum[1], sum_e);
+    atomicAdd(&s_cnt[0], trials); atomicAdd(&s_cnt[1], viol);
+    __syncthreads();
+    for (int i = tid; i < 2 * n_bins; i += blockDim.x)
+        if (s_ht[i]) atomicAdd(out_hist + i, (unsigned long long)s_ht[i]);
+    if (tid < 2) { atomicAdd(out_sum + tid, s_sum[tid]); atomicAdd(out_cnt + tid, s_cnt[tid]); }
+}
+
+cudaError_t launch_phase_check(const float2 *phase, uint32_t K, uint32_t log2K, uint32_t frac_mask, const float4 *coef,
+                               int n_terms, float i_max, unsigned long long n_samples, unsigned long long seed, int n_bins,
+                               unsigned long long *out_hist, double *out_sum, unsigned long long *out_cnt, int n_sm,
+                               cudaStream_t st) {
+    if (n_samples == 0) return cudaSuccess;
+    const int smem = 16 * n_terms + 8 * n_bins;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(phase_check_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+    }
+    // a block's private counts are 32-bit: at most 2^32 - 1 samples per block
+    unsigned long long grid = (unsigned long long)n_sm * 4ull;
+    const unsigned long long need = (n_samples + 0xFFFFFFFEull) / 0xFFFFFFFFull;
+    if (grid < need) grid = need;
+    const unsigned long long useful = (n_samples + 255ull) / 256ull;
+    if (grid > useful) grid = useful;
+    phase_check_kernel<<<(unsigned)grid, 256, smem, st>>>(phase, K, log2K, frac_mask, coef, n_terms, i_max, n_samples, seed,
+                                                          n_bins, out_hist, out_sum, out_cnt);
+    return cudaGetLastError();
+}
+
 // ---- issue-rate microbenchmarks: the FP32/SFU denominators of the roofline ---------------------
 // Each thread runs 8 independent chains so the pipe, not the dependency latency, limits the rate.
 __global__ void __launch_bounds__(512) ffma_peak_kernel(unsigned long long iters, float seed, float *sink,

@@ -245,6 +245,7 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     HostCloud h;
     h.n_classes = p.n_classes; h.K = K; h.n_depth = nd;
     h.v_fs = p.v_fs; h.v_max = p.vmax_ratio * p.v_fs; h.R = p.surface_reflectivity; h.surface_model = p.surface_model;
+    h.m_re = p.m_re; h.m_im = p.m_im; h.wavelength = p.wavelength; h.phase_model = p.phase_model;
     h.depth_model = p.depth_model; h.beta = p.profile_kind == 0 ? p.beta : 0.0;
     h.diameter.assign(p.diameter, p.diameter + p.n_classes);
     h.weight.resize(p.n_classes);

@@ -20,6 +20,8 @@ struct HostCloud {
     int surface_model = 0;
     int depth_model = 0;                             // 1: closed-form v(T) of the exponential profile (then beta > 0)
     double beta = 0;
+    double m_re = 0, m_im = 0, wavelength = 0;       // kept for pdv_phase_sampling_check
+    int phase_model = 0;
 };
 
 // Mie coefficients a_n, b_n (n = 1..n_max) of a homogeneous sphere, size parameter x, relative index m.

@@ -119,6 +119,14 @@ def test_run_argument_validation_and_no_cpu_fallback():
         with pytest.raises(P.PdvError) as e:
             P.pdv_spectrum_peaks(np.ones((2, 64)), 10, 0.0, 6000.0, 2000.0)
         assert e.value.status == 3 and "no CPU fallback" in str(e.value)
+    for args in ((1, 10, 1, 8), (0, 10, 1, 0), (0, 10, 1, 5000)):                                   # class / n_bins out of range
+        with pytest.raises(P.PdvError) as e:
+            P.pdv_phase_sampling_check(c, *args)
+        assert e.value.status == 1
+    if not torch.cuda.is_available():
+        with pytest.raises(P.PdvError) as e:
+            P.pdv_phase_sampling_check(c, 0, 10, 1, 8)
+        assert e.value.status == 3
     for bad in (dict(half=-1), dict(n_pass=17), dict(fit_half=0), dict(x_min=2.0, x_max=1.0)):      # rejected before any CUDA call
         with pytest.raises(P.PdvError) as e:
             P.pdv_spectrum_peaks(np.ones((2, 64)), 10, 0.0, 6000.0, 2000.0, **bad)
