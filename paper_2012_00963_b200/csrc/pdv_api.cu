@@ -123,6 +123,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     hd.guide_shift = shift; hd.depth_bisect = bisect;
     if (h.depth_model == 1) {              // v/2 = v_fs/2 - (v_fs ln2 / (2 beta)) lg2(E + (1 - E) T / tau_ext)   (R26)
         const double E = std::exp(-h.beta * (h.v_max / h.v_fs - 1.0));
+        hd.depth_bisect = 2;
         hd.an_c0 = (float)(0.5 * h.v_fs);
         hd.an_c1 = (float)(-0.5 * h.v_fs * 0.6931471805599453 / h.beta);
         hd.an_c2 = Tf[nd] > 0.f ? (float)E : 1.f;             // empty cloud: every event is at the surface, v = v_fs
@@ -286,10 +287,20 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     kv.sso = o->single_scatter_only != 0;
     kv.trace = trace;
     kv.roulette = o->max_events > 0;
-    kv.closed_depth = clouds[0]->host.depth_model == 1;
-    for (int i = 1; i < n_clouds; ++i)
-        if ((clouds[i]->host.depth_model == 1) != kv.closed_depth)
-            return fail(PDV_E_UNSUPPORTED, "all clouds of one launch must use the same depth_model");
+    // dm 0: every cloud uses the one-probe depth table and the paper's surface law; 1: every cloud uses the closed-form
+    // depth model and the paper's surface law; 2 (general kernel): anything else, decided per unit at run time
+    {
+        int n_closed = 0;
+        bool odd = kv.sso || kv.trace;
+        for (int i = 0; i < n_clouds; ++i) {
+            DevCloudHeader hd;
+            std::memcpy(&hd, clouds[i]->blob.data(), sizeof(hd));
+            n_closed += hd.depth_bisect == 2u ? 1 : 0;
+            odd = odd || hd.depth_bisect == 1u || hd.surface_model != 0u;
+        }
+        kv.dm = odd || (n_closed != 0 && n_closed != n_clouds) ? 2 : (n_closed ? 1 : 0);
+        if (const char *e = std::getenv("PDV_X_DM")) if (atoi(e) == 2) kv.dm = 2;      // experiments: force the general kernel
+    }
 
     const DeviceInfo &di = device_info(device);
     if (!di.valid) return fail(PDV_E_CUDA, "cannot query the CUDA device");
@@ -306,7 +317,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         static std::vector<std::pair<Key, int>> cache;       // occupancy queries are not free either
         std::lock_guard<std::mutex> lk(mu);
         for (const auto &e : cache)
-            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.closed_depth == kv.closed_depth &&
+            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.dm == kv.dm &&
                 e.first.block == block && e.first.smem == smem && e.first.device == device) { per_sm = e.second; break; }
         if (per_sm == 0) {
             CU(transport_max_blocks_per_sm(kv, block, smem, &per_sm), "occupancy query");

@@ -56,7 +56,7 @@ struct DevCloudHeader {
     uint32_t off_phase, off_rows, off_thr, off_albedo, off_albthr, off_guide;   // byte offsets from the blob start
     uint32_t guide_base;       // (float bits of T) >> guide_shift of guide cell 0
     uint32_t guide_shift;
-    uint32_t depth_bisect;     // 0: one guide probe; 1: bisect the rows
+    uint32_t depth_bisect;     // 0: one guide probe; 1: bisect the rows; 2: closed form  v/2 = an_c0 + an_c1 lg2(an_c2 + an_c3 T)
     float tau_ext, vh_fs;      // vh_fs = v_fs / 2
     float R_f;                 // surface reflectivity
     uint32_t R_thr;            // analog mode: reflected iff xi_absorb word < R_thr
@@ -101,7 +101,7 @@ struct RunParams {
 struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
-struct KernelVariant { bool poly, analog, sso, trace, roulette, closed_depth; };   // template instantiation of transport_kernel
+struct KernelVariant { bool poly, analog, sso, trace, roulette; int dm; };   // dm: see transport_kernel   // template instantiation of transport_kernel
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,

@@ -102,9 +102,10 @@ struct CloudView {               // per-unit scalars and shared-memory table poi
 };
 
 // half the particle velocity at vertical optical depth Tc, 0 <= Tc <= tau_ext (depth rows: see pdv_device.h).
+template <bool GENERAL>
 __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float Tc) {
     uint32_t j;
-    if (cv.depth_bisect) {                                   // pathological table (unit-uniform branch)
+    if (GENERAL && cv.depth_bisect) {                        // pathological table (unit-uniform branch)
         uint32_t lo = 0u, hi = cv.n_depth;                   // T_lo <= Tc < T_hi
         while (hi - lo > 1u) {
             const uint32_t mid = (lo + hi) >> 1;
@@ -165,7 +166,7 @@ __device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t i
 // History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
 enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
 __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     extern __shared__ __align__(16) unsigned char smem[];
@@ -219,15 +220,20 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
         const float albedo0 = cv.albedo[0];               // monodisperse: the only class
-        // CF: closed form of the exponential profile (pdv_cloud_params.depth_model 1) instead of the depth rows:
-        // v/2 = an0 + an1 lg2(an2 + an3 T), exactly v_fs / 2 at T = tau_ext
-        float an0 = 0.f, an1 = 0.f, an2 = 1.f, an3 = 0.f;
-        if (CF) {
-            const DevCloudHeader *h = reinterpret_cast<const DevCloudHeader *>(s_blob);
-            an0 = h->an_c0; an1 = h->an_c1; an2 = h->an_c2; an3 = h->an_c3;
-        }
         const uint32_t albthr0 = cv.albthr[0];
 
+        // DM (KernelVariant::dm): how the particle velocity at a depth is found, and which rare models are compiled in.
+        //   0  one guide probe of the depth rows, the paper's surface law: nothing else in the instruction stream
+        //   1  closed form of the exponential profile (pdv_cloud_params.depth_model 1): v/2 = an0 + an1 lg2(an2 + an3 T),
+        //      exactly v_fs / 2 at T = tau_ext
+        //   2  general: per unit, any of guide probe / bisection of a pathological table / closed form, either surface law
+        float an0 = 0.f, an1 = 0.f, an2 = 1.f, an3 = 0.f;
+        bool closed = DM == 1;
+        if (DM != 0) {
+            const DevCloudHeader *h = reinterpret_cast<const DevCloudHeader *>(s_blob);
+            an0 = h->an_c0; an1 = h->an_c1; an2 = h->an_c2; an3 = h->an_c3;
+            if (DM == 2) closed = h->depth_bisect == 2u;
+        }
         // ---- per-thread accumulators (flushed once per unit) ------------------------------------------------
         // acc_lost = sum over finished histories of (1 - final weight) + roulette gains: all weight that went into
         // particles or the surface; absorbed_particles = acc_lost - acc_abss.
@@ -319,7 +325,9 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             if (SSO && !surf && nfl != n_refl) return F_TRUNC;    // single-scatter-only: cut at the 2nd particle event
             // ---------------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ------
             T = fminf(Tn, cv.tau_ext);
-            const float vh = CF ? fmaf(an1, fast_lg2(fmaf(an3, T, an2)), an0) : depth_half_velocity(cv, T);   // = v_fs / 2 at the surface
+            float vh;                                         // = v_fs / 2 at the surface
+            if (DM == 1 || (DM == 2 && closed)) vh = fmaf(an1, fast_lg2(fmaf(an3, T, an2)), an0);
+            else vh = depth_half_velocity<DM == 2>(cv, T);
             uint32_t c = 0u;
             float alb = albedo0;
             uint32_t albt = albthr0;
@@ -355,7 +363,7 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             // takes |(1 - ct^2)(1 - mu^2)|
             const float mu_s = fmaf(mu, ct, -cosv * sq);
             float mu_r = cosv;
-            if (cv.surface_model) mu_r = lambert_mu(pwf);     // unit-uniform branch
+            if (DM == 2 && cv.surface_model) mu_r = lambert_mu(pwf);     // unit-uniform branch
             const float mu_new = surf ? mu_r : mu_s;
             vt = fmaf(mu_new - mu, vh, vt);                   // Eq. 4 (vh = v/2)
             mu = mu_new;
@@ -482,11 +490,11 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
 
 // ------------------------------------------------------------------------------------------------------------
 // The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
 static cudaError_t ensure_smem(int smem) {
     static int smem_set = 48 * 1024;
     if (smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, CF>,
+        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         smem_set = smem;
@@ -494,34 +502,50 @@ static cudaError_t ensure_smem(int smem) {
     return cudaSuccess;
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
 static cudaError_t launch_t(const RunParams &rp, LaunchShape s, cudaStream_t st) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, CF>(s.smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM>(s.smem);
     if (e != cudaSuccess) return e;
-    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, CF><<<s.grid, s.block, s.smem, st>>>(rp);
+    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM><<<s.grid, s.block, s.smem, st>>>(rp);
     return cudaGetLastError();
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, bool CF>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
 static cudaError_t occ_t(int block, int smem, int *out) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, CF>(smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM>(smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, CF>, block, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM>, block, smem);
 }
 
-#define PDV_DC(FN, A, B, C, D, E, ...) (v.closed_depth ? FN<A, B, C, D, E, true>(__VA_ARGS__) : FN<A, B, C, D, E, false>(__VA_ARGS__))
-#define PDV_D0(FN, A, B, C, D, ...) (v.roulette ? PDV_DC(FN, A, B, C, D, true, __VA_ARGS__) : PDV_DC(FN, A, B, C, D, false, __VA_ARGS__))
+// DM = 0 / 1 exist for the production variants only; single-scatter-only and trace runs always take the general kernel.
+template <bool A, bool B, bool C, bool D, bool E>
+static cudaError_t launch_dm(int dm, const RunParams &rp, LaunchShape s, cudaStream_t st) {
+    if constexpr (C || D) {
+        return launch_t<A, B, C, D, E, 2>(rp, s, st);
+    } else {
+        return dm == 0 ? launch_t<A, B, C, D, E, 0>(rp, s, st) : dm == 1 ? launch_t<A, B, C, D, E, 1>(rp, s, st) : launch_t<A, B, C, D, E, 2>(rp, s, st);
+    }
+}
+template <bool A, bool B, bool C, bool D, bool E>
+static cudaError_t occ_dm(int dm, int block, int smem, int *out) {
+    if constexpr (C || D) {
+        return occ_t<A, B, C, D, E, 2>(block, smem, out);
+    } else {
+        return dm == 0 ? occ_t<A, B, C, D, E, 0>(block, smem, out) : dm == 1 ? occ_t<A, B, C, D, E, 1>(block, smem, out) : occ_t<A, B, C, D, E, 2>(block, smem, out);
+    }
+}
+#define PDV_D0(FN, A, B, C, D, ...) (v.roulette ? FN<A, B, C, D, true>(v.dm, __VA_ARGS__) : FN<A, B, C, D, false>(v.dm, __VA_ARGS__))
 #define PDV_D1(FN, A, B, C, ...) (v.trace ? PDV_D0(FN, A, B, C, true, __VA_ARGS__) : PDV_D0(FN, A, B, C, false, __VA_ARGS__))
 #define PDV_D2(FN, A, B, ...) (v.sso ? PDV_D1(FN, A, B, true, __VA_ARGS__) : PDV_D1(FN, A, B, false, __VA_ARGS__))
 #define PDV_D3(FN, A, ...) (v.analog ? PDV_D2(FN, A, true, __VA_ARGS__) : PDV_D2(FN, A, false, __VA_ARGS__))
 #define PDV_DISPATCH(FN, ...) (v.poly ? PDV_D3(FN, true, __VA_ARGS__) : PDV_D3(FN, false, __VA_ARGS__))
 
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st) {
-    return PDV_DISPATCH(launch_t, rp, shape, st);
+    return PDV_DISPATCH(launch_dm, rp, shape, st);
 }
 
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out) {
-    return PDV_DISPATCH(occ_t, block, smem, out);
+    return PDV_DISPATCH(occ_dm, block, smem, out);
 }
 
 // ---- finalize: Q31 integers -> doubles (H12 input; stats) ------------------------------------------------------
