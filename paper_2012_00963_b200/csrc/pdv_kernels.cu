@@ -292,7 +292,7 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
                 } else {
                     acc_esc += wq;
                 }
-            } else if (fate == F_KILLED) {
+            } else if (ROUL && fate == F_KILLED) {
                 smem_add64(&s_stats[ST_KILLED], wq);
             } else if (SSO && fate == F_TRUNC) {
                 smem_add64(&s_stats[ST_TRUNC], wq);
@@ -380,8 +380,9 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             return F_NONE;
         };
 
+        bool refill = true;                                   // warp-uniform: some lane waits for a photon id
         for (;;) {
-            if (__any_sync(FULL_MASK, want)) {
+            if (refill) {
                 // ---- some lane found the warp pool empty: refill it from the unit's cursor (guided self-scheduling: a warp
                 // claims clamp(remaining / (2 warps), 32 chunk_min, 32 chunk) ids, sized from a fresh look at the cursor) and
                 // hand ids to the waiting lanes; lanes still waiting when the unit is drained are done
@@ -437,6 +438,7 @@ __global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kerne
             }
             __syncwarp();                                     // histories that ended in either flight are finished in ONE pass
             if (fate != F_NONE) finish(fate);                 // the one place where a lane moves on to its next photon
+            refill = __any_sync(FULL_MASK, want);             // only a finished history can leave a lane waiting for an id
         }
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
