@@ -330,6 +330,7 @@ def main():
                     "includes": "pdv_cloud_create (host Mie + tables + H2D), pdv_mc_run (host outputs), pdv_spectrogram"},
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12, "unit": "Tthread-inst/s",
                          "frac": achieved / issue_peak, "traffic": traffic,
+                         "frac_executed": (traffic / (tr_ms / args.steps * 1e-3) / issue_peak) if traffic else None,
                          "peak_is": f"{n_sm} SMs x 4 sub-partitions x 32 lanes x {sm_max:.0f} MHz (DESIGN.md), not in MEASURED_PEAKS.json",
                          "kernel": "pdv::transport_kernel",
                          "alg_inst_per_flight": a,
