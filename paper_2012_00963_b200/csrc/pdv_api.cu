@@ -310,6 +310,8 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     // 1024 resident threads per SM (64 registers each): two blocks of 512 when their shared memory fits twice, else one of 1024
     int block = o->threads_per_block, per_sm = 0;
     if (const char *e = std::getenv("PDV_X_BLOCK")) block = atoi(e);      // kernel experiments
+    // polydisperse clouds: one block of PDV_LB_THREADS_POLY threads per SM (80 registers each), see pdv_device.h
+    if (kv.poly) block = block == 0 ? PDV_LB_THREADS_POLY : std::min(block, PDV_LB_THREADS_POLY);
     if (block == 0) block = 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024 ? 512 : 1024;
     {
         struct Key { KernelVariant v; int block, smem, device; };

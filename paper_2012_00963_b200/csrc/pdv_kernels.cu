@@ -167,7 +167,7 @@ __device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t i
 enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
 template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
-__global__ void __launch_bounds__(PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
+__global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned long long s_stats[ST_COUNT];
