@@ -303,6 +303,8 @@ def main():
         a = dict(ALG_INST_PER_FLIGHT)
         if args.depth_model == 1:                      # closed-form v(T): log + 2 FMA (4 with the clamp) instead of the 8 of the table probe
             a["scatter"] -= 4
+        if any(len(c.get("diameters", [])) > 1 or "lognormal" in c for c in cfg["clouds"]):
+            a["scatter"] += 6                        # polydisperse: class pick (guide byte, threshold, compare, clamp) + per-class albedo and table base
         alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
         achieved = alg / (tr_ms * 1e-3)
         traffic = None
