@@ -144,25 +144,43 @@ static void draw_flight(rng_t *r, const oracle_params *p, uint32_t flight, fligh
         d->xi_class = rng_u53(r); d->xi_cos = rng_u53(r); d->xi_phi = rng_u53(r);
         d->xi_roulette = rng_u53(r); d->xi_absorb = rng_u53(r);
     } else {                                       /* DESIGN.md D1/D2: the shared counter-based stream */
-        /* D1: block index `draw` = flight (several size classes: one block per flight) or flight/2 (one class: one
-         * block feeds two flights, words (x0,x1) then (x2,x3)); counter word 3 = 2 draw, and 2 draw + 1 for the
-         * second block (absorption / roulette words). */
+        /* D1/D2.  Counter word 3 of a block = 2 * (block index), + 1 for its companion block (absorption /
+         * roulette words).  A flight reads a path word a, a phase word b and, with several size classes, a class word cw.
+         * One class: block index = flight / 2; the block feeds two flights, (a, b) = (x0, x1) then (x2, x3); companion
+         *   words: absorption y[half], roulette y[2 + half].
+         * Several classes: flights come in groups of three, group g = flight / 3 reads blocks 2g and 2g + 1 as eight words
+         *   W0..W7: (a, b, cw) = (W0, W1, W2'), (W3, W4, W5'), (W6, W7, cw2), where W' = the word with its low byte
+         *   replaced by 0x80 and cw2 = (W2.byte0, W5.byte0, W6 bits 23..8) from the top; companions: absorption =
+         *   word r of the companion of block 2g, roulette = word r of the companion of block 2g + 1 (r = flight % 3).
+         * Azimuth word, both cases: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top. */
         int mono = p->n_classes == 1;
-        uint32_t draw = mono ? flight >> 1 : flight, half = mono ? (flight & 1u) : 0u;
-        uint32_t c[4] = { r->id_lo, r->id_hi, r->stream, 2u * draw }, x[4], y[4];
-        oracle_philox4x32_10(c, r->key, x);
-        c[3] = 2u * draw + 1u;
-        oracle_philox4x32_10(c, r->key, y);
-        uint32_t a, b, pw;
+        uint32_t a, b, pw, w_abs, w_roul;
         if (mono) {
+            uint32_t draw = flight >> 1, half = flight & 1u;
+            uint32_t c[4] = { r->id_lo, r->id_hi, r->stream, 2u * draw }, x[4], y[4];
+            oracle_philox4x32_10(c, r->key, x);
+            c[3] = 2u * draw + 1u;
+            oracle_philox4x32_10(c, r->key, y);
             a = x[2 * half]; b = x[2 * half + 1];
-            /* azimuth word of a two-word flight: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top */
-            pw = ((a & 0xFFu) << 24) | ((b & 0xFFu) << 16) | (((a >> 8) & 0xFFu) << 8) | ((a >> 16) & 0xFFu);
+            w_abs = y[half]; w_roul = y[2 + half];
             d->xi_class = 0.0;
         } else {
-            a = x[0]; b = x[2]; pw = x[3];
-            d->xi_class = ((double)x[1] + 0.5) * (1.0 / 4294967296.0);
+            uint32_t g = flight / 3u, rr = flight % 3u, W[8], ya[4], yr[4], cw;
+            uint32_t c[4] = { r->id_lo, r->id_hi, r->stream, 2u * (2u * g) };
+            oracle_philox4x32_10(c, r->key, W);
+            c[3] = 2u * (2u * g) + 1u;
+            oracle_philox4x32_10(c, r->key, ya);
+            c[3] = 2u * (2u * g + 1u);
+            oracle_philox4x32_10(c, r->key, W + 4);
+            c[3] = 2u * (2u * g + 1u) + 1u;
+            oracle_philox4x32_10(c, r->key, yr);
+            if (rr == 0u)      { a = W[0]; b = W[1]; cw = (W[2] & 0xFFFFFF00u) | 0x80u; }
+            else if (rr == 1u) { a = W[3]; b = W[4]; cw = (W[5] & 0xFFFFFF00u) | 0x80u; }
+            else               { a = W[6]; b = W[7]; cw = ((W[2] & 0xFFu) << 24) | ((W[5] & 0xFFu) << 16) | ((W[6] >> 8) & 0xFFFFu); }
+            w_abs = ya[rr]; w_roul = yr[rr];
+            d->xi_class = ((double)cw + 0.5) * (1.0 / 4294967296.0);
         }
+        pw = ((a & 0xFFu) << 24) | ((b & 0xFFu) << 16) | (((a >> 8) & 0xFFu) << 8) | ((a >> 16) & 0xFFu);
         /* D2: path = top 23 bits of a; phase = top (log2 K + 12) bits of b; azimuth = pw */
         int log2K = 0;
         while ((1 << log2K) < p->K) ++log2K;
@@ -170,8 +188,8 @@ static void draw_flight(rng_t *r, const oracle_params *p, uint32_t flight, fligh
         d->xi_path = 1.0 - (double)(a >> 9) * (1.0 / 8388608.0);         /* (0,1], 23 bits */
         d->xi_cos = (double)(b >> (32u - keep)) / (double)(1ull << keep);
         d->xi_phi = (double)pw * (1.0 / 4294967296.0);
-        d->xi_absorb = (double)y[half] * (1.0 / 4294967296.0);
-        d->xi_roulette = (double)y[2 + half] * (1.0 / 4294967296.0);
+        d->xi_absorb = (double)w_abs * (1.0 / 4294967296.0);
+        d->xi_roulette = (double)w_roul * (1.0 / 4294967296.0);
     }
 }
 

@@ -29,8 +29,8 @@ __shared__ unsigned int s_dbg[8];
 #ifndef PDV_BLOCKS_MONO
 #define PDV_BLOCKS_MONO 1
 #endif
-#ifndef PDV_BLOCKS_POLY
-#define PDV_BLOCKS_POLY 4
+#ifndef PDV_GROUPS_POLY
+#define PDV_GROUPS_POLY 1
 #endif
 // Register budget of transport_kernel: PDV_LB_THREADS x PDV_LB_BLOCKS resident threads per SM (pdv_device.h).
 namespace pdv {
@@ -154,12 +154,13 @@ __device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, u
     return o;
 }
 
-// second Philox block of a draw (absorption / roulette words), out of line for the roulette path of the implicit-capture kernels
-__device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t draw, const uint4 *keys,
-                                                      uint32_t sub) {
+// roulette word of a flight for the implicit-capture kernels, which do not draw the companion blocks: word `word` of the
+// block with counter word 3 = ctr3 (D1/D2), out of line
+__device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t ctr3, const uint4 *keys,
+                                                      uint32_t word) {
     uint32_t y0, y1, y2, y3;
-    philox4x32_10(id_lo, id_hi, stream, 2u * draw + 1u, keys, y0, y1, y2, y3);
-    return sub ? y3 : y2;
+    philox4x32_10(id_lo, id_hi, stream, ctr3, keys, y0, y1, y2, y3);
+    return word == 0u ? y0 : word == 1u ? y1 : word == 2u ? y2 : y3;
 }
 
 
@@ -371,8 +372,11 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cnt_refl += surf ? 1u : 0u;
             if (NREFL) n_refl += surf ? 1u : 0u;
             if (ROUL && nfl - n_refl >= P.max_events && w <= P.roulette_p) {       // Russian roulette (rare path)
+                // the flight that just ended is nfl - 1: monodisperse, word 2 + sub of the companion of block (nfl - 1) / 2;
+                // polydisperse, word sub of the companion of the group's second block
                 const uint32_t yr = ANALOG ? y_roul
-                                           : philox_roulette_word(id_lo, id_hi, ud.stream, POLY ? nfl - 1u : (nfl - 1u) >> 1, s_keys, sub);
+                                    : POLY ? philox_roulette_word(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, s_keys, sub)
+                                           : philox_roulette_word(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, s_keys, 2u + sub);
                 const RouletteOut o = roulette(w, abss, yr, P.roulette_thr, P.roulette_inv_p, s_stats);
                 if (o.killed) return F_KILLED;
                 w = o.w; abss = o.abss; acc_lost += o.add_lost; acc_abss += o.add_abss;
@@ -416,21 +420,37 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             }
             int fate = F_NONE;
             if (run) {
-                // -------- random numbers (step (3)): one Philox4x32-10 block feeds one flight of a polydisperse cloud
-                // (path, class, phase, azimuth words) or two flights of a monodisperse one (path + phase word each).
-                // PDV_BLOCKS_* blocks per pass: the end-of-history code below runs at the few lanes whose history ended, so it
-                // is entered once per several flights; a lane whose history ended waits for the others meanwhile ------
+                // -------- random numbers (step (3); D1/D2).  A flight reads a path word a, a phase word b, an azimuth
+                // word made of their low bytes (a.byte0, b.byte0, a.byte1, a.byte2 from the top: neither the 23 path bits nor
+                // the 22 phase bits reach the two leading ones) and, with several size classes, a class word.
+                // One class: one Philox4x32-10 block feeds two flights.  Several classes: two blocks feed three flights.
+                // A pass flies PDV_BLOCKS_MONO blocks / PDV_GROUPS_POLY groups: the end-of-history code below runs at the few
+                // lanes whose history ended, so it is entered once per several flights; those lanes wait meanwhile ------
+                if (POLY) {
 #pragma unroll 1
-                for (int blk = 0; blk < (POLY ? PDV_BLOCKS_POLY : PDV_BLOCKS_MONO) && fate == F_NONE; ++blk) {
-                    const uint32_t draw = POLY ? nfl : nfl >> 1;
-                    uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
-                    philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
-                    if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, s_keys, y0, y1, y2, y3);
-                    if (POLY) {
-                        fate = flight(x0, x1, x2, x3, y0, y2, 0u);
-                    } else {
-                        // azimuth word of a two-word flight: bytes (a.byte0, b.byte0, a.byte1, a.byte2) from the top -- neither
-                        // the path (top 23 bits of a) nor the phase lookup (top 22 bits of b) reads the two leading ones
+                    for (int grp = 0; grp < PDV_GROUPS_POLY && fate == F_NONE; ++grp) {
+                        const uint32_t b2 = 2u * (nfl / 3u);      // nfl is a multiple of 3 here: blocks b2 and b2 + 1
+                        uint32_t w0, w1, w2, w3, w4, w5, w6, w7, ya0 = 0u, ya1 = 0u, ya2 = 0u, ya3 = 0u, yr0 = 0u, yr1 = 0u, yr2 = 0u, yr3 = 0u;
+                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2, s_keys, w0, w1, w2, w3);
+                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 2u, s_keys, w4, w5, w6, w7);
+                        if (ANALOG) {                                 // companion blocks: absorption words, roulette words
+                            philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 1u, s_keys, ya0, ya1, ya2, ya3);
+                            if (ROUL) philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 3u, s_keys, yr0, yr1, yr2, yr3);
+                        }
+                        // class words: 24 bits of w2 and of w5, and (w2.byte0, w5.byte0, w6 bits 23..8) for the third flight
+                        fate = flight(w0, (w2 & 0xFFFFFF00u) | 0x80u, w1, __byte_perm(w0, w1, 0x0412), ya0, yr0, 0u);
+                        if (fate == F_NONE) fate = flight(w3, (w5 & 0xFFFFFF00u) | 0x80u, w4, __byte_perm(w3, w4, 0x0412), ya1, yr1, 1u);
+                        if (fate == F_NONE)
+                            fate = flight(w6, (w2 << 24) | ((w5 & 0xFFu) << 16) | ((w6 >> 8) & 0xFFFFu), w7, __byte_perm(w6, w7, 0x0412),
+                                          ya2, yr2, 2u);
+                    }
+                } else {
+#pragma unroll 1
+                    for (int blk = 0; blk < PDV_BLOCKS_MONO && fate == F_NONE; ++blk) {
+                        const uint32_t draw = nfl >> 1;
+                        uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
+                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
+                        if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, s_keys, y0, y1, y2, y3);
                         fate = flight(x0, 0u, x1, __byte_perm(x0, x1, 0x0412), y0, y2, 0u);
                         if (fate == F_NONE) fate = flight(x2, 0u, x3, __byte_perm(x2, x3, 0x0412), y1, y3, 1u);
                     }
