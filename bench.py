@@ -109,6 +109,11 @@ class ClockSampler:
                 "samples": len(self.samples), "power_w_max": max(self.power) if self.power else None}
 
 
+def _workload(index: int) -> dict:
+    """BASELINE.json configs 0..4, or 5: the paper's Figs. 13-15 parameter sweep (row f1)."""
+    return W.paper_sweep("fig13_15", n_photons=10 ** 7) if index == 5 else W.config(index)
+
+
 # ------------------------------------------------------------------------------------------------------ CPU oracle
 def oracle_timed(cfg: dict, seconds: float, seed: int):
     """Times the oracle, as it stands, on all host cores for about `seconds` of work on unit 0 of `cfg`."""
@@ -137,7 +142,7 @@ def run_reference(args):
     from oracle import cloud as ocloud
     from oracle import mc as omc
     omc.build()
-    cfg = W.config(args.config)
+    cfg = _workload(args.config)
     oc = ocloud.build_cloud(cfg["clouds"][0])
     cores = os.cpu_count() or 1
     n = int(min(args.ref_photons, cfg["run"]["n_photons"]))
@@ -167,7 +172,9 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1 = headline)")
+    ap.add_argument("--config", type=int, default=1,
+                    help="BASELINE.json configs index (default 1 = headline); 5 = the paper's Figs. 13-15 sweep (SURVEY.md 8(f) row "
+                         "f1: 14 clouds x 1e7 photons in one launch, then pdv_spectrum_peaks on the device)")
     ap.add_argument("--photons", type=int, default=0, help="override histories per unit (debugging; invalidates the number)")
     ap.add_argument("--depth-model", type=int, default=0, choices=[0, 1],
                     help="0: depth table (the headline design); 1: closed-form v(T), exponential profiles only (variant f2)")
@@ -196,7 +203,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    cfg = W.config(args.config)
+    cfg = _workload(args.config)
     if args.depth_model:
         cfg["clouds"] = [dict(c, depth_model=args.depth_model) for c in cfg["clouds"]]
     run = dict(cfg["run"])
@@ -211,6 +218,9 @@ def main():
     stats = torch.zeros(n_units * P.STATS_DTYPE.itemsize, dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
     stream = torch.cuda.current_stream()
+    v_fs_dev = None
+    if "points" in cfg:                                      # sweep + interpretation workload: one v_fs per spectrum
+        v_fs_dev = torch.tensor([c["v_fs"] for c in cfg["clouds"] for _ in t_snap], dtype=torch.float64, device=dev)
 
     def barrier():
         if world > 1:
@@ -221,8 +231,12 @@ def main():
         P.pdv_mc_run_device(clouds, t_snap, n, run["seed"] + 7919 * i, run, hist, hist2, stats, stream=stream.cuda_stream)
         if world > 1:
             allreduce_tallies(hist, hist2)
-        return P.pdv_spectrogram(hist.view(n_units, nb), n * world, run["v_lo"], run["v_hi"], scale=2,
-                                 stream=stream.cuda_stream)
+        sp = P.pdv_spectrogram(hist.view(n_units, nb), n * world, run["v_lo"], run["v_hi"], scale=2,
+                               stream=stream.cuda_stream)
+        if v_fs_dev is not None:                             # row f1: peak position / value / curvature of every spectrum
+            return P.pdv_spectrum_peaks(hist.view(n_units, nb), n * world, run["v_lo"], run["v_hi"], v_fs_dev, half=6, n_pass=2,
+                                        fit_half=16, x_min=1.03, stream=stream.cuda_stream)
+        return sp
 
     def read_stats():
         return np.frombuffer(stats.cpu().numpy().tobytes(), dtype=P.STATS_DTYPE)
@@ -269,6 +283,9 @@ def main():
         cl = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
         r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run)
         sp = P.pdv_spectrogram(r.hist.reshape(n_units, nb), n, run["v_lo"], run["v_hi"], scale=2)
+        if v_fs_dev is not None:
+            sp = P.pdv_spectrum_peaks(r.hist.reshape(n_units, nb), n, run["v_lo"], run["v_hi"],
+                                      [c["v_fs"] for c in cfg["clouds"] for _ in t_snap], half=6, n_pass=2, fit_half=16, x_min=1.03)
         for c in cl:
             c.destroy()
         return int(r.stats["particle_events"].sum()), sp
@@ -323,7 +340,7 @@ def main():
                        "events_per_history": events / histories, "reflections_per_history": reflections / histories},
             "histories_per_s": histories / (step_ms * 1e-3),
             "events_incl_surface_per_s": (events + reflections) / (step_ms * 1e-3),
-            "gpu_launches": 3 * args.steps,                 # transport + finalize + spectrogram kernels per step
+            "gpu_launches": (4 if v_fs_dev is not None else 3) * args.steps,    # transport + finalize + spectrogram (+ peak) kernels per step
             "launch": {"grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
                        "transport_ms_per_step": tr_ms / args.steps},
             "clocks": clocks,

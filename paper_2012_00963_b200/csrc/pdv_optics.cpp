@@ -14,6 +14,7 @@
 #include <cmath>
 #include <complex>
 #include <thread>
+#include <utility>
 
 namespace pdv {
 
@@ -119,7 +120,7 @@ __attribute__((target("avx2,fma"))) static void intensity_nodes_avx2(const doubl
     PDV_INTENSITY_NODES_BODY
 }
 
-void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M) {
+void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M, int max_threads) {
     std::vector<cplx> a, b;
     mie_ab(x, cplx(m_re, m_im), a, b);
     // psi = pi - theta in [0, pi]; mu = -cos(psi) increases with psi; density in psi: I(mu) sin(psi).
@@ -136,7 +137,7 @@ void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M) {
         }
         const bool avx2 = __builtin_cpu_supports("avx2") && __builtin_cpu_supports("fma");
         const unsigned hw = std::thread::hardware_concurrency();
-        const int n_thr = (int)std::min<unsigned>(std::max(1u, hw), 8u);
+        const int n_thr = std::max(1, std::min((int)std::min<unsigned>(std::max(1u, hw), 8u), max_threads));
         const int per = ((N + 1 + n_thr - 1) / n_thr + 15) & ~15;
         auto work = [&](int t) {
             const int i0 = t * per, i1 = std::min(N + 1, i0 + per);
@@ -253,22 +254,25 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     h.k_ext.resize(p.n_classes); h.k_sca.resize(p.n_classes); h.g.resize(p.n_classes); h.p_class.resize(p.n_classes);
     h.phase.resize((size_t)p.n_classes * (K + 1));
     double s_ext = 0.0, s_d3 = 0.0, s_d2 = 0.0;
+    std::vector<int> todo;                               // classes whose phase table is still to be computed
+    std::vector<std::pair<int, int>> copies;
     for (int c = 0; c < p.n_classes; ++c) {
         const double d = h.diameter[c], x = kPi * d / p.wavelength;
         int same = -1;                                   // identical diameters share a table
         for (int e = 0; e < c; ++e) if (h.diameter[e] == d) { same = e; break; }
         if (same >= 0) {
             h.k_ext[c] = h.k_ext[same]; h.k_sca[c] = h.k_sca[same]; h.g[c] = h.g[same];
-            std::copy(h.phase.begin() + (size_t)same * (K + 1), h.phase.begin() + (size_t)(same + 1) * (K + 1),
-                      h.phase.begin() + (size_t)c * (K + 1));
+            copies.emplace_back(c, same);                // the table itself is copied once it exists, below
         } else {
             mie_efficiencies(x, p.m_re, p.m_im, &h.k_ext[c], &h.k_sca[c], &h.g[c]);
             double *M = &h.phase[(size_t)c * (K + 1)];
             if (p.phase_model == 1) {
                 for (int k = 0; k <= K; ++k) M[k] = -1.0 + 2.0 * (double)k / (double)K;
                 h.g[c] = 0.0;
-            } else {
+            } else if (p.n_classes < 4) {
                 mie_phase_quantiles(x, p.m_re, p.m_im, K, M);
+            } else {
+                todo.push_back(c);                           // many classes: one class per host thread, below
             }
         }
         if (!(h.k_ext[c] > 0.0) || !std::isfinite(h.k_ext[c])) return bad("Mie series failed (K_ext not positive)");
@@ -276,6 +280,22 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
         s_d3 += h.weight[c] * d * d * d;
         s_d2 += h.weight[c] * d * d;
     }
+    if (!todo.empty()) {                                 // the tables of different classes are independent
+        const int n_thr = (int)std::min<size_t>(todo.size(), std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 16u));
+        auto work = [&](int t) {
+            for (size_t i = t; i < todo.size(); i += n_thr) {
+                const int c = todo[i];
+                mie_phase_quantiles(kPi * h.diameter[c] / p.wavelength, p.m_re, p.m_im, K, &h.phase[(size_t)c * (K + 1)], 1);
+            }
+        };
+        std::vector<std::thread> pool;
+        for (int t = 1; t < n_thr; ++t) pool.emplace_back(work, t);
+        work(0);
+        for (auto &th : pool) th.join();
+    }
+    for (const auto &cs : copies)
+        std::copy(h.phase.begin() + (size_t)cs.second * (K + 1), h.phase.begin() + (size_t)(cs.second + 1) * (K + 1),
+                  h.phase.begin() + (size_t)cs.first * (K + 1));
     for (int c = 0; c < p.n_classes; ++c)
         h.p_class[c] = h.weight[c] * h.diameter[c] * h.diameter[c] * h.k_ext[c] / s_ext;       // Eq. 8 sums
     h.kappa = 3.0 * s_ext / (2.0 * p.density * s_d3);                                         // Eq. 10

@@ -32,7 +32,8 @@ void mie_coefficients(double x, double m_re, double m_im, std::vector<double> &a
 void mie_efficiencies(double x, double m_re, double m_im, double *k_ext, double *k_sca, double *g);
 
 // Inverse-CDF table of the unpolarised phase function in mu = cos(theta): M[k] = F^-1(k/K), k = 0..K.
-void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M);
+// The nodes of the angular integral are evaluated on up to min(8, max_threads) host threads.
+void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M, int max_threads = 8);
 
 // Validates params and fills `out`.  Returns PDV_OK or PDV_E_INVALID with a message in `err`.
 pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::string &err);
