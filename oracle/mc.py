@@ -48,7 +48,7 @@ class _Params(C.Structure):
         ("n_bins", C.c_int32), ("v_lo", C.c_double), ("v_hi", C.c_double), ("mu_aperture", C.c_double),
         ("mode", C.c_int32), ("max_events", C.c_int32), ("p_roulette", C.c_double),
         ("single_scatter_only", C.c_int32), ("rng_mode", C.c_int32), ("seed", C.c_uint64),
-        ("stream", C.c_uint32),
+        ("stream", C.c_uint32), ("launch_model", C.c_int32),
     ]
 
 
@@ -117,13 +117,15 @@ class OracleResult:
 
 def run(cloud: OracleCloud, run_opts: dict, *, n_photons: int | None = None, first_id: int = 0, stream: int = 0,
         seed: int | None = None, rng_mode: int = 0, n_threads: int | None = None, analytic_profile: bool = False,
-        exact_mie: dict | None = None, trace: bool = False) -> OracleResult:
+        exact_mie: dict | None = None, trace: bool = False, launch_model: int = 0) -> OracleResult:
     """Run the oracle Monte-Carlo for one (cloud, snapshot) unit.
 
     run_opts: the "run" dictionary of a pdv_workloads config (n_bins, v_lo, v_hi, aperture_sr, mode,
     max_events, roulette_survival, single_scatter_only, n_photons, seed).
     exact_mie: {"m": complex, "wavelength": float} switches theta sampling to acceptance-rejection
     on the exact Mie function; requires rng_mode 0.
+    launch_model 1: diffuse (Lambertian) illumination of the cloud top instead of the paper's collimated beam -- exists
+    only for the invariance pin of the multiple-scattering core (tests/test_oracle_mc.py), rng_mode 0.
     """
     lib = _load()
     n = int(run_opts["n_photons"] if n_photons is None else n_photons)
@@ -166,6 +168,9 @@ def run(cloud: OracleCloud, run_opts: dict, *, n_photons: int | None = None, fir
     p.p_roulette = float(run_opts.get("roulette_survival", 0.1))
     p.single_scatter_only = int(run_opts.get("single_scatter_only", 0))
     p.rng_mode, p.seed, p.stream = int(rng_mode), int(run_opts["seed"] if seed is None else seed), int(stream)
+    if launch_model and rng_mode != 0:
+        raise ValueError("launch_model 1 (diffuse illumination, pins only) needs rng_mode 0")
+    p.launch_model = int(launch_model)
     hist = np.zeros(p.n_bins)
     hist2 = np.zeros(p.n_bins)
     st = _Stats()

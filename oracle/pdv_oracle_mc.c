@@ -29,9 +29,13 @@
  * Mode 1 exists so that single histories can be compared with the GPU; it is pinned by the
  * published known-answer vectors of Philox4x32-10 (tests/golden/philox4x32_10_kat.txt).
  *
- * Parity status: every closed-form consequence is pinned (tests/test_oracle_*.py, pins P1-P12 of
- * SURVEY.md 8(c)); the multiple-scattering spectrum itself has no closed form and no figure data
- * is available: "parity unpinned" for that output beyond those pins.
+ * Parity status: every closed-form consequence is pinned (tests/test_oracle_*.py, pins P1-P13 of
+ * SURVEY.md 8(c)), and the multiple-scattering transport core (free paths, direction updates,
+ * reflections, over many events) by the mean-path invariance of a non-absorbing medium under diffuse
+ * illumination (P16: <events> = 4 tau_ext, <reflections> = 1, Lambertian exit; launch_model 1).  The
+ * Doppler bookkeeping is pinned per event (P2, P3).  Their composition, the SHAPE of the
+ * multiple-scattering spectrum, has no closed form and no figure data is available: "parity
+ * unpinned" for that output beyond those pins.
  */
 #include <math.h>
 #include <pthread.h>
@@ -67,6 +71,9 @@ typedef struct {
     int32_t rng_mode;         /* 0 xoshiro (independent), 1 shared Philox stream */
     uint64_t seed;
     uint32_t stream;
+    int32_t launch_model;     /* 0: the paper's collimated beam, u = (0,0,-1) (reading R1); 1: diffuse (Lambertian) illumination of
+                               * the cloud top, pdf of the polar cosine proportional to it -- used only by the invariance pin
+                               * (mean-chord-length theorem), rng_mode 0 only */
 } oracle_params;
 
 typedef struct {
@@ -285,6 +292,10 @@ static void run_history(const oracle_params *p, uint64_t id, tally_t *ty, oracle
     uint32_t flight = 0;
     flight_draws d;
     ty->st.histories += 1;
+    if (p->launch_model == 1 && rng.mode == 0) {
+        double m0 = sqrt(rng_u53(&rng)), ph = 6.283185307179586 * rng_u53(&rng), sn = sqrt(fmax(0.0, 1.0 - m0 * m0));
+        u[0] = sn * cos(ph); u[1] = sn * sin(ph); u[2] = -m0;
+    }
     for (;;) {
         draw_flight(&rng, p, flight++, &d);
         double s = -log(d.xi_path);

@@ -265,3 +265,35 @@ def test_thread_count_and_id_ranges_do_not_change_results(cfg2_oracle_cloud):
         b2 = mc.run(cfg2_oracle_cloud, _run_opts(n), n_photons=n // 2, first_id=n // 2, n_threads=3, rng_mode=rng_mode)
         assert np.allclose(a.hist, b1.hist + b2.hist, rtol=0, atol=1e-9)
         assert a.stats["particle_events"] == b1.stats["particle_events"] + b2.stats["particle_events"]
+
+
+@pytest.mark.parametrize("m0,d_um", [(1.0, 5.0), (3.0, 2.0)])
+def test_multiple_scattering_core_obeys_the_mean_path_invariance(m0, d_um):
+    """The multiple-scattering transport itself, pinned by a theorem instead of a closed form: in a NON-ABSORBING medium
+    under uniform diffuse (Lambertian) illumination the mean path length of a photon inside is 4 V / S, whatever the
+    phase function and the optical thickness (the mean-chord-length invariance; equilibrium radiance is uniform and
+    isotropic).  For the slab in optical units V/S = tau_ext per unit of open surface, with a Lambertian, lossless
+    bottom, so per history:
+        <optical path> = <particle events> = 4 tau_ext,   <surface reflections> = 1   (bottom area = open area),
+    and what leaves is Lambertian again: P(mu_exit >= mu_a) = 1 - mu_a^2, <mu_exit> = 2/3.
+    Cloud: real refractive index 1.5 (K_abs = 0, albedo 1) with the full Mie phase table, Lambertian surface, R = 1.
+    A wrong sign or factor in T' = T - mu s, in the z row of Eq. 16 or in the reflection law breaks every one of these."""
+    params = dict(W._cloud(m0, 4.0, 2000.0, diameter_um=d_um), m_re=1.5, m_im=0.0, surface_model=1,
+                  surface_reflectivity=1.0)
+    c = cloud.build_cloud(params)
+    assert np.allclose(c.omega0, 1.0, atol=1e-12)
+    n = 400_000
+    run = dict(W.config(1)["run"], aperture_sr=0.1, v_lo=-20000.0, v_hi=20000.0)
+    r = mc.run(c, dict(run, seed=31), n_photons=n, launch_model=1, trace=True)
+    ev = r.trace["n_scatter"].astype(np.float64)
+    assert r.stats["particle_events"] / n == pytest.approx(4.0 * c.tau_ext, abs=5 * ev.std() / math.sqrt(n))
+    rf = r.trace["n_reflect"].astype(np.float64)
+    assert r.stats["surface_reflections"] / n == pytest.approx(1.0, abs=5 * rf.std() / math.sqrt(n))
+    mu_a = mc.aperture_mu(0.1)
+    p_in = 1.0 - mu_a ** 2
+    assert (r.stats["detected"] + r.stats["underflow"] + r.stats["overflow"]) / n == pytest.approx(
+        p_in, abs=5 * math.sqrt(p_in / n))
+    assert float(np.mean(r.trace["mu_exit"])) == pytest.approx(2.0 / 3.0, abs=5 * math.sqrt(1.0 / 18.0 / n))
+    # the same cloud under the paper's collimated beam does NOT have these values: the pin is not vacuous
+    r0 = mc.run(c, dict(run, seed=31), n_photons=100_000)
+    assert abs(r0.stats["particle_events"] / 100_000 - 4.0 * c.tau_ext) > 0.05 * 4.0 * c.tau_ext
