@@ -207,7 +207,9 @@ def test_weight_conservation_is_exact_in_fixed_point(P, kw):
                                     (dict(), dict(surface_model=1)), (dict(), dict(phase_model=1)),
                                     (dict(max_events=6, roulette_survival=0.8), dict()),
                                     (dict(n_bins=8192, v_lo=1000.0, v_hi=5000.0), dict(surface_reflectivity=1.0)),
-                                    (dict(aperture_sr=2 * math.pi), dict(surface_reflectivity=0.0))])
+                                    (dict(aperture_sr=2 * math.pi), dict(surface_reflectivity=0.0)),
+                                    # conservative scattering (real index: albedo 1), lossless Lambertian bottom: the cloud of pin P16
+                                    (dict(v_lo=-6000.0, v_hi=12000.0), dict(m_re=1.5, m_im=0.0, surface_model=1, surface_reflectivity=1.0))])
 def test_variants_match_oracle(P, kw, ckw):
     cfg = W.config(1)
     params = dict(cfg["clouds"][0], **ckw)
