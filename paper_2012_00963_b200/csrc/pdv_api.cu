@@ -256,6 +256,7 @@ pdv_status check_opts(const pdv_run_opts *o) {
         return fail(PDV_E_INVALID, "roulette_survival not in (0,1]");
     if (o->threads_per_block < 0 || o->threads_per_block > 1024 || (o->threads_per_block % 32) != 0)
         return fail(PDV_E_INVALID, "threads_per_block must be a multiple of 32, <= 1024");
+    if (o->launch_model != 0 && o->launch_model != 1) return fail(PDV_E_INVALID, "launch_model must be 0 or 1");
     if (o->blocks_per_sm < 0 || o->blocks_per_sm > 32) return fail(PDV_E_INVALID, "blocks_per_sm out of range");
     return PDV_OK;
 }
@@ -277,6 +278,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     rp.mu_aperture = (float)(1.0 - o->aperture_sr / (2.0 * 3.14159265358979323846));
     rp.n_photons = n_photons;
     rp.first_id = o->first_photon_id;
+    rp.launch_model = (uint32_t)o->launch_model;
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) { rp.key0[r] = k0; rp.key1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
 
@@ -291,7 +293,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     // depth model and the paper's surface law; 2 (general kernel): anything else, decided per unit at run time
     {
         int n_closed = 0;
-        bool odd = kv.sso || kv.trace;
+        bool odd = kv.sso || kv.trace || o->launch_model != 0;
         for (int i = 0; i < n_clouds; ++i) {
             DevCloudHeader hd;
             std::memcpy(&hd, clouds[i]->blob.data(), sizeof(hd));

@@ -99,6 +99,7 @@ struct RunParams {
     float roulette_p;                  // play only while w <= p (then w / p <= 1)
     float roulette_inv_p;
     float v_lo, inv_dv, mu_aperture;
+    uint32_t launch_model;             // 1: diffuse illumination (general kernel only), see pdv_run_opts
     unsigned long long n_photons, first_id;
     uint32_t key0[10], key1[10];       // Philox round keys
 };

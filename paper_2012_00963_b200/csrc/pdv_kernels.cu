@@ -131,6 +131,14 @@ __device__ __noinline__ uint32_t class_walk(const uint32_t *thr, uint32_t c, uin
     return c;
 }
 
+// diffuse illumination of the cloud top (pdv_run_opts.launch_model 1): mu = -sqrt(xi), xi from word 0 of the block with
+// counter word 3 = 0xffffffff, which no flight ever reaches
+__device__ __noinline__ float diffuse_launch_mu(uint32_t id_lo, uint32_t id_hi, uint32_t stream, const uint4 *keys) {
+    uint32_t x0, x1, x2, x3;
+    philox4x32_10(id_lo, id_hi, stream, 0xFFFFFFFFu, keys, x0, x1, x2, x3);
+    return -fast_sqrt((__uint2float_rn(x0 >> 8) + 0.5f) * 5.9604644775390625e-8f);
+}
+
 // Lambertian surface (surface_model 1): mu = sqrt(xi)
 __device__ __noinline__ float lambert_mu(float pwf) { return fast_sqrt(pwf * 2.3283064365386963e-10f); }
 
@@ -274,6 +282,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             }
             T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u;
             if (NREFL) n_refl = 0u;
+            if (DM == 2 && P.launch_model) mu = diffuse_launch_mu(id_lo, id_hi, ud.stream, s_keys);      // unit-uniform, general kernel only
         };
         // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
         auto finish = [&](int fate) {

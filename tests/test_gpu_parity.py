@@ -427,6 +427,32 @@ def test_full_size_configs_3_4_5(P):
     assert top_g == pytest.approx(top_o, abs=5 * math.sqrt(top_o / oo.n_photons))
 
 
+@pytest.mark.parametrize("m0,d_um", [(1.0, 5.0), (3.0, 2.0)])
+def test_mean_path_invariance_on_the_device(P, m0, d_um):
+    """The CUDA transport against a theorem, with no reference implementation in the loop (pin P16 on the device):
+    non-absorbing particles (real index 1.5, full Mie table), lossless Lambertian bottom, diffuse illumination
+    (launch_model 1) => per history <particle events> = 4 tau_ext, <surface reflections> = 1, and the light that leaves is
+    Lambertian: P(mu_exit >= mu_a) = 1 - mu_a^2.  1e8 histories: the 5 sigma band is 1.5e-4 of the value, far below anything
+    a wrong constant, a biased uniform or a sloppy approximation in the fp32 flight could hide in."""
+    params = dict(W._cloud(m0, 4.0, 2000.0, diameter_um=d_um), m_re=1.5, m_im=0.0, surface_model=1, surface_reflectivity=1.0)
+    c = P.pdv_cloud_create(params)
+    tau = c.info()["tau_ext"]
+    run = dict(W.config(1)["run"], aperture_sr=0.1, v_lo=-20000.0, v_hi=20000.0, launch_model=1)
+    _, rec = P.pdv_mc_trace(c, 0, 200_000, 5, run)                      # spread of the per-history counts
+    sd_ev, sd_rf = rec["n_scatter"].std(), rec["n_reflect"].std()
+    n = 100_000_000
+    r = P.pdv_mc_run([c], [1e-6], n, 77, run)
+    s = r.stats[0, 0]
+    assert s["histories"] == n and s["absorbed_particles"] == 0.0 and s["absorbed_surface"] == 0.0
+    assert s["particle_events"] / n == pytest.approx(4.0 * tau, abs=5 * sd_ev / math.sqrt(n))
+    assert s["surface_reflections"] / n == pytest.approx(1.0, abs=5 * sd_rf / math.sqrt(n))
+    p_in = 1.0 - (1.0 - 0.1 / (2 * math.pi)) ** 2
+    assert (s["detected"] + s["underflow"] + s["overflow"]) / n == pytest.approx(p_in, abs=5 * math.sqrt(p_in / n))
+    # not vacuous: the collimated beam on the same cloud does not give 4 tau
+    r0 = P.pdv_mc_run([c], [1e-6], 1_000_000, 77, dict(run, launch_model=0))
+    assert abs(r0.stats[0, 0]["particle_events"] / 1e6 - 4.0 * tau) > 0.05 * 4.0 * tau
+
+
 def test_rare_paths_stress_many_short_runs(P):
     """Short runs that spend most of their time in the rare paths (roulette kill / survive, analog absorption,
     single-scatter truncation, drained-queue lanes) in varying order: every run must complete, conserve weight
