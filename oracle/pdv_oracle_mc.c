@@ -33,9 +33,10 @@
  * SURVEY.md 8(c)), and the multiple-scattering transport core (free paths, direction updates,
  * reflections, over many events) by the mean-path invariance of a non-absorbing medium under diffuse
  * illumination (P16: <events> = 4 tau_ext, <reflections> = 1, Lambertian exit; launch_model 1).  The
- * Doppler bookkeeping is pinned per event (P2, P3).  Their composition, the SHAPE of the
- * multiple-scattering spectrum, has no closed form and no figure data is available: "parity
- * unpinned" for that output beyond those pins.
+ * Doppler bookkeeping is pinned per event (P2, P3) and over whole multiple-scattering histories in
+ * a rigid cloud, where it telescopes to the exit angle (P17).  The SHAPE of the multiple-scattering
+ * spectrum of a cloud with a velocity profile has no closed form and no figure data is available:
+ * "parity unpinned" for that output beyond those pins.
  */
 #include <math.h>
 #include <pthread.h>

@@ -454,6 +454,32 @@ def test_mean_path_invariance_on_the_device(P, m0, d_um):
     assert abs(r0.stats[0, 0]["particle_events"] / 1e6 - 4.0 * tau) > 20 * sd_ev / math.sqrt(1e6)       # 2.7 % ... 12 % off
 
 
+@pytest.mark.parametrize("poly", [False, True])
+def test_rigid_cloud_doppler_telescopes_on_the_device(P, poly):
+    """Pin P17 on the device, no reference in the loop: particles and free surface all at v = 2000 m/s => the Doppler
+    velocity of a history is (1 + mu_exit) v / 2 whatever its length, so all detected weight lies in
+    [(1 + mu_a)/2 v, v] = [1984.08, 2000.00] m/s.  fp32 accumulation over up to ~70 events: edges within 0.05 m/s."""
+    base = W.config(2 if poly else 1)["clouds"][0]
+    params = dict(base, area_mass=2.0e-2, profile_kind=1, prof_v=np.array([2000.0, 2000.002]), prof_cum_mass=np.array([0.0, 1.0]),
+                  vmax_ratio=1.000001)
+    c = P.pdv_cloud_create(params)
+    n, nb, lo, hi = 20_000_000, 2000, 1950.0, 2050.0               # 0.05 m/s per bin (16 classes + 8000 bins exceed shared memory)
+    run = dict(W.config(1)["run"], n_bins=nb, v_lo=lo, v_hi=hi)
+    r = P.pdv_mc_run([c], [1e-6], n, 17, run)
+    s = r.stats[0, 0]
+    assert s["particle_events"] / n > 5.0 and s["max_events_in_history"] > 50
+    assert s["underflow"] == 0.0 and s["overflow"] == 0.0 and s["detected"] / n > 0.01
+    mu_a = 1.0 - 0.1 / (2 * math.pi)
+    centres = lo + (np.arange(nb) + 0.5) * (hi - lo) / nb
+    inside = (centres > 0.5 * (1 + mu_a) * 2000.0 - 0.05) & (centres < 2000.002 + 0.05)
+    h = r.hist[0, 0]
+    assert h[~inside].sum() == 0.0 and h[inside].sum() == pytest.approx(s["detected"], rel=1e-12)
+    _, rec = P.pdv_mc_trace(c, 0, 300_000, 17, run)
+    out = rec["fate"] != 2
+    resid = rec["vt"][out].astype(np.float64) - 0.5 * (1.0 + rec["mu_exit"][out].astype(np.float64)) * 2000.0
+    assert np.max(np.abs(resid)) < 0.05
+
+
 def test_rare_paths_stress_many_short_runs(P):
     """Short runs that spend most of their time in the rare paths (roulette kill / survive, analog absorption,
     single-scatter truncation, drained-queue lanes) in varying order: every run must complete, conserve weight

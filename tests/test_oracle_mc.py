@@ -297,3 +297,32 @@ def test_multiple_scattering_core_obeys_the_mean_path_invariance(m0, d_um):
     # the same cloud under the paper's collimated beam does NOT have these values: the pin is not vacuous
     r0 = mc.run(c, dict(run, seed=31), n_photons=100_000)
     assert abs(r0.stats["particle_events"] / 100_000 - 4.0 * c.tau_ext) > 0.05 * 4.0 * c.tau_ext
+
+
+@pytest.mark.parametrize("kw", [dict(), dict(mode=1)])
+def test_rigid_cloud_doppler_telescopes_to_the_exit_angle_P17(kw):
+    """A closed form for the MULTIPLE-scattering spectrum, in a special cloud: if every particle and the free surface move
+    with the same velocity v, the shifts of Eq. 4 telescope over any number of events,
+        v~ = 1/2 sum_k (mu_k_out - mu_k_in) v = 1/2 (mu_exit - mu_launch) v = 1/2 (1 + mu_exit) v     (collimated launch),
+    so every detected photon (mu_exit >= mu_a) lands in [ (1 + mu_a)/2 v, v ] whatever happened to it on the way -- with
+    0.1 sr and v = 2000 m/s that is [1984.08, 2000] m/s out of a 0-6000 m/s axis.  A dropped, doubled or wrongly signed
+    term at ANY event of a long history puts weight outside.  Cloud: tabulated profile with all the mass within 2 mm/s of
+    v_fs, 2 mg/cm^2 (7 events per history on average, up to ~70)."""
+    base = W.config(1)["clouds"][0]
+    params = dict(base, profile_kind=1, prof_v=np.array([2000.0, 2000.002]), prof_cum_mass=np.array([0.0, 1.0]),
+                  vmax_ratio=1.000001)
+    c = cloud.build_cloud(params)
+    assert c.v_max == pytest.approx(2000.002, abs=1e-9)
+    n, nb, lo, hi = 400_000, 8000, 1900.0, 2100.0
+    run = dict(W.config(1)["run"], n_bins=nb, v_lo=lo, v_hi=hi, **kw)
+    r = mc.run(c, dict(run, seed=17), n_photons=n, trace=True)
+    assert r.stats["particle_events"] / n > 3.5 and r.trace["n_scatter"].max() > 30      # analog histories are shorter
+    assert r.stats["underflow"] == 0.0 and r.stats["overflow"] == 0.0
+    mu_a = mc.aperture_mu(0.1)
+    centres = lo + (np.arange(nb) + 0.5) * (hi - lo) / nb
+    inside = (centres > 0.5 * (1 + mu_a) * 2000.0 - 0.05) & (centres < 2000.002 + 0.05)
+    assert r.hist[~inside].sum() == 0.0 and r.hist[inside].sum() == pytest.approx(r.stats["detected"], rel=1e-12)
+    assert r.stats["detected"] / n > 0.01
+    # history by history: v~ = (1 + mu_exit) v / 2 for every photon that left through the top, detected or not
+    out = r.trace["fate"] <= 1
+    assert np.max(np.abs(r.trace["vt"][out] - 0.5 * (1.0 + r.trace["mu_exit"][out]) * 2000.0)) < 0.002 * 40
