@@ -325,7 +325,7 @@ def main():
         alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
         achieved = alg / (tr_ms * 1e-3)
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "transport_thread_inst.json")     # written by hand from the ncu capture
+        tpath = os.path.join(ROOT, "profiles", "transport_thread_inst.txt")     # written by hand from the ncu capture
         if os.path.exists(tpath):
             with open(tpath) as f:
                 tj = json.load(f)
