@@ -124,7 +124,9 @@ void mie_phase_quantiles(double x, double m_re, double m_im, int K, double *M, i
     std::vector<cplx> a, b;
     mie_ab(x, cplx(m_re, m_im), a, b);
     // psi = pi - theta in [0, pi]; mu = -cos(psi) increases with psi; density in psi: I(mu) sin(psi).
-    const int n_panel = std::max(16384, (int)std::ceil(300.0 * x));   // Simpson panels of two intervals
+    // Simpson panels of two intervals.  I(mu) is a polynomial of degree ~2x in mu: 4096 panels (or 300 per unit of x) leave the
+    // quantiles within 6e-12 of the 16384-panel ones for x = 2 ... 20 (measured), 1e-9 being what the tests ask for
+    const int n_panel = std::max(4096, (int)std::ceil(300.0 * x));
     const int N = 2 * n_panel;
     const double h = kPi / N;
     std::vector<double> gv(N + 1);
