@@ -62,18 +62,21 @@ def spectrum_peak(hist, n_photons: int, v_lo: float, v_hi: float, v_fs: float, *
         if x_min <= x[k] <= x_max and sm[k] > best:
             k_star, best = k, sm[k]
     if k_star < 0:
-        return dict(x_peak=0.0, i_peak=0.0, curvature=0.0, k_peak=-1, status=1)
+        return dict(x_peak=0.0, i_peak=0.0, curvature=0.0, k_peak=-1, status=1, beta_eq35=0.0, tau0_eq35=0.0)
     lo, hi = max(0, k_star - fit_half), min(n - 1, k_star + fit_half)
     if hi - lo + 1 < 3:
-        return dict(x_peak=float(x[k_star]), i_peak=float(sm[k_star]), curvature=0.0, k_peak=k_star, status=1)
+        return dict(x_peak=float(x[k_star]), i_peak=float(sm[k_star]), curvature=0.0, k_peak=k_star, status=1, beta_eq35=0.0,
+                    tau0_eq35=0.0)
     u = x[lo:hi + 1] - x[k_star]                                         # R29
     design = np.stack([np.ones_like(u), u, u * u], axis=1)
     (a, b, c), *_ = np.linalg.lstsq(design, s[lo:hi + 1], rcond=None)
     if not c < 0.0:
-        return dict(x_peak=float(x[k_star]), i_peak=float(sm[k_star]), curvature=0.0, k_peak=k_star, status=2)
+        return dict(x_peak=float(x[k_star]), i_peak=float(sm[k_star]), curvature=0.0, k_peak=k_star, status=2, beta_eq35=0.0,
+                    tau0_eq35=0.0)
     i_peak = a - b * b / (4.0 * c)
-    return dict(x_peak=float(x[k_star] - b / (2.0 * c)), i_peak=float(i_peak), curvature=float(2.0 * c / i_peak),
-                k_peak=k_star, status=0)
+    x_peak, curv = float(x[k_star] - b / (2.0 * c)), float(2.0 * c / i_peak)
+    beta, tau0 = ejecta_from_peak(x_peak, curv)
+    return dict(x_peak=x_peak, i_peak=float(i_peak), curvature=curv, k_peak=k_star, status=0, beta_eq35=beta, tau0_eq35=tau0)
 
 
 def spectrum_peaks(hist, n_photons: int, v_lo: float, v_hi: float, v_fs, **kw) -> list:
@@ -81,3 +84,14 @@ def spectrum_peaks(hist, n_photons: int, v_lo: float, v_hi: float, v_fs, **kw) -
     hist = np.atleast_2d(np.asarray(hist, dtype=np.float64))
     v = np.broadcast_to(np.asarray(v_fs, dtype=np.float64), (hist.shape[0],))
     return [spectrum_peak(hist[i], n_photons, v_lo, v_hi, float(v[i]), **kw) for i in range(hist.shape[0])]
+
+
+def ejecta_from_peak(x_peak: float, curvature: float):
+    """Eq. 35 read backwards (section III.C): the relative curvature at the peak gives the velocity
+    profile coefficient, beta = sqrt(-I''/I); the peak position then gives the optical thickness, tau0 = exp(beta (x_peak - 1)).
+    (For a weight tally, R31, that tau0 is 2 g tau_ext.)  Returns (beta, tau0); (0, 0) if the curvature is not negative."""
+    if not curvature < 0.0:
+        return 0.0, 0.0
+    beta = (-curvature) ** 0.5
+    return beta, float(np.exp(beta * (x_peak - 1.0)))
+

@@ -95,3 +95,23 @@ def test_status_codes():
     assert cup["status"] == 2 and cup["curvature"] == 0.0
     empty = peak.spectrum_peak(np.zeros(32), 0, v_lo, v_hi, v_fs, x_min=0.0)   # n_photons = 0: zero spectrum
     assert empty["status"] == 2 and empty["i_peak"] == 0.0
+
+
+def test_eq35_read_backwards_reproduces_the_papers_printed_estimate():
+    """peak at v/v_fs = 1.32, relative curvature about -110 => beta = 10.5 and tau0 = 28.79."""
+    import os
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_printed_values.txt")):
+        if line.strip() and not line.startswith("#"):
+            name, val, tol = line.split()[:3]
+            gold[name] = (float(val), float(tol))
+    beta, tau0 = peak.ejecta_from_peak(1.32, -110.0)
+    assert beta == pytest.approx(gold["eq35_beta_from_curvature"][0], abs=gold["eq35_beta_from_curvature"][1])
+    _, tau0_rounded = peak.ejecta_from_peak(1.32, -(10.5 ** 2))            # the paper continues with the rounded beta
+    assert tau0_rounded == pytest.approx(gold["eq35_tau0_from_position"][0], abs=gold["eq35_tau0_from_position"][1])
+    assert tau0 == pytest.approx(28.79, rel=5e-3)
+    assert peak.ejecta_from_peak(1.2, 0.0) == (0.0, 0.0) and peak.ejecta_from_peak(1.2, 3.0) == (0.0, 0.0)
+    r = peak.spectrum_peak(np.maximum(3.0 - 40.0 * (np.arange(512) / 512 * 3 + 3 / 1024 - 1.3) ** 2, 0), 1, 0.0, 6000.0, 2000.0)
+    assert r["beta_eq35"] == pytest.approx(math.sqrt(-r["curvature"])) and r["tau0_eq35"] == pytest.approx(
+        math.exp(r["beta_eq35"] * (r["x_peak"] - 1.0)))
+
