@@ -224,6 +224,8 @@ typedef struct {
     double curvature;            /* I''/I at the peak          (Eq. 34), per unit x squared */
     int32_t k_peak;              /* arg-max bin k*, -1 if none */
     int32_t status;
+    double beta_eq35;            /* Eq. 35 read backwards: beta = sqrt(-curvature); 0 unless status = 0 */
+    double tau0_eq35;            /* tau0 = exp(beta (x_peak - 1)); for this library's weight tally that is 2 g tau_ext (R31) */
 } pdv_peak;
 
 /* hist [n_units][n_bins] doubles, v_fs [n_units] doubles (m/s, > 0), out [n_units]: all three HOST when on_device = 0,

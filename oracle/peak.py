@@ -93,5 +93,6 @@ def ejecta_from_peak(x_peak: float, curvature: float):
     if not curvature < 0.0:
         return 0.0, 0.0
     beta = (-curvature) ** 0.5
-    return beta, float(np.exp(beta * (x_peak - 1.0)))
+    with np.errstate(over="ignore"):                      # a noise spectrum can give any exponent: inf is the honest answer
+        return beta, float(np.exp(beta * (x_peak - 1.0)))
 

@@ -60,7 +60,8 @@ STAT_INTS = ("histories", "particle_events", "surface_reflections", "max_events_
 STATS_DTYPE = np.dtype([(n, "f8") for n in STAT_FLOATS] + [(n, "u8") for n in STAT_INTS])
 TRACE_DTYPE = np.dtype([("vt", "f4"), ("weight", "f4"), ("mu_exit", "f4"), ("fate", "i4"), ("n_scatter", "i4"),
                         ("n_reflect", "i4")])
-PEAK_DTYPE = np.dtype([("x_peak", "f8"), ("i_peak", "f8"), ("curvature", "f8"), ("k_peak", "i4"), ("status", "i4")])
+PEAK_DTYPE = np.dtype([("x_peak", "f8"), ("i_peak", "f8"), ("curvature", "f8"), ("k_peak", "i4"), ("status", "i4"),
+                       ("beta_eq35", "f8"), ("tau0_eq35", "f8")])
 
 
 class PhaseCheck(C.Structure):

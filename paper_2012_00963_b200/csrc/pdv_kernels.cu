@@ -688,7 +688,7 @@ __global__ void __launch_bounds__(256) peak_kernel(const double *hist, int n_bin
     if (tid != 0) return;
     pdv_peak r;
     const int ks = red_k[0];
-    r.k_peak = ks; r.x_peak = 0.0; r.i_peak = 0.0; r.curvature = 0.0; r.status = 1;
+    r.k_peak = ks; r.x_peak = 0.0; r.i_peak = 0.0; r.curvature = 0.0; r.status = 1; r.beta_eq35 = 0.0; r.tau0_eq35 = 0.0;
     if (ks >= 0) {
         r.x_peak = xk(ks); r.i_peak = a[ks];
         const int lo = max(0, ks - o.fit_half), hi = min(n_bins - 1, ks + o.fit_half);
@@ -710,6 +710,10 @@ __global__ void __launch_bounds__(256) peak_kernel(const double *hist, int n_bin
                 r.i_peak = ip;
                 r.curvature = 2.0 * C / (dx * dx * ip);
                 r.status = 0;
+                if (r.curvature < 0.0) {                      // Eq. 35 read backwards
+                    r.beta_eq35 = sqrt(-r.curvature);
+                    r.tau0_eq35 = exp(r.beta_eq35 * (r.x_peak - 1.0));
+                }
             } else {
                 r.status = 2;
             }

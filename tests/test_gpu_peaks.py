@@ -25,7 +25,7 @@ def _compare(P, opeak, hist, n, v_lo, v_hi, v_fs, **kw):
     assert len(got) == len(want)
     for g, w in zip(got, want):
         assert int(g["k_peak"]) == w["k_peak"] and int(g["status"]) == w["status"], (g, w)
-        for key in ("x_peak", "i_peak", "curvature"):
+        for key in ("x_peak", "i_peak", "curvature", "beta_eq35", "tau0_eq35"):
             assert float(g[key]) == pytest.approx(w[key], rel=1e-9, abs=1e-300), (key, g, w)
     return got
 
