@@ -20,6 +20,7 @@ struct pdv_cloud {
     std::vector<unsigned char> blob;     // device image (host copy)
     mutable std::mutex mu;
     mutable unsigned char *d_blob = nullptr;
+    mutable size_t d_bytes = 0;
     mutable int device = -1;
 };
 
@@ -190,12 +191,47 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     }
 }
 
+// Device images of destroyed clouds are kept for the next cloud instead of going back to the driver: cudaFree was measured at
+// 0.5 ... 750 ms for the 14 images of a sweep (it synchronises the device and may unmap memory).  At most 64 buffers / 64 MiB.
+struct BlobCache {
+    struct Entry { unsigned char *p; size_t bytes; int device; };
+    std::mutex mu;
+    std::vector<Entry> free_list;
+    size_t total = 0;
+    unsigned char *take(size_t bytes, int device) {           // smallest cached buffer that is large enough
+        std::lock_guard<std::mutex> lk(mu);
+        int best = -1;
+        for (int i = 0; i < (int)free_list.size(); ++i)
+            if (free_list[i].device == device && free_list[i].bytes >= bytes && (best < 0 || free_list[i].bytes < free_list[best].bytes)) best = i;
+        if (best < 0) return nullptr;
+        unsigned char *p = free_list[best].p;
+        total -= free_list[best].bytes;
+        free_list.erase(free_list.begin() + best);
+        return p;
+    }
+    bool give(unsigned char *p, size_t bytes, int device) {
+        std::lock_guard<std::mutex> lk(mu);
+        if (free_list.size() >= 64 || total + bytes > ((size_t)64 << 20)) return false;
+        free_list.push_back({p, bytes, device});
+        total += bytes;
+        return true;
+    }
+};
+BlobCache g_blob_cache;
+
 pdv_status ensure_on_device(const pdv_cloud *c, int device) {
     std::lock_guard<std::mutex> lk(c->mu);
     if (c->d_blob && c->device == device) return PDV_OK;
     if (c->d_blob) return fail(PDV_E_INVALID, "cloud was uploaded to another CUDA device");
-    unsigned char *d = nullptr;
-    CU(cudaMalloc(&d, c->blob.size()), "cudaMalloc(cloud tables)");
+    unsigned char *d = g_blob_cache.take(c->blob.size(), device);
+    if (d) {
+        // the buffer belonged to a destroyed cloud: whatever may still read it (a run enqueued on a non-blocking stream)
+        // must be over before it is overwritten -- what cudaFree used to guarantee
+        CU(cudaDeviceSynchronize(), "cudaDeviceSynchronize(reuse of a cloud buffer)");
+    } else {
+        CU(cudaMalloc(&d, c->blob.size()), "cudaMalloc(cloud tables)");
+    }
+    c->d_bytes = c->blob.size();                              // a reused buffer may be larger: only this much is vouched for
     cudaError_t e = cudaMemcpy(d, c->blob.data(), c->blob.size(), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(cloud tables)"); }
     c->d_blob = d;
@@ -511,7 +547,7 @@ pdv_status pdv_cloud_create(const pdv_cloud_params *params, pdv_cloud **out) {
 
 void pdv_cloud_destroy(pdv_cloud *c) {
     if (!c) return;
-    if (c->d_blob) cudaFree(c->d_blob);
+    if (c->d_blob && !g_blob_cache.give(c->d_blob, c->d_bytes, c->device)) cudaFree(c->d_blob);
     delete c;
 }
 
