@@ -18,3 +18,11 @@ def cfg2_oracle_cloud():
     import pdv_workloads as W
     from oracle import cloud
     return cloud.build_cloud(W.config(1)["clouds"][0])
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _library_is_built():
+    """The in-tree CUDA library is (re)built once per session when a source is newer than it: nvcc cross-compiles without a
+    GPU, and every test module may then load it."""
+    from paper_2012_00963_b200 import build as pbuild
+    pbuild.build()
