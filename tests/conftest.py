@@ -20,9 +20,11 @@ def cfg2_oracle_cloud():
     return cloud.build_cloud(W.config(1)["clouds"][0])
 
 
-@pytest.fixture(scope="session", autouse=True)
+@pytest.fixture(scope="session")
 def _library_is_built():
-    """The in-tree CUDA library is (re)built once per session when a source is newer than it: nvcc cross-compiles without a
-    GPU, and every test module may then load it."""
+    """The in-tree CUDA library is (re)built once per session when a source is newer than it (nvcc cross-compiles without a
+    GPU).  Requested only by the modules that load the library (ABI, shard, GPU tests: `pytestmark = usefixtures(...)`); the
+    oracle's own pins (tests/test_oracle_*.py) neither build nor load the product, so they run on a box without nvcc and an
+    nvcc failure cannot mask an oracle failure."""
     from paper_2012_00963_b200 import build as pbuild
     pbuild.build()

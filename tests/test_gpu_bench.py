@@ -6,7 +6,7 @@ import sys
 
 import pytest
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("_library_is_built")]
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 

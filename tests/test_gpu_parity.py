@@ -17,7 +17,7 @@ from oracle import mc as omc
 
 from histcmp import compare
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("_library_is_built")]
 
 
 @pytest.fixture(scope="module")

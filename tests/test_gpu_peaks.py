@@ -13,7 +13,7 @@ import pytest
 
 import pdv_workloads as W
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("_library_is_built")]
 
 OPTION_SETS = [dict(half=6, n_pass=2, fit_half=12, x_min=1.03), dict(half=0, n_pass=0, fit_half=1, x_min=0.0),
                dict(half=15, n_pass=3, fit_half=40, x_min=1.03, x_max=1.6), dict(half=1, n_pass=16, fit_half=3, x_min=0.5)]

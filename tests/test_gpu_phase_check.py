@@ -13,7 +13,7 @@ import pytest
 import pdv_workloads as W
 from oracle import cloud as ocloud, mie as omie, phase_check as opc
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("_library_is_built")]
 M_SN = complex(W.M_RE, W.M_IM)
 
 
