@@ -164,7 +164,15 @@ typedef struct {                 /* weights in units of photons; identity (exact
  * Reproducibility: the same (clouds, n_snap, n_photons, seed, first_photon_id, opts) give bit-identical
  * hist/hist2/stats for any launch shape -- tallies are integer fixed point (Q31) and every history draws
  * from its own Philox4x32-10 counter stream keyed by (seed, photon id, unit).  Runs over id ranges [a,b)
- * and [b,c) sum to the run over [a,c).  n_photons = 0 is valid and yields zeros. */
+ * and [b,c) sum to the run over [a,c).  n_photons = 0 is valid and yields zeros.
+ * Limits: n_photons <= 2^33 per unit (a tally is a Q31 sum in 64 bits: it holds the weight of 2^33 photons; larger runs are
+ * split by the caller into id ranges, whose results add), n_clouds * n_snap <= 2^20, photon ids below 2^63; otherwise
+ * PDV_E_INVALID.
+ * Streams: every call takes its device scratch (id cursors, Q31 tallies, unit table, output staging) from the device's
+ * stream-ordered memory pool on cuda_stream and releases it there behind its last kernel, so calls enqueued on DIFFERENT
+ * streams, from one host thread or several, are independent of each other, and calls on one stream run in order.  With
+ * output_on_device = 1 the caller's device buffers must stay valid, and the clouds alive, until the work enqueued on
+ * cuda_stream has finished. */
 pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const double *t_snap, int32_t n_snap,
                       uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
                       double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream);

@@ -32,16 +32,16 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile the CUDA library if a source is newer than the .so.  Returns the .so path."""
-    if force or needs_build():
-        tmp = LIB + f".tmp{os.getpid()}"
-        extra = os.environ.get("PDV_NVCC_EXTRA", "").split()          # e.g. -DPDV_BLOCKS_POLY=2 (kernel experiments)
-        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str | None = None) -> str:
+    """Compile the CUDA library if a source is newer than the .so.  Returns the .so path.
+    extra_flags / out: an experiment build (-D macros of csrc/) into another file; the product build passes neither."""
+    if out is not None or force or needs_build():
+        tmp = (out or LIB) + f".tmp{os.getpid()}"
+        cmd = [_nvcc()] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
         subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, out or LIB)
+    return out or LIB
 
 
 if __name__ == "__main__":

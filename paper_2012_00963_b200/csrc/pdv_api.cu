@@ -29,16 +29,21 @@ namespace {
 thread_local std::string g_err;
 thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0; bool pending = false; } g_last;
 
-struct Workspace {
-    unsigned char *d = nullptr;
-    size_t bytes = 0;
-    int device = -1;
+// Timing events of the last run of this host thread (pdv_last_launch_info).
+struct LastEvents {
     cudaEvent_t e0 = nullptr, e1 = nullptr;
-    ~Workspace() {
-        // process teardown: the CUDA context may already be gone; leak rather than fault
-    }
+    int device = -1;
+    // process teardown: the CUDA context may already be gone; leak rather than fault
 };
-thread_local Workspace g_ws;
+thread_local LastEvents g_ev;
+
+// Pinned host staging buffer of this host thread for the read-back of a host-output run (one D2H copy at PCIe speed instead
+// of several pageable ones); grown on demand, never shrunk.
+struct PinnedStage {
+    unsigned char *p = nullptr;
+    size_t bytes = 0;
+};
+thread_local PinnedStage g_stage;
 
 pdv_status fail(pdv_status s, const std::string &msg) { g_err = msg; return s; }
 pdv_status cuda_fail(cudaError_t e, const char *what) {
@@ -108,7 +113,6 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
             guide.assign(n_guide, 0);
         }
     }
-    if (std::getenv("PDV_X_DEBUG")) fprintf(stderr, "blob: nd=%d n_guide=%u shift=%u bisect=%u tau=%g\n", nd, n_guide, shift, bisect, (double)Tf[nd]);
     DevCloudHeader hd;
     std::memset(&hd, 0, sizeof(hd));
     size_t off = sizeof(DevCloudHeader);
@@ -118,7 +122,37 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * n_pad);
     hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
-    hd.off_cguide = (uint32_t)off; off = align16(off + 256);
+    // class thresholds first: the class guide is sized from them (layout: pdv_device.h)
+    std::vector<uint32_t> thr_v(n_pad, 0xFFFFFFFFu);
+    {
+        double cum = 0.0;
+        for (int c = 0; c < nc - 1; ++c) {
+            cum += h.p_class[c];
+            const double v = std::ceil(cum * 4294967296.0 - 0.5);     // x1 + 0.5 >= cum 2^32
+            thr_v[c] = v <= 0.0 ? 0u : (v >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)v);
+        }
+    }
+    auto cell_counts = [&](uint32_t sh, uint32_t g, int &below, int &inside) {
+        const uint32_t first = g << sh, last = first | ((1u << sh) - 1u);
+        below = inside = 0;
+        for (int j = 0; j < nc - 1; ++j) {
+            if (thr_v[j] <= first) ++below;
+            else if (thr_v[j] <= last) ++inside;
+        }
+    };
+    uint32_t cg_shift = 24;                                   // coarsest guide without a cell that holds two thresholds
+    for (; cg_shift > 20; --cg_shift) {
+        bool clean = true;
+        for (uint32_t g = 0; g < (1u << (32 - cg_shift)) && clean; ++g) {
+            int below, inside;
+            cell_counts(cg_shift, g, below, inside);
+            clean = inside <= 1;
+        }
+        if (clean) break;
+    }
+    const uint32_t n_cg = nc > 1 ? 1u << (32 - cg_shift) : 16u;
+    hd.off_cguide = (uint32_t)off; off = align16(off + n_cg);
+    hd.cguide_shift = cg_shift;
     hd.blob_bytes = (uint32_t)off;
     hd.n_classes = nc; hd.K = K; hd.n_depth = nd; hd.n_guide = n_guide; hd.guide_base = base;
     hd.guide_shift = shift; hd.depth_bisect = bisect;
@@ -165,28 +199,17 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     uint32_t *thr = reinterpret_cast<uint32_t *>(blob.data() + hd.off_thr);
     float *alb = reinterpret_cast<float *>(blob.data() + hd.off_albedo);
     uint32_t *albt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albthr);
-    double cum = 0.0;
     for (int c = 0; c < n_pad; ++c) {
-        if (c < nc - 1) {
-            cum += h.p_class[c];
-            const double v = std::ceil(cum * 4294967296.0 - 0.5);     // x1 + 0.5 >= cum 2^32
-            thr[c] = v <= 0.0 ? 0u : (v >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)v);
-        } else {
-            thr[c] = 0xFFFFFFFFu;
-        }
+        thr[c] = thr_v[c];
         const double om = c < nc ? h.k_sca[c] / h.k_ext[c] : 0.0;
         alb[c] = (float)std::min(std::max(om, 0.0), 1.0);
         albt[c] = to_thr32(om);
     }
     std::memcpy(blob.data() + hd.off_guide, guide.data(), sizeof(uint16_t) * n_guide);
     unsigned char *cg = blob.data() + hd.off_cguide;          // class guide (layout: pdv_device.h)
-    for (uint32_t g = 0; g < 256u; ++g) {
-        const uint32_t first = g << 24, last = first | 0x00FFFFFFu;
-        int below = 0, inside = 0;
-        for (int j = 0; j < nc - 1; ++j) {
-            if (thr[j] <= first) ++below;
-            else if (thr[j] <= last) ++inside;
-        }
+    for (uint32_t g = 0; nc > 1 && g < n_cg; ++g) {
+        int below, inside;
+        cell_counts(cg_shift, g, below, inside);
         cg[g] = (unsigned char)(below | (inside > 1 ? 0x80 : 0));
     }
 }
@@ -239,22 +262,57 @@ pdv_status ensure_on_device(const pdv_cloud *c, int device) {
     return PDV_OK;
 }
 
-pdv_status get_workspace(size_t bytes, int device, unsigned char **out) {
-    Workspace &w = g_ws;
-    if (w.d && (w.device != device || w.bytes < bytes)) {
-        cudaFree(w.d);
-        w.d = nullptr; w.bytes = 0;
+// Device scratch of ONE call (tally workspace, unit table, output staging): allocated on the caller's stream from the device's
+// stream-ordered pool and released, in stream order, behind the call's last kernel.  Two runs enqueued on different streams
+// (output_on_device = 1) therefore never share cursors or tallies, and nothing a kernel in flight uses is ever freed or
+// reused early.  The pool keeps its memory (release threshold = max), so after the first call this costs microseconds.
+struct StreamScratch {
+    unsigned char *p = nullptr;
+    cudaStream_t st = nullptr;
+    ~StreamScratch() { if (p) cudaFreeAsync(p, st); }
+};
+pdv_status scratch_alloc(size_t bytes, int device, cudaStream_t st, StreamScratch &out) {
+    static std::mutex mu;
+    static bool pool_ready[64] = {false};
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        if (!pool_ready[device & 63]) {
+            cudaMemPool_t pool;
+            CU(cudaDeviceGetDefaultMemPool(&pool, device), "cudaDeviceGetDefaultMemPool");
+            unsigned long long keep = ~0ull;
+            CU(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep), "cudaMemPoolSetAttribute");
+            pool_ready[device & 63] = true;
+        }
     }
-    if (!w.d) {
-        const size_t want = std::max(bytes, (size_t)1 << 20);
-        CU(cudaMalloc(&w.d, want), "cudaMalloc(workspace)");
-        w.bytes = want; w.device = device;
+    void *p = nullptr;
+    CU(cudaMallocAsync(&p, std::max(bytes, (size_t)256), st), "cudaMallocAsync(workspace)");
+    out.p = static_cast<unsigned char *>(p);
+    out.st = st;
+    return PDV_OK;
+}
+
+pdv_status ensure_events(int device) {
+    if (g_ev.e0 && g_ev.device != device) {
+        cudaEventDestroy(g_ev.e0); cudaEventDestroy(g_ev.e1);
+        g_ev.e0 = g_ev.e1 = nullptr;
     }
-    if (!w.e0) {
-        CU(cudaEventCreate(&w.e0), "cudaEventCreate");
-        CU(cudaEventCreate(&w.e1), "cudaEventCreate");
+    if (!g_ev.e0) {
+        CU(cudaEventCreate(&g_ev.e0), "cudaEventCreate");
+        CU(cudaEventCreate(&g_ev.e1), "cudaEventCreate");
+        g_ev.device = device;
     }
-    *out = w.d;
+    return PDV_OK;
+}
+
+pdv_status stage_buffer(size_t bytes, unsigned char **out) {
+    if (g_stage.bytes < bytes) {
+        if (g_stage.p) cudaFreeHost(g_stage.p);
+        g_stage.p = nullptr; g_stage.bytes = 0;
+        const size_t want = std::max(bytes, (size_t)1 << 16);
+        CU(cudaMallocHost(&g_stage.p, want), "cudaMallocHost(read-back staging)");
+        g_stage.bytes = want;
+    }
+    *out = g_stage.p;
     return PDV_OK;
 }
 
@@ -337,7 +395,6 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
             odd = odd || hd.depth_bisect == 1u || hd.surface_model != 0u;
         }
         kv.dm = odd || (n_closed != 0 && n_closed != n_clouds) ? 2 : (n_closed ? 1 : 0);
-        if (const char *e = std::getenv("PDV_X_DM")) if (atoi(e) == 2) kv.dm = 2;      // experiments: force the general kernel
     }
 
     const DeviceInfo &di = device_info(device);
@@ -347,7 +404,6 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         return fail(PDV_E_UNSUPPORTED, "cloud tables + histogram exceed the shared memory of one block");
     // 1024 resident threads per SM (64 registers each): two blocks of 512 when their shared memory fits twice, else one of 1024
     int block = o->threads_per_block, per_sm = 0;
-    if (const char *e = std::getenv("PDV_X_BLOCK")) block = atoi(e);      // kernel experiments
     // polydisperse clouds: one block of PDV_LB_THREADS_POLY threads per SM (80 registers each), see pdv_device.h
     if (kv.poly) block = block == 0 ? PDV_LB_THREADS_POLY : std::min(block, PDV_LB_THREADS_POLY);
     if (block == 0) block = 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024 ? 512 : 1024;
@@ -371,18 +427,19 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     const long long useful = (long long)((total + block - 1) / block);       // one history per thread at least
     if (useful < grid) grid = std::max(1LL, useful);
     plan.shape.grid = (int)grid; plan.shape.block = block; plan.shape.smem = smem;
-    // Guided self-scheduling of photon ids: a lane claims clamp(remaining / (2 * threads on the unit), 1, chunk) ids
-    const double threads = (double)grid * block / std::min<double>((double)n_units, (double)grid);
-    double chunk = std::floor((double)n_photons / (threads * 4.0));
-    chunk = std::min(std::max(chunk, 1.0), 128.0);
-    rp.chunk = (uint32_t)chunk;
-    rp.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
-    rp.chunk_min = 1;
-    if (const char *e = std::getenv("PDV_X_CHUNKMIN")) rp.chunk_min = (uint32_t)std::max(1, atoi(e));
-    if (const char *e = std::getenv("PDV_X_CHUNKDIV")) rp.chunk_per_remaining = (float)(1.0 / (atof(e) * threads));
-    if (const char *e = std::getenv("PDV_X_CHUNKMAX")) rp.chunk = (uint32_t)std::max(1, atoi(e));
-    rp.chunk_min = std::min(rp.chunk_min, rp.chunk);
     return PDV_OK;
+}
+
+// Estimated flights (particle events + reflections + the exit flight) of one history in a cloud of vertical optical thickness
+// tau: only the RATIOS between the units of a launch matter (they place the blocks, see RunParams::block_start), and a wrong
+// estimate costs a few more unit visits, never a wrong result.  Measured on the configs of BASELINE.json: 4.9 (tau 1.25), 9.8
+// (1.87), 20 (4.1), 45 (9.3), 92 (18.7) -- the mean path of a slab grows linearly with its thickness.
+double estimated_flights(double tau, double mean_albedo, const pdv_run_opts *o) {
+    double f = 2.3 + 4.8 * tau;
+    if (o->max_events > 0) { const double m = 1.25 * o->max_events; f = m * (1.0 - std::exp(-f / m)); }
+    if (o->mode == 1) f = 1.0 / (1.0 / f + std::max(0.0, 1.0 - mean_albedo));      // analog histories end by absorption
+    if (o->single_scatter_only) f = std::min(f, 3.0);
+    return f;
 }
 
 pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, const uint32_t *unit_streams,
@@ -408,7 +465,9 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     if (s != PDV_OK) return s;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t nb = (size_t)o->n_bins;
-    // workspace layout
+    const int grid = plan.shape.grid;
+    // scratch layout: [cursors | Q31 hist | Q31 hist2 | stats] (zeroed) [unit table | block starts] (one H2D copy)
+    // [double hist | double hist2 | run stats] (host-output runs: one D2H copy)
     size_t off = 0;
     const size_t o_next = off;  off = align16(off + 8 * (size_t)n_units);
     const size_t o_hist = off;  off = align16(off + 8 * nb * n_units);
@@ -416,30 +475,54 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     const size_t o_stats = off; off = align16(off + 8 * (size_t)ST_COUNT * n_units);
     const size_t zero_bytes = off;
     const size_t o_units = off; off = align16(off + sizeof(UnitDesc) * (size_t)n_units);
+    const size_t o_start = off; off = align16(off + sizeof(uint32_t) * (size_t)grid);
+    const size_t table_bytes = off - o_units;
     const size_t o_oh = off;    off = align16(off + 8 * nb * n_units);
-    const size_t o_oh2 = off;   off = align16(off + 8 * nb * n_units);
-    const size_t o_os = off;    off = align16(off + sizeof(pdv_run_stats) * (size_t)n_units);
-    unsigned char *ws = nullptr;
-    if ((s = get_workspace(off, device, &ws)) != PDV_OK) return s;
+    const size_t o_oh2 = off;   off = align16(off + (hist2 ? 8 * nb * n_units : 0));
+    const size_t o_os = off;    off = align16(off + (stats ? sizeof(pdv_run_stats) * (size_t)n_units : 0));
+    const size_t out_bytes = off - o_oh;
+    StreamScratch scratch;
+    if ((s = scratch_alloc(off, device, st, scratch)) != PDV_OK) return s;
+    unsigned char *ws = scratch.p;
+    if ((s = ensure_events(device)) != PDV_OK) return s;
 
-    std::vector<UnitDesc> units(n_units);
-    for (int i = 0; i < n_clouds; ++i)
-        for (int j = 0; j < n_snap; ++j) {
-            UnitDesc &u = units[(size_t)i * n_snap + j];
-            u.cloud_blob = clouds[i]->d_blob;
-            u.stream = unit_streams ? unit_streams[(size_t)i * n_snap + j] : (uint32_t)(i * n_snap + j);
-            u.visit = 0;
+    // ---- unit table: visiting order (descending estimated cost), where each block starts, guided chunk sizes per unit ----
+    std::vector<unsigned char> table(table_bytes, 0);
+    UnitDesc *units = reinterpret_cast<UnitDesc *>(table.data());
+    uint32_t *block_start = reinterpret_cast<uint32_t *>(table.data() + (o_start - o_units));
+    {
+        std::vector<double> cost(n_units);
+        for (int i = 0; i < n_clouds; ++i) {
+            const HostCloud &h = clouds[i]->host;
+            double om = 0.0;
+            for (int c = 0; c < h.n_classes; ++c) om += h.p_class[c] * h.k_sca[c] / h.k_ext[c];
+            const double f = estimated_flights(h.tau_ext, om, o);
+            for (int j = 0; j < n_snap; ++j) cost[(size_t)i * n_snap + j] = f;
         }
-    {   // visiting order: descending cost.  The cost of a unit grows with the optical thickness of its cloud (events per
-        // history ~ tau^2 for thick clouds); n_photons is the same for all units.  Stable, so equal clouds keep their order.
         std::vector<uint32_t> ord(n_units);
         for (int k = 0; k < n_units; ++k) ord[k] = (uint32_t)k;
-        auto tau = [&](uint32_t k) { return clouds[k / n_snap]->host.tau_ext; };
-        std::stable_sort(ord.begin(), ord.end(), [&](uint32_t x, uint32_t y) { return tau(x) > tau(y); });
-        uint32_t n_lead = 0;
-        while (n_lead < (uint32_t)n_units && tau(ord[n_lead]) >= 0.99 * tau(ord[0])) ++n_lead;
+        std::stable_sort(ord.begin(), ord.end(), [&](uint32_t x, uint32_t y) { return cost[x] > cost[y]; });   // equal clouds keep their order
+        double total = 0.0;
+        for (int k = 0; k < n_units; ++k) total += cost[k];
+        for (int i = 0; i < n_clouds; ++i)
+            for (int j = 0; j < n_snap; ++j) {
+                const size_t k = (size_t)i * n_snap + j;
+                UnitDesc &u = units[k];
+                u.cloud_blob = clouds[i]->d_blob;
+                u.stream = unit_streams ? unit_streams[k] : (uint32_t)k;
+                // threads expected on this unit: its share of the grid, at least one block
+                const double threads = std::max(1.0, cost[k] / total * grid) * plan.shape.block;
+                u.chunk = (uint32_t)std::min(std::max(std::floor((double)n_photons / (threads * 4.0)), 1.0), 128.0);
+                u.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
+            }
         for (int k = 0; k < n_units; ++k) units[k].visit = ord[k];
-        plan.rp.n_lead = n_lead ? n_lead : 1u;
+        double cum = 0.0;                                          // cost line: unit ord[k] covers [cum, cum + cost)
+        int k = 0;
+        for (int b = 0; b < grid; ++b) {
+            const double x = (b + 0.5) / grid * total;
+            while (k + 1 < n_units && cum + cost[ord[k]] <= x) { cum += cost[ord[k]]; ++k; }
+            block_start[b] = (uint32_t)k;
+        }
     }
     pdv_trace_record *d_trace = nullptr;
     if (trace && n_photons) CU(cudaMalloc(&d_trace, sizeof(pdv_trace_record) * n_photons), "cudaMalloc(trace)");
@@ -447,9 +530,10 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
 #define CUX(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return cuda_fail(e_, what); } } while (0)
 
     CUX(cudaMemsetAsync(ws, 0, zero_bytes, st), "cudaMemsetAsync(workspace)");
-    CUX(cudaMemcpyAsync(ws + o_units, units.data(), sizeof(UnitDesc) * n_units, cudaMemcpyHostToDevice, st), "copy unit table");
+    CUX(cudaMemcpyAsync(ws + o_units, table.data(), table_bytes, cudaMemcpyHostToDevice, st), "copy unit table");
     RunParams &rp = plan.rp;
     rp.units = reinterpret_cast<const UnitDesc *>(ws + o_units);
+    rp.block_start = reinterpret_cast<const uint32_t *>(ws + o_start);
     rp.next_id = reinterpret_cast<unsigned long long *>(ws + o_next);
     rp.hist = reinterpret_cast<unsigned long long *>(ws + o_hist);
     rp.hist2 = reinterpret_cast<unsigned long long *>(ws + o_hist2);
@@ -458,12 +542,12 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
 
     g_last.n_kernels = 0; g_last.ms = 0.f; g_last.pending = false;
     g_last.grid = plan.shape.grid; g_last.block = plan.shape.block; g_last.smem = plan.shape.smem;
-    CUX(cudaEventRecord(g_ws.e0, st), "cudaEventRecord");
+    CUX(cudaEventRecord(g_ev.e0, st), "cudaEventRecord");
     if (n_photons > 0) {
         CUX(launch_transport(rp, plan.variant, plan.shape, st), "transport kernel launch");
         g_last.n_kernels += 1;
     }
-    CUX(cudaEventRecord(g_ws.e1, st), "cudaEventRecord");
+    CUX(cudaEventRecord(g_ev.e1, st), "cudaEventRecord");
     g_last.pending = true;               // elapsed time is read when the events have completed
 
     const bool dev_out = o->output_on_device != 0;
@@ -473,21 +557,19 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     CUX(launch_finalize(rp.hist, rp.hist2, rp.stats, (uint32_t)n_units, (uint32_t)nb, oh, oh2, os, st), "finalize kernel launch");
     g_last.n_kernels += 1;
     if (!dev_out) {
-        // stage into host temporaries first so that the caller's buffers stay untouched on failure
-        std::vector<double> th(nb * n_units), th2(hist2 ? nb * n_units : 0);
-        std::vector<pdv_run_stats> ts(stats ? n_units : 0);
-        std::vector<pdv_trace_record> tr;
-        CUX(cudaMemcpyAsync(th.data(), oh, 8 * nb * n_units, cudaMemcpyDeviceToHost, st), "read back hist");
-        if (hist2) CUX(cudaMemcpyAsync(th2.data(), oh2, 8 * nb * n_units, cudaMemcpyDeviceToHost, st), "read back hist2");
-        if (stats) CUX(cudaMemcpyAsync(ts.data(), os, sizeof(pdv_run_stats) * n_units, cudaMemcpyDeviceToHost, st), "read back stats");
+        // one D2H copy into this thread's pinned staging buffer; the caller's buffers are written only after everything
+        // has succeeded, so they stay untouched on failure
+        unsigned char *stage = nullptr;
+        if ((s = stage_buffer(out_bytes, &stage)) != PDV_OK) { cleanup(); return s; }
+        CUX(cudaMemcpyAsync(stage, ws + o_oh, out_bytes, cudaMemcpyDeviceToHost, st), "read back tallies");
         CUX(cudaStreamSynchronize(st), "transport kernel execution");
         if (trace && n_photons) CUX(cudaMemcpy(records, d_trace, sizeof(pdv_trace_record) * n_photons, cudaMemcpyDeviceToHost), "read back trace");
         float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, g_ws.e0, g_ws.e1) == cudaSuccess) g_last.ms = ms;
+        if (cudaEventElapsedTime(&ms, g_ev.e0, g_ev.e1) == cudaSuccess) g_last.ms = ms;
         g_last.pending = false;
-        std::memcpy(hist, th.data(), 8 * nb * n_units);
-        if (hist2) std::memcpy(hist2, th2.data(), 8 * nb * n_units);
-        if (stats) std::memcpy(stats, ts.data(), sizeof(pdv_run_stats) * n_units);
+        std::memcpy(hist, stage, 8 * nb * n_units);
+        if (hist2) std::memcpy(hist2, stage + (o_oh2 - o_oh), 8 * nb * n_units);
+        if (stats) std::memcpy(stats, stage + (o_os - o_oh), sizeof(pdv_run_stats) * n_units);
     } else if (trace) {
         CUX(cudaStreamSynchronize(st), "transport kernel execution");
         if (n_photons) CUX(cudaMemcpy(records, d_trace, sizeof(pdv_trace_record) * n_photons, cudaMemcpyDeviceToHost), "read back trace");
@@ -597,7 +679,8 @@ pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const do
     for (int i = 0; i < n_clouds; ++i) if (!clouds[i]) return fail(PDV_E_INVALID, "clouds[i] is NULL");
     for (int j = 0; j < n_snap; ++j) if (!(t_snap[j] > 0.0) || !std::isfinite(t_snap[j])) return fail(PDV_E_INVALID, "snapshot times must be > 0");
     if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
-    if (n_photons > (1ull << 62) || opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
+    if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
+    if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
     return run_impl(clouds, n_clouds, n_snap, nullptr, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
 }
 
@@ -637,9 +720,10 @@ pdv_status pdv_spectrogram(const double *hist, int32_t n_snap, int32_t n_bins, u
     }
     int device = 0;
     CU(cudaGetDevice(&device), "cudaGetDevice");
-    unsigned char *ws = nullptr;
-    pdv_status s = get_workspace(align16(8 * n) + 4 * n, device, &ws);
+    StreamScratch scratch;
+    pdv_status s = scratch_alloc(align16(8 * n) + 4 * n, device, st, scratch);
     if (s != PDV_OK) return s;
+    unsigned char *ws = scratch.p;
     double *dh = reinterpret_cast<double *>(ws);
     float *dout = reinterpret_cast<float *>(ws + align16(8 * n));
     std::vector<float> tmp(n);
@@ -680,9 +764,10 @@ pdv_status pdv_spectrum_peaks(const double *hist, int32_t n_units, int32_t n_bin
     CU(cudaGetDevice(&device), "cudaGetDevice");
     const size_t n = (size_t)n_units * n_bins;
     const size_t off_v = align16(8 * n), off_o = align16(off_v + 8 * (size_t)n_units);
-    unsigned char *ws = nullptr;
-    pdv_status s = get_workspace(off_o + sizeof(pdv_peak) * (size_t)n_units, device, &ws);
+    StreamScratch scratch;
+    pdv_status s = scratch_alloc(off_o + sizeof(pdv_peak) * (size_t)n_units, device, st, scratch);
     if (s != PDV_OK) return s;
+    unsigned char *ws = scratch.p;
     std::vector<pdv_peak> tmp(n_units);
     CU(cudaMemcpyAsync(ws, hist, 8 * n, cudaMemcpyHostToDevice, st), "copy hist");
     CU(cudaMemcpyAsync(ws + off_v, v_fs, 8 * (size_t)n_units, cudaMemcpyHostToDevice, st), "copy v_fs");
@@ -744,8 +829,9 @@ pdv_status pdv_phase_sampling_check(const pdv_cloud *cloud, int32_t class_index,
     if (!di.valid) return fail(PDV_E_CUDA, "cannot query the CUDA device");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t o_hist = align16(16 * (size_t)n_terms), o_sum = align16(o_hist + 16 * (size_t)n_bins), o_cnt = o_sum + 16;
-    unsigned char *ws = nullptr;
-    if ((s = get_workspace(o_cnt + 16, device, &ws)) != PDV_OK) return s;
+    StreamScratch scratch;
+    if ((s = scratch_alloc(o_cnt + 16, device, st, scratch)) != PDV_OK) return s;
+    unsigned char *ws = scratch.p;
     DevCloudHeader hd;
     std::memcpy(&hd, cloud->blob.data(), sizeof(hd));
     const float2 *phase = reinterpret_cast<const float2 *>(cloud->d_blob + hd.off_phase) + (size_t)class_index * hd.K;
@@ -788,9 +874,9 @@ pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mh
 }
 
 pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes) {
-    if (g_last.pending && g_ws.e0 && g_ws.e1) {      // output_on_device run: wait for its transport kernel only
+    if (g_last.pending && g_ev.e0 && g_ev.e1) {      // output_on_device run: wait for its transport kernel only
         float ms = 0.f;
-        if (cudaEventSynchronize(g_ws.e1) == cudaSuccess && cudaEventElapsedTime(&ms, g_ws.e0, g_ws.e1) == cudaSuccess)
+        if (cudaEventSynchronize(g_ev.e1) == cudaSuccess && cudaEventElapsedTime(&ms, g_ev.e0, g_ev.e1) == cudaSuccess)
             g_last.ms = ms;
         else
             cudaGetLastError();

@@ -52,9 +52,11 @@ enum StatSlot {
 // cell.  The host picks guide_shift so that no cell straddles two bin edges (then one probe is exact); if it cannot,
 // depth_bisect = 1 and the kernel bisects the rows instead.
 // Class guide (polydisperse clouds): the class of a class word cw is  c = #{j < n_classes-1 : thr[j] <= cw}  (cumulative
-// pick probabilities of Eq. 8, R12).  cguide[cw >> 24] holds that count for the first word of the cell in its low
-// 7 bits, and bit 7 is set if more than one threshold lies inside the cell; so  c = low7 + (thr[low7] <= cw)  settles every
-// cell but the flagged ones (tiny classes at the ends of the distribution), which walk on.
+// pick probabilities of Eq. 8, R12).  cguide[cw >> cguide_shift] holds that count for the first word of the cell in
+// its low 7 bits, and bit 7 is set if more than one threshold lies inside the cell; so  c = low7 + (thr[low7] <= cw)  settles
+// every cell but the flagged ones, which walk on.  The host takes the coarsest guide of 2^8 ... 2^12 cells in which no cell
+// holds two thresholds (config 3: 2^10); if even 2^12 cells leave flagged ones (config 5: the two smallest classes, hit with
+// probability 1.7e-6 and 2.7e-5) it stays at 2^12 and one flight in 4096 walks.
 struct DevCloudHeader {
     uint32_t blob_bytes;       // multiple of 16
     uint32_t n_classes, K, log2K, n_depth, n_guide;
@@ -67,16 +69,21 @@ struct DevCloudHeader {
     uint32_t R_thr;            // analog mode: reflected iff xi_absorb word < R_thr
     uint32_t surface_model;
     uint32_t frac_mask;        // the 12 bits of a phase word below its log2K index bits
-    uint32_t off_cguide;       // class guide: 256 bytes, see below
+    uint32_t off_cguide;       // class guide: 2^(32 - cguide_shift) bytes, see above
     float an_c0, an_c1, an_c2, an_c3;   // closed-form depth model (pdv_cloud_params.depth_model 1)
-    uint32_t pad[2];
+    uint32_t cguide_shift;     // 24 ... 20
+    uint32_t pad[1];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 
 struct UnitDesc {
     const unsigned char *cloud_blob;   // device pointer
     uint32_t stream;                   // Philox counter word 2 (unit index)
-    uint32_t visit;                    // entry k of the table: the unit a block works on k-th (see RunParams::n_lead)
+    uint32_t visit;                    // entry k of the table: the k-th unit of the visiting order (descending cost)
+    // Guided self-scheduling of the unit's photon ids: a warp claims 32 * clamp(remaining * chunk_per_remaining, 1, chunk)
+    // ids at a time; chunk_per_remaining = 1 / (2 * threads expected to work on the unit)
+    uint32_t chunk;
+    float chunk_per_remaining;
 };
 
 struct RunParams {
@@ -86,14 +93,13 @@ struct RunParams {
     unsigned long long *hist2;         // [n_units][n_bins] Q31 sum w^2
     unsigned long long *stats;         // [n_units][ST_COUNT]
     pdv_trace_record *trace;           // TRACE only: [n_photons]
+    const uint32_t *block_start;       // [grid] entry of the visiting order at which block b starts.  The units are laid on a
+                                       // line in descending cost, each as long as its estimated cost, and block b starts in the
+                                       // unit that holds point (b + 1/2) / grid of the line: a unit is staged by about as many
+                                       // blocks as its share of the work, each block stages few units, and a block that runs out
+                                       // of work walks on along the order (wrapping) and helps wherever photons are left
     uint32_t n_units;
-    uint32_t n_lead;                   // blocks visit the units in descending cost (units[k].visit), so that the long tails of
-                                       // the expensive ones overlap with other work; block b starts at entry b % n_lead, n_lead =
-                                       // number of leading units of equal cost (all of them when the units are alike)
     uint32_t n_bins;
-    uint32_t chunk;                    // photon ids a lane claims per fetch at the start of a unit (guided: shrinks
-    float chunk_per_remaining;         //   to clamp(remaining * chunk_per_remaining, chunk_min, chunk) as the unit drains)
-    uint32_t chunk_min;
     uint32_t max_events;               // roulette once n_scatter >= max_events; 0xffffffff: never
     uint32_t roulette_thr;             // survive iff the roulette word < roulette_thr
     float roulette_p;                  // play only while w <= p (then w / p <= 1)

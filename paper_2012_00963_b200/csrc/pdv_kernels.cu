@@ -96,7 +96,7 @@ struct CloudView {               // per-unit scalars and shared-memory table poi
     const float *albedo;
     const uint16_t *guide;
     const unsigned char *cguide;
-    uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, depth_bisect;
+    uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, depth_bisect, cg_shift;
     float tau_ext, R_f, one_minus_R;
     uint32_t R_thr, surface_model;
 };
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
     if (tid < 5) s_keys[tid] = make_uint4(P.key0[2 * tid], P.key1[2 * tid], P.key0[2 * tid + 1], P.key1[2 * tid + 1]);
 
     for (uint32_t visit = 0; visit < P.n_units; ++visit) {
-        const uint32_t u = P.units[(blockIdx.x % P.n_lead + visit) % P.n_units].visit;
+        const uint32_t u = P.units[(P.block_start[blockIdx.x] + visit) % P.n_units].visit;
         if (tid == 0) s_go = (*(volatile unsigned long long *)(P.next_id + u) < P.n_photons) ? 1 : 0;
         __syncthreads();
         const bool go = s_go != 0;
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cv.cguide = s_blob + h->off_cguide;
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
-            cv.depth_bisect = h->depth_bisect;
+            cv.depth_bisect = h->depth_bisect; cv.cg_shift = h->cguide_shift;
             cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
@@ -244,9 +244,11 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             if (DM == 2) closed = h->depth_bisect == 2u;
         }
         // ---- per-thread accumulators (flushed once per unit) ------------------------------------------------
-        // acc_lost = sum over finished histories of (1 - final weight) + roulette gains: all weight that went into
-        // particles or the surface; absorbed_particles = acc_lost - acc_abss.
-        unsigned long long acc_esc = 0ull, acc_lost = 0ull, acc_abss = 0ull;
+        // Weight that went into particles or the surface = sum over finished histories of (1 - final weight) + roulette gains.
+        // The final weights are tallied anyway (escaped: acc_esc; aperture hits, roulette kills, truncations: shared memory,
+        // and once more per thread in acc_rare), so that sum needs no per-history work of its own: at the flush
+        //   absorbed_particles = histories * 2^31 + acc_gain - acc_esc - acc_rare - acc_abss      (exact, in Q31).
+        unsigned long long acc_esc = 0ull, acc_rare = 0ull, acc_gain = 0ull, acc_abss = 0ull;
         // cnt_fl = flights that ended in an interaction (particle events + reflections), cnt_refl = reflections
         uint32_t cnt_hist = 0u, cnt_fl = 0u, cnt_refl = 0u, max_ev = 0u;
 
@@ -266,29 +268,35 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         if (lane == 0) *pool_next = 0u;
         __syncwarp();
 
-        // next photon of this lane: the next id of its private slice, else a new slice of `slice` ids from the warp pool
-        // (want = true if the pool is exhausted); resets the history state
-        auto take_photon = [&]() {
-            if (left) {
-                --left;
-                if (++id_lo == 0u) ++id_hi;
-            } else {
-                const uint32_t off = atomicAdd(pool_next, slice);
-                run = off < pool_len;
-                want = !run;
-                left = run ? min(slice, pool_len - off) - 1u : 0u;
-                id_lo = pool_lo + off;
-                id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
-            }
+        // a new slice of `slice` ids from the warp pool for this lane (want = true if the pool is exhausted): the rare half of
+        // "next photon"; the common half (next id of the lane's private slice) is inline in settle()
+        auto take_slice = [&]() {
+            const uint32_t off = atomicAdd(pool_next, slice);
+            run = off < pool_len;
+            want = !run;
+            left = run ? min(slice, pool_len - off) - 1u : 0u;
+            id_lo = pool_lo + off;
+            id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
+        };
+        auto reset_history = [&]() {
             T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u;
             if (NREFL) n_refl = 0u;
             if (DM == 2 && P.launch_model) mu = diffuse_launch_mu(id_lo, id_hi, ud.stream, s_keys);      // unit-uniform, general kernel only
         };
-        // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
-        auto finish = [&](int fate) {
+        // End of the histories of this pass (step (7)), for the whole warp at once: `fate` != F_NONE marks the lanes whose
+        // history ended.  The common case -- the photon left outside the aperture, or was absorbed -- is straight-line code
+        // under that predicate (selects and predicated adds: no divergent region, nothing to reconverge); only an aperture
+        // hit (Eq. 19 tally, ~2 % of the histories), a roulette kill, a truncation, a trace record and the claim of a new id
+        // slice branch.
+        auto settle = [&](int fate) {
+            const bool end = fate != F_NONE;
             const uint32_t wq = __float2uint_rn(w * kWOneF);
-            if (fate == F_EXIT) {
-                if (mu >= P.mu_aperture) {                    // inside the probe aperture: Eq. 19
+            const bool out = fate == F_EXIT;
+            bool rare = out && mu >= P.mu_aperture;
+            if (ROUL) rare = rare || fate == F_KILLED;
+            if (SSO) rare = rare || fate == F_TRUNC;
+            if (rare) {
+                if (out) {                                    // inside the probe aperture: Eq. 19
                     const float fb = (vt - P.v_lo) * P.inv_dv;
                     const uint32_t bin = (uint32_t)__float2int_rd(fb);       // floor; negative -> huge
                     if (bin < P.n_bins) {
@@ -299,28 +307,32 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                         smem_add64(&s_stats[fb < 0.f ? ST_UNDER : ST_OVER], wq);
                         fate = F_DET_OUT;
                     }
-                } else {
-                    acc_esc += wq;
+                } else if (ROUL && fate == F_KILLED) {
+                    smem_add64(&s_stats[ST_KILLED], wq);
+                } else if (SSO && fate == F_TRUNC) {
+                    smem_add64(&s_stats[ST_TRUNC], wq);
                 }
-            } else if (ROUL && fate == F_KILLED) {
-                smem_add64(&s_stats[ST_KILLED], wq);
-            } else if (SSO && fate == F_TRUNC) {
-                smem_add64(&s_stats[ST_TRUNC], wq);
+                acc_rare += wq;
             }
-            const uint32_t lost = kWOne - wq;
-            acc_lost += lost;
-            acc_abss += min(__float2uint_rn(abss * kWOneF), lost);
+            acc_esc += (out && !rare) ? wq : 0u;
+            acc_abss += end ? min(__float2uint_rn(abss * kWOneF), kWOne - wq) : 0u;
             const uint32_t n_int = nfl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);     // scatters + reflections
-            cnt_fl += nfl;                                    // an absorbing interaction is a particle event too
-            max_ev = max(max_ev, n_int);
-            if (TRACE) {
+            cnt_fl += end ? nfl : 0u;                         // an absorbing interaction is a particle event too
+            max_ev = max(max_ev, end ? n_int : 0u);
+            if (TRACE && end) {
                 const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
                 pdv_trace_record r;
                 r.vt = vt; r.weight = w; r.mu_exit = mu; r.fate = fate == F_ABS_PART ? F_ABS_SURF : fate;
                 r.n_scatter = (int)(n_int - n_refl); r.n_reflect = (int)n_refl;
                 P.trace[idx] = r;
             }
-            take_photon();
+            // the lane's next photon: the next id of its private slice, else (rare) a new slice from the warp pool
+            const bool next = end && left != 0u;
+            left -= next ? 1u : 0u;
+            id_lo += next ? 1u : 0u;
+            id_hi += (next && id_lo == 0u) ? 1u : 0u;
+            if (end && !next) take_slice();
+            if (end) reset_history();
         };
         // One flight (D2): `a` = path word, `cw` = class word (POLY), `b` = phase word, `pw` = azimuth / surface
         // polar-angle word, `ya` = absorption word (ANALOG), `sub` = which roulette word of the second block.
@@ -343,7 +355,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             uint32_t albt = albthr0;
             if (POLY) {
                 // c = #{j : thr[j] <= cw} through the class guide (pdv_device.h); thr is padded with 0xffffffff
-                const uint32_t e = cv.cguide[cw >> 24];
+                const uint32_t e = cv.cguide[cw >> cv.cg_shift];
                 c = e & 0x7Fu;
                 c += cv.thr[c] <= cw ? 1u : 0u;
                 if (e & 0x80u) c = class_walk(cv.thr, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
@@ -388,7 +400,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                                            : philox_roulette_word(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, s_keys, 2u + sub);
                 const RouletteOut o = roulette(w, abss, yr, P.roulette_thr, P.roulette_inv_p, s_stats);
                 if (o.killed) return F_KILLED;
-                w = o.w; abss = o.abss; acc_lost += o.add_lost; acc_abss += o.add_abss;
+                w = o.w; abss = o.abss; acc_gain += o.add_lost; acc_abss += o.add_abss;
             }
             return F_NONE;
         };
@@ -397,7 +409,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         for (;;) {
             if (refill) {
                 // ---- some lane found the warp pool empty: refill it from the unit's cursor (guided self-scheduling: a warp
-                // claims clamp(remaining / (2 warps), 32 chunk_min, 32 chunk) ids, sized from a fresh look at the cursor) and
+                // claims clamp(remaining / (2 warps), 32, 32 chunk) ids, sized from a fresh look at the cursor) and
                 // hand ids to the waiting lanes; lanes still waiting when the unit is drained are done
                 for (;;) {
                     unsigned long long b = 0ull;
@@ -405,8 +417,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     if (lane == 0) {
                         const unsigned long long seen = *(volatile unsigned long long *)(P.next_id + u);
                         if (seen < P.n_photons) {
-                            const uint32_t ask = 32u * min(max(__float2uint_rd(__ull2float_rd(P.n_photons - seen) * P.chunk_per_remaining),
-                                                               P.chunk_min), P.chunk);
+                            const uint32_t ask = 32u * min(max(__float2uint_rd(__ull2float_rd(P.n_photons - seen) * ud.chunk_per_remaining),
+                                                               1u), ud.chunk);
                             b = atomicAdd(P.next_id + u, (unsigned long long)ask);
                             if (b < P.n_photons) {
                                 const unsigned long long rem = P.n_photons - b;
@@ -422,7 +434,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     const unsigned long long id0 = P.first_id + __shfl_sync(FULL_MASK, b, 0);
                     pool_lo = (uint32_t)id0; pool_hi = (uint32_t)(id0 >> 32); pool_len = len;
                     slice = max(len >> 5, 1u);                    // a lane takes 1/32 of the pool at a time: 1 id from the last pools
-                    if (want) take_photon();
+                    if (want) { take_slice(); reset_history(); }
                     if (!__any_sync(FULL_MASK, want)) break;
                 }
                 if (!__any_sync(FULL_MASK, run)) break;
@@ -465,13 +477,14 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     }
                 }
             }
-            __syncwarp();                                     // histories that ended in either flight are finished in ONE pass
-            if (fate != F_NONE) finish(fate);                 // the one place where a lane moves on to its next photon
+            __syncwarp();                                     // histories that ended in any flight of the pass are settled together
+            settle(fate);                                     // the one place where a lane moves on to its next photon
             refill = __any_sync(FULL_MASK, want);             // only a finished history can leave a lane waiting for an id
         }
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
-        unsigned long long acc_absp = acc_lost - acc_abss;
+        // mod 2^64 per thread; the sum over a warp is the non-negative total (every history is claimed and settled in one warp)
+        unsigned long long acc_absp = ((unsigned long long)cnt_hist << 31) + acc_gain - acc_esc - acc_rare - acc_abss;
         uint32_t cnt_ev = cnt_fl - cnt_refl;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

@@ -349,6 +349,40 @@ def test_device_output_path_and_spectrogram(P):
     assert lin.shape == (3, nb) and lin.dtype == np.float32
 
 
+def test_two_device_output_runs_on_two_streams_are_independent(P):
+    """Two output_on_device = 1 runs with different n_bins enqueued back to back on two streams from one host thread (the
+    second needs the larger scratch): each must equal its host-buffer twin bit for bit.  The device scratch of a call is
+    stream-ordered (include/pdv.h, "Streams"), so neither run can zero, reuse or free what the other is using."""
+    import torch
+    cfg = W.scaled(W.config(1), 3_000_000)
+    c = P.pdv_cloud_create(cfg["clouds"][0])
+    n = cfg["run"]["n_photons"]
+    runs = [dict(cfg["run"], n_bins=256), dict(cfg["run"], n_bins=8192, v_lo=500.0, v_hi=5500.0)]
+    seeds = [101, 202]
+    twins = [P.pdv_mc_run([c], cfg["t_snap"], n, sd, r) for sd, r in zip(seeds, runs)]
+    for rep in range(3):
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        outs = [(torch.zeros((1, 1, r["n_bins"]), dtype=torch.float64, device="cuda"),
+                 torch.zeros((1, 1, r["n_bins"]), dtype=torch.float64, device="cuda"),
+                 torch.zeros(P.STATS_DTYPE.itemsize, dtype=torch.uint8, device="cuda")) for r in runs]
+        torch.cuda.synchronize()
+        for sd, r, st, (h, h2, stt) in zip(seeds, runs, streams, outs):       # back to back: both kernels are in flight together
+            P.pdv_mc_run_device([c], cfg["t_snap"], n, sd, r, h, h2, stt, stream=st.cuda_stream)
+        torch.cuda.synchronize()
+        for (h, h2, stt), tw in zip(outs, twins):
+            assert np.array_equal(h.cpu().numpy(), tw.hist) and np.array_equal(h2.cpu().numpy(), tw.hist2)
+            ds = np.frombuffer(stt.cpu().numpy().tobytes(), dtype=P.STATS_DTYPE)
+            for k in ds.dtype.names:
+                assert np.array_equal(ds[k], tw.stats[0][k]), k
+
+
+def test_photon_count_limit_of_the_fixed_point_tallies(P):
+    cfg = W.config(1)
+    c = P.pdv_cloud_create(cfg["clouds"][0])
+    with pytest.raises(P.PdvError):
+        P.pdv_mc_run([c], cfg["t_snap"], 2 ** 33 + 1, 1, cfg["run"])
+
+
 def test_full_size_config2_in_bench_launch_configuration(P):
     """BASELINE.json configs[1] at full size (1e8 photons, default launch shape = what bench.py times): invariants
     that hold at any size, plus parity against an oracle run the CPU can afford (4e7 histories)."""
