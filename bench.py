@@ -1,24 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Monte-Carlo PDV hot path on B200 (contract: see DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl b200|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--scaling weak|strong] [--impl b200|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
         bench.py --gpus N --steps K --warmup W
 
-A "step" is one pass of the whole hot path over one batch of synthetic input: one
-pdv_mc_run of BASELINE.json configs[I] (default I = 1: 2 mg/cm^2 tin cloud, 1e8 photons, 512 bins, t = 3 us)
-followed by pdv_spectrogram.  Every step uses a new seed.  Rank 0 prints ONE JSON line.
+A "step" is one pass of the whole hot path over one batch of synthetic input: one pdv_mc_run of
+BASELINE.json configs[I] (default I = 1: 2 mg/cm^2 tin cloud, 1e8 photons, 512 bins, t = 3 us) followed by pdv_spectrogram
+(and pdv_spectrum_peaks for the sweep workload).  Every step uses a new seed.  Rank 0 prints ONE JSON line.
 
-  value      scattering events/s (particle interactions, BASELINE.json "metric"), whole job, cloud tables resident in
-             HBM and outputs left in HBM, timed with CUDA events on the launching stream (max over ranks)
-  e2e        the same metric through the host-buffer C-ABI calls a user makes: pdv_cloud_create (host Mie tables + H2D)
-             + pdv_mc_run into host arrays (D2H inside) + pdv_spectrogram on host arrays, wall clock
+  value      scattering events/s (particle interactions, BASELINE.json "metric"), whole job, cloud tables resident in HBM and
+             outputs left in HBM, timed with CUDA events on the launching stream (max over ranks)
+  e2e        the same metric through the host-buffer C-ABI calls a user makes: pdv_cloud_create (host Mie tables + H2D) +
+             pdv_mc_run into host arrays (D2H inside) + pdv_spectrogram on host arrays, wall clock
   roofline   transport kernel against the instruction-issue peak (bound "alu": no HBM traffic, no contraction)
   cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores, bounded sample of the same workload
+  configs    (N = 1, default run) the other BASELINE.json configs and the row-f1 sweep at full size, 2 timed steps each, each
+             with ms_per_step, events/s, roofline and clocks -- so that every config is measured by whoever runs this file
 
 --impl reference times the oracle itself (there is no reference code).
-N > 1: weak scaling, rank r runs the same number of histories on photon ids [r n, (r+1) n); one all-reduce of the
-tallies per step.
+N > 1 (paper_2012_00963_b200/_shard.py::plan): --scaling weak (default): rank r runs the same number of histories per unit on
+photon ids [r n, (r+1) n); --scaling strong: the job is fixed, one-unit configs split the id range, multi-unit configs give
+whole units to ranks.  Either way the only exchange is one reduction of the tallies per step.
 """
 from __future__ import annotations
 
@@ -39,13 +42,13 @@ import pdv_workloads as W  # noqa: E402
 
 METRIC = "scattering events/s"
 UNIT = "events/s"
-N_SM_B200 = 148
 
 # Algorithmic thread-instructions of ONE flight (one Philox block + free flight + interaction / reflection / exit) on the
 # common path, counted from the method's operations, not from what the compiler emitted (DESIGN.md "Roofline",
 # table "algorithmic instructions per flight").  A particle event, a surface reflection and the final exit flight are
 # one flight each.
 ALG_INST_PER_FLIGHT = {"scatter": 96, "reflect": 70, "exit": 64}
+COUNTERS_FILE = os.path.join(ROOT, "profiles", "r2_transport_counters.txt")
 
 
 def _env_int(name, default):
@@ -63,9 +66,8 @@ class ClockSampler:
                0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
 
     def __init__(self, index: int, uuid: str | None = None):
-        self.samples, self.reason_bits, self.power = [], 0, []
         self.max_mhz = None
-        self._stop = threading.Event()
+        self.reset()
         self._thr = None
         try:
             import pynvml
@@ -79,6 +81,10 @@ class ClockSampler:
         except Exception:
             self._nv = None
 
+    def reset(self):
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self._stop = threading.Event()
+
     def _loop(self):
         nv = self._nv
         while not self._stop.is_set():
@@ -91,6 +97,7 @@ class ClockSampler:
             self._stop.wait(0.005)
 
     def __enter__(self):
+        self._stop.clear()
         if self._nv is not None:
             self._thr = threading.Thread(target=self._loop, daemon=True)
             self._thr.start()
@@ -100,6 +107,7 @@ class ClockSampler:
         self._stop.set()
         if self._thr is not None:
             self._thr.join()
+            self._thr = None
 
     def summary(self) -> dict:
         if not self.samples:
@@ -157,7 +165,7 @@ def run_reference(args):
     sample = f"unit 0 of {cfg['name']}: {n} histories per step (of {cfg['run']['n_photons']}), {args.steps} steps"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": args.scaling,
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "histories_per_step": n, "n_bins": cfg["run"]["n_bins"]},
         "histories_per_s": n * args.steps / dt,
@@ -167,99 +175,95 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------------- GPU arm
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1,
-                    help="BASELINE.json configs index (default 1 = headline); 5 = the paper's Figs. 13-15 sweep (SURVEY.md 8(f) row "
-                         "f1: 14 clouds x 1e7 photons in one launch, then pdv_spectrum_peaks on the device)")
-    ap.add_argument("--photons", type=int, default=0, help="override histories per unit (debugging; invalidates the number)")
-    ap.add_argument("--depth-model", type=int, default=0, choices=[0, 1],
-                    help="0: depth table (the headline design); 1: closed-form v(T), exponential profiles only (variant f2)")
-    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--ref-photons", type=int, default=2_000_000, help="--impl reference: histories per step")
-    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work of the cpu_baseline leg (0: skip)")
-    ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-buffer leg (0: same as --steps)")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        run_reference(args)
-        return
-    args.warmup = max(args.warmup, 3)
+def _captured_counters(workload: str, histories_per_launch: int):
+    """Counters of one transport-kernel launch of this workload from the committed ncu capture (written by
+    `python -m paper_2012_00963_b200.ncu_counters`), or None when there is none for the kernel sources as they are now."""
+    from paper_2012_00963_b200.build import kernel_source_hash
+    if not os.path.exists(COUNTERS_FILE):
+        return None
+    want = kernel_source_hash()
+    found = None
+    with open(COUNTERS_FILE) as f:
+        for line in f:
+            line = line.strip()
+            if not line.startswith("{"):
+                continue
+            rec = json.loads(line)
+            if rec.get("workload") == workload and rec.get("histories_per_launch") == histories_per_launch \
+                    and rec.get("kernel_source_sha256") == want:
+                found = rec
+    return found
 
-    import torch
-    import torch.distributed as dist
 
-    import paper_2012_00963_b200 as P
-    from paper_2012_00963_b200._shard import allreduce_tallies
-
-    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, world, local, clk, want_peaks=None):
+    """Times `steps` steps of workload `cfg` on this rank's GPU (device-resident leg and host-buffer leg); returns the
+    measurements reduced over ranks (times: max; counts: sum)."""
+    from paper_2012_00963_b200 import _shard
     dev = torch.device("cuda", local)
-
-    cfg = _workload(args.config)
     if args.depth_model:
-        cfg["clouds"] = [dict(c, depth_model=args.depth_model) for c in cfg["clouds"]]
+        cfg = dict(cfg, clouds=[dict(c, depth_model=args.depth_model) for c in cfg["clouds"]])
     run = dict(cfg["run"])
-    n = int(args.photons or run["n_photons"])
-    run["first_photon_id"] = rank * n                       # weak scaling: disjoint id ranges, same count per rank
-    nb, t_snap = run["n_bins"], cfg["t_snap"]
-    clouds = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
+    n_job = int(args.photons or run["n_photons"])                      # histories per unit of the job (per rank when weak)
+    nb, t_all_snaps = run["n_bins"], cfg["t_snap"]
+    nc_job, ns_job = len(cfg["clouds"]), len(t_all_snaps)
+    plan = _shard.plan(nc_job, ns_job, n_job, rank, world, args.scaling)
+    n = plan["n_photons"]
+    run["first_photon_id"] = plan["first_photon_id"]
+    if world > 1 and args.scaling == "strong":
+        run["unit_streams"] = plan["unit_ids"]
+    params = [cfg["clouds"][i] for i in plan["clouds"]]
+    t_snap = [t_all_snaps[j] for j in plan["snaps"]]
+    clouds = [P.pdv_cloud_create(c) for c in params]
     nc, ns = len(clouds), len(t_snap)
-    n_units = nc * ns
-    hist = torch.zeros((nc, ns, nb), dtype=torch.float64, device=dev)
+    n_units, n_units_job = nc * ns, nc_job * ns_job
+    photons_job = n_job * (world if args.scaling == "weak" else 1)     # histories per unit of the whole job
+    hist = torch.zeros((max(nc, 1), max(ns, 1), nb), dtype=torch.float64, device=dev)
     hist2 = torch.zeros_like(hist)
-    stats = torch.zeros(n_units * P.STATS_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    stats = torch.zeros(max(n_units, 1) * P.STATS_DTYPE.itemsize, dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
     stream = torch.cuda.current_stream()
-    v_fs_dev = None
-    if "points" in cfg:                                      # sweep + interpretation workload: one v_fs per spectrum
-        v_fs_dev = torch.tensor([c["v_fs"] for c in cfg["clouds"] for _ in t_snap], dtype=torch.float64, device=dev)
+    sweep = "points" in cfg                                   # sweep + interpretation workload: one v_fs per spectrum
+    v_fs_job = torch.tensor([c["v_fs"] for c in cfg["clouds"] for _ in t_all_snaps], dtype=torch.float64, device=dev) if sweep else None
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
+    def read_stats():
+        return np.frombuffer(stats.cpu().numpy().tobytes(), dtype=P.STATS_DTYPE)[:n_units]
+
     def step(i):
-        P.pdv_mc_run_device(clouds, t_snap, n, run["seed"] + 7919 * i, run, hist, hist2, stats, stream=stream.cuda_stream)
-        if world > 1:
-            allreduce_tallies(hist, hist2)
-        sp = P.pdv_spectrogram(hist.view(n_units, nb), n * world, run["v_lo"], run["v_hi"], scale=2,
-                               stream=stream.cuda_stream)
-        if v_fs_dev is not None:                             # row f1: peak position / value / curvature of every spectrum
-            return P.pdv_spectrum_peaks(hist.view(n_units, nb), n * world, run["v_lo"], run["v_hi"], v_fs_dev, half=6, n_pass=2,
-                                        fit_half=16, x_min=1.03, stream=stream.cuda_stream)
+        if n_units:
+            P.pdv_mc_run_device(clouds, t_snap, n, run["seed"] + 7919 * i, run, hist, hist2, stats, stream=stream.cuda_stream)
+        if world > 1:                                        # the one exchange: tallies of the whole job on every rank
+            h, _, _ = _shard.reduce_job(hist.view(-1, nb)[:n_units], hist2.view(-1, nb)[:n_units], read_stats(), plan["unit_ids"], n_units_job)
+        else:
+            h = hist.view(n_units, nb)
+        sp = P.pdv_spectrogram(h, photons_job, run["v_lo"], run["v_hi"], scale=2, stream=stream.cuda_stream)
+        if sweep:                                            # row f1: peak position / value / curvature of every spectrum
+            return P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"], v_fs_job, half=6, n_pass=2, fit_half=16,
+                                        x_min=1.03, stream=stream.cuda_stream)
         return sp
 
-    def read_stats():
-        return np.frombuffer(stats.cpu().numpy().tobytes(), dtype=P.STATS_DTYPE)
-
-    for i in range(args.warmup):
+    for i in range(warmup):
         flush.zero_()
         step(i)
     barrier()
 
-    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
     tot = dict(particle_events=0, surface_reflections=0, histories=0)
     transport_ms = []
-    # sampled during the device-timed steps and the end-to-end steps (both keep the GPU under the same load)
-    clk = ClockSampler(local, str(getattr(torch.cuda.get_device_properties(local), "uuid", "")))
-    with clk:
+    clk.reset()
+    with clk:                                                # sampled during the device-timed steps and the end-to-end steps
         barrier()
-        for i in range(args.steps):
+        for i in range(steps):
             flush.zero_()                                    # L2 flush between timed iterations (outside the events)
             ev0[i].record(stream)
-            step(args.warmup + i)
+            step(warmup + i)
             ev1[i].record(stream)
-            transport_ms.append(P.pdv_last_launch_info()["transport_ms"])      # waits for this step's kernel
+            transport_ms.append(P.pdv_last_launch_info()["transport_ms"] if n_units else 0.0)      # waits for this step's kernel
             s = read_stats()
             for k in tot:
                 tot[k] += int(s[k].sum())
@@ -273,47 +277,55 @@ def main():
         dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
     step_ms, tr_ms = (float(x) for x in t_all.cpu())
     events, reflections, histories = (float(x) for x in cnt.cpu())
-    value = events / (step_ms * 1e-3)
 
     # ---- end to end through the host-buffer API (every step: host Mie tables + H2D, run, D2H, spectrogram) -------------
-    k_e2e = args.e2e_steps or args.steps
     e2e_events = 0
 
     def e2e_step(i):
-        cl = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
-        r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run)
-        sp = P.pdv_spectrogram(r.hist.reshape(n_units, nb), n, run["v_lo"], run["v_hi"], scale=2)
-        if v_fs_dev is not None:
-            sp = P.pdv_spectrum_peaks(r.hist.reshape(n_units, nb), n, run["v_lo"], run["v_hi"],
-                                      [c["v_fs"] for c in cfg["clouds"] for _ in t_snap], half=6, n_pass=2, fit_half=16, x_min=1.03)
+        cl = [P.pdv_cloud_create(c) for c in params]
+        r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run) if n_units else None
+        ev = int(r.stats["particle_events"].sum()) if r is not None else 0
+        if world > 1:
+            import torch as _t
+            h, _, _ = _shard.reduce_job(_t.from_numpy(r.hist.reshape(-1, nb)).to(dev), _t.from_numpy(r.hist2.reshape(-1, nb)).to(dev),
+                                        r.stats.reshape(-1), plan["unit_ids"], n_units_job)
+            h = h.cpu().numpy()
+        else:
+            h = r.hist.reshape(n_units, nb)
+        sp = P.pdv_spectrogram(h, photons_job, run["v_lo"], run["v_hi"], scale=2)
+        if sweep:
+            sp = P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"],
+                                      [c["v_fs"] for c in cfg["clouds"] for _ in t_all_snaps], half=6, n_pass=2, fit_half=16, x_min=1.03)
         for c in cl:
             c.destroy()
-        return int(r.stats["particle_events"].sum()), sp
+        return ev, sp
 
-    for i in range(2):
+    for i in range(2 if e2e_steps else 0):
         e2e_step(-1 - i)
     barrier()
-    clk._stop.clear()
-    with clk:
-        t0 = time.perf_counter()
-        for i in range(k_e2e):
-            e2e_events += e2e_step(i)[0]
-        torch.cuda.synchronize()
-        e2e_s = time.perf_counter() - t0
+    e2e_s = 0.0
+    if e2e_steps:
+        with clk:
+            t0 = time.perf_counter()
+            for i in range(e2e_steps):
+                e2e_events += e2e_step(i)[0]
+            torch.cuda.synchronize()
+            e2e_s = time.perf_counter() - t0
     e2e_t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
     e2e_c = torch.tensor([float(e2e_events)], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
         dist.all_reduce(e2e_c, op=dist.ReduceOp.SUM)
-    blob_bytes = info["smem_bytes"] - 16 * nb                                   # largest cloud image staged per block
-    h2d = nc * blob_bytes + 16 * n_units + 8 * n_units * nb                     # tables + unit table + hist (spectrogram)
-    d2h = 2 * 8 * n_units * nb + n_units * P.STATS_DTYPE.itemsize + 4 * n_units * nb
+    blob_bytes = max(info["smem_bytes"] - 16 * nb, 0)                           # largest cloud image staged per block
+    h2d = nc * blob_bytes + 24 * n_units + 4 * info["grid"] + 8 * n_units_job * nb   # tables + unit table + block starts + hist (spectrogram)
+    d2h = 2 * 8 * n_units * nb + n_units * P.STATS_DTYPE.itemsize + 4 * n_units_job * nb
+    for c in clouds:
+        c.destroy()
 
-    # ---- roofline of the transport kernel: instruction issue ---------------------------------------------------------
-    peaks = P.pdv_issue_peaks(30.0) if rank == 0 else None
     out = None
     if rank == 0:
         clocks = clk.summary()
+        peaks = want_peaks
         sm_max = clocks["sm_max_mhz"] or 1965.0
         n_sm = peaks["n_sm"]
         issue_peak = n_sm * 4 * 32 * sm_max * 1e6                               # 1 warp-instruction / clk / sub-partition
@@ -323,50 +335,119 @@ def main():
         if any(len(c.get("diameters", [])) > 1 or "lognormal" in c for c in cfg["clouds"]):
             a["scatter"] += 6                        # polydisperse: class pick (guide byte, threshold, compare, clamp) + per-class albedo and table base
         alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
-        achieved = alg / (tr_ms * 1e-3)
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "transport_thread_inst.txt")     # written by hand from the ncu capture
-        if os.path.exists(tpath):
-            with open(tpath) as f:
-                tj = json.load(f)
-            if tj.get("workload") == cfg["name"] and tj.get("histories_per_launch") == n:
-                traffic = tj.get("thread_inst_executed_per_launch")
+        tr_s = max(tr_ms, 1e-9) * 1e-3
+        achieved = alg / tr_s
+        cap = _captured_counters(cfg["name"], n * n_units) if world == 1 else None
+        roof = {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12, "unit": "Tthread-inst/s",
+                "frac": achieved / issue_peak,
+                "traffic": (cap["dram_bytes_read"] + cap["dram_bytes_write"]) if cap else None,
+                "traffic_is": "dram bytes of one launch (ncu capture of the same workload and kernel sources)" if cap else
+                              "no ncu capture of this workload for the kernel sources as they are",
+                "executed_thread_inst_per_launch": cap["thread_inst_executed"] if cap else None,
+                "frac_executed": (cap["thread_inst_executed"] / (tr_s / steps) / issue_peak) if cap else None,
+                "peak_is": f"{n_sm} SMs x 4 sub-partitions x 32 lanes x {sm_max:.0f} MHz (DESIGN.md), not in MEASURED_PEAKS.json",
+                "kernel": "pdv::transport_kernel", "alg_inst_per_flight": a,
+                "measured_ffma_Tinst_s": peaks["ffma_thread_inst_per_s"] / 1e12,
+                "measured_mufu_Tinst_s": peaks["mufu_thread_inst_per_s"] / 1e12,
+                "frac_of_measured_ffma": achieved / peaks["ffma_thread_inst_per_s"],
+                "sm_clock_mhz_in_microbench": peaks["sm_clock_mhz"]}
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units, "depth_model": args.depth_model,
-                       "n_bins": nb, "parallelism": f"photon-id ranges x{world}", "l2": "flushed between steps (256 MiB write)",
-                       "events_per_history": events / histories, "reflections_per_history": reflections / histories},
+            "value": events / (step_ms * 1e-3), "ms_per_step": step_ms / steps, "steps": steps, "warmup": warmup,
+            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units_job, "depth_model": args.depth_model,
+                       "n_bins": nb, "parallelism": f"{args.scaling}: " + ("photon-id ranges" if args.scaling == "weak" or n_units_job == 1 else "whole units") + f" x{world}",
+                       "l2": "flushed between steps (256 MiB write)",
+                       "events_per_history": events / max(histories, 1), "reflections_per_history": reflections / max(histories, 1)},
             "histories_per_s": histories / (step_ms * 1e-3),
             "events_incl_surface_per_s": (events + reflections) / (step_ms * 1e-3),
-            "gpu_launches": (4 if v_fs_dev is not None else 3) * args.steps,    # transport + finalize + spectrogram (+ peak) kernels per step
+            "gpu_launches": (4 if sweep else 3) * steps,    # transport + finalize + spectrogram (+ peak) kernels per step
             "launch": {"grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
-                       "transport_ms_per_step": tr_ms / args.steps},
+                       "transport_ms_per_step": tr_ms / steps},
             "clocks": clocks,
-            "e2e": {"value": float(e2e_c) / float(e2e_t), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h, "steps": k_e2e, "ms_per_step": 1e3 * float(e2e_t) / k_e2e,
+            "e2e": {"value": (float(e2e_c) / float(e2e_t)) if e2e_steps else None, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": (1e3 * float(e2e_t) / e2e_steps) if e2e_steps else None,
                     "includes": "pdv_cloud_create (host Mie + tables + H2D), pdv_mc_run (host outputs), pdv_spectrogram"},
-            "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12, "unit": "Tthread-inst/s",
-                         "frac": achieved / issue_peak, "traffic": traffic,
-                         "frac_executed": (traffic / (tr_ms / args.steps * 1e-3) / issue_peak) if traffic else None,
-                         "peak_is": f"{n_sm} SMs x 4 sub-partitions x 32 lanes x {sm_max:.0f} MHz (DESIGN.md), not in MEASURED_PEAKS.json",
-                         "kernel": "pdv::transport_kernel",
-                         "alg_inst_per_flight": a,
-                         "measured_ffma_Tinst_s": peaks["ffma_thread_inst_per_s"] / 1e12,
-                         "measured_mufu_Tinst_s": peaks["mufu_thread_inst_per_s"] / 1e12,
-                         "frac_of_measured_ffma": achieved / peaks["ffma_thread_inst_per_s"],
-                         "sm_clock_mhz_in_microbench": peaks["sm_clock_mhz"]},
+            "roofline": roof,
         }
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1,
+                    help="BASELINE.json configs index (default 1 = headline); 5 = the paper's Figs. 13-15 sweep (SURVEY.md 8(f) row "
+                         "f1: 14 clouds x 1e7 photons in one launch, then pdv_spectrum_peaks on the device)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: how the job is shared (see the module docstring)")
+    ap.add_argument("--photons", type=int, default=0, help="override histories per unit (debugging; invalidates the number)")
+    ap.add_argument("--depth-model", type=int, default=0, choices=[0, 1],
+                    help="0: depth table (the headline design); 1: closed-form v(T), exponential profiles only (variant f2)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--ref-photons", type=int, default=2_000_000, help="--impl reference: histories per step")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work of the cpu_baseline leg (0: skip)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-buffer leg (0: same as --steps)")
+    ap.add_argument("--other-configs", type=int, default=-1,
+                    help="1: append the 'configs' array (the other workloads at full size, 2 timed steps each); 0: skip; "
+                         "default: 1 for the plain default run on one GPU (no --config), else 0")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2012_00963_b200 as P
+
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    clk = ClockSampler(local, str(getattr(torch.cuda.get_device_properties(local), "uuid", "")))
+    peaks = P.pdv_issue_peaks(30.0) if rank == 0 else None
+
+    cfg = _workload(args.config)
+    main_out = time_workload(P, torch, dist, cfg, args, steps=args.steps, warmup=args.warmup, e2e_steps=args.e2e_steps or args.steps,
+                             rank=rank, world=world, local=local, clk=clk, want_peaks=peaks)
+    others = []
+    do_others = args.other_configs == 1 or (args.other_configs < 0 and world == 1 and args.config == 1 and not args.depth_model)
+    if do_others:
+        for idx in (0, 2, 3, 4, 5):
+            if idx == args.config:
+                continue
+            o = time_workload(P, torch, dist, _workload(idx), args, steps=2, warmup=3, e2e_steps=1, rank=rank, world=world, local=local,
+                              clk=clk, want_peaks=peaks)
+            if o is not None:
+                others.append({"workload": o["config"]["workload"], "config_index": idx, "value": o["value"], "unit": UNIT,
+                               "ms_per_step": o["ms_per_step"], "steps": o["steps"], "warmup": o["warmup"],
+                               "histories_per_s": o["histories_per_s"], "transport_ms_per_step": o["launch"]["transport_ms_per_step"],
+                               "launch": o["launch"], "config": o["config"], "gpu_launches": o["gpu_launches"],
+                               "e2e": {"value": o["e2e"]["value"], "ms_per_step": o["e2e"]["ms_per_step"]},
+                               "roofline": {k: o["roofline"][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic",
+                                                                          "executed_thread_inst_per_launch", "frac_executed")},
+                               "clocks": o["clocks"]})
+    if rank == 0:
+        out = {"metric": METRIC, "value": main_out["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+               "ms_per_step": main_out["ms_per_step"], "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
+               "dtype": "f32", "data": "synthetic"}
+        out.update({k: main_out[k] for k in ("config", "histories_per_s", "events_incl_surface_per_s", "gpu_launches", "launch", "clocks",
+                                             "e2e", "roofline")})
         if args.cpu_seconds > 0:
             o = oracle_timed(cfg, args.cpu_seconds, seed=97)
             out["cpu_baseline"] = {"value": o["events"] / o["seconds"], "unit": UNIT, "cores": o["cores"], "kind": "oracle",
                                    "histories_per_s": o["n"] / o["seconds"],
                                    "sample": f"unit 0 of {cfg['name']}: {o['n']} histories in {o['seconds']:.1f} s"}
+        if others:
+            out["configs"] = others
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
-    if out is not None:
+    if rank == 0:
         print(json.dumps(out))
 
 

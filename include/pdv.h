@@ -133,6 +133,10 @@ typedef struct {
                                        the history's Philox block with counter word 3 = 0xffffffff.  Not in the paper: it makes
                                        the mean-path invariance of a non-absorbing medium (<events> = 4 tau_ext, pin P16)
                                        testable on the device without any reference implementation */
+    const uint32_t *unit_streams; /* HOST [n_clouds][n_snap] or NULL.  Random sub-stream (Philox counter word 2) of each unit; NULL:
+                                    the unit index u = i_cloud * n_snap + i_snap.  A process that runs a SUBSET of the units of a
+                                    larger job (whole units per GPU) passes the units' indices in the whole job
+                                    here, so that its spectra are bit-identical to the rows of the one-process run */
 } pdv_run_opts;
 
 #define PDV_MAX_BINS 8192

@@ -51,7 +51,8 @@ class RunOpts(C.Structure):
                 ("aperture_sr", C.c_double), ("mode", C.c_int32), ("max_events", C.c_int32),
                 ("roulette_survival", C.c_double), ("single_scatter_only", C.c_int32),
                 ("first_photon_id", C.c_uint64), ("output_on_device", C.c_int32), ("blocks_per_sm", C.c_int32),
-                ("threads_per_block", C.c_int32), ("launch_model", C.c_int32)]
+                ("threads_per_block", C.c_int32), ("launch_model", C.c_int32),
+                ("unit_streams", C.POINTER(C.c_uint32))]
 
 
 STAT_FLOATS = ("detected", "underflow", "overflow", "escaped", "absorbed_particles", "absorbed_surface",
@@ -217,6 +218,11 @@ def _opts(run: dict, output_on_device: bool = False) -> RunOpts:
     o.output_on_device = int(output_on_device)
     o.blocks_per_sm, o.threads_per_block = int(run.get("blocks_per_sm", 0)), int(run.get("threads_per_block", 0))
     o.launch_model = int(run.get("launch_model", 0))
+    us = run.get("unit_streams")
+    if us is not None:                 # [n_clouds * n_snap] sub-stream index of each unit (units of a larger job)
+        arr = np.ascontiguousarray(us, dtype=np.uint32)
+        o._keep_unit_streams = arr     # keeps the buffer alive as long as the options struct
+        o.unit_streams = arr.ctypes.data_as(C.POINTER(C.c_uint32))
     return o
 
 

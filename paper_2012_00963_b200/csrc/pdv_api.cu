@@ -681,7 +681,7 @@ pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const do
     if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
     if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
     if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
-    return run_impl(clouds, n_clouds, n_snap, nullptr, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
+    return run_impl(clouds, n_clouds, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
 }
 
 pdv_status pdv_mc_trace(const pdv_cloud *cloud, uint32_t unit, uint64_t n_photons, uint64_t seed,

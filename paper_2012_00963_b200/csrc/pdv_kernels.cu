@@ -39,6 +39,11 @@ namespace pdv {
 
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
 
+// Block-wide state that the out-of-line rare paths touch as well: at file scope, so that they address it as shared memory
+// (a pointer parameter would make it a generic address: window-base arithmetic at every call site, generic loads inside).
+__shared__ __align__(16) uint4 s_keys[5];                 // Philox round keys, two rounds per uint4
+__shared__ unsigned long long s_stats[ST_COUNT];          // per-unit statistics of the block (transport_kernel)
+
 // Philox4x32-10 block function.  The 10 round keys (k0_r, k1_r) are precomputed on the host and staged in shared memory,
 // two rounds per uint4: five broadcast LDS.128 per block instead of ten constant-bank loads (the ADU pipe that serves
 // LDC was a third busy with the keys alone).
@@ -133,9 +138,9 @@ __device__ __noinline__ uint32_t class_walk(const uint32_t *thr, uint32_t c, uin
 
 // diffuse illumination of the cloud top (pdv_run_opts.launch_model 1): mu = -sqrt(xi), xi from word 0 of the block with
 // counter word 3 = 0xffffffff, which no flight ever reaches
-__device__ __noinline__ float diffuse_launch_mu(uint32_t id_lo, uint32_t id_hi, uint32_t stream, const uint4 *keys) {
+__device__ __noinline__ float diffuse_launch_mu(uint32_t id_lo, uint32_t id_hi, uint32_t stream) {
     uint32_t x0, x1, x2, x3;
-    philox4x32_10(id_lo, id_hi, stream, 0xFFFFFFFFu, keys, x0, x1, x2, x3);
+    philox4x32_10(id_lo, id_hi, stream, 0xFFFFFFFFu, s_keys, x0, x1, x2, x3);
     return -fast_sqrt((__uint2float_rn(x0 >> 8) + 0.5f) * 5.9604644775390625e-8f);
 }
 
@@ -146,7 +151,7 @@ __device__ __noinline__ float lambert_mu(float pwf) { return fast_sqrt(pwf * 2.3
 // that w / p <= 1.  `yr` is the roulette word of the flight's second Philox block.  Everything by value: a reference
 // parameter would pin the caller's weight registers to local memory.
 struct RouletteOut { float w, abss; uint32_t add_lost, add_abss, killed; };
-__device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, uint32_t thr, float inv_p, unsigned long long *s_stats) {
+__device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, uint32_t thr, float inv_p) {
     RouletteOut o;
     o.w = w; o.abss = abss; o.add_lost = 0u; o.add_abss = 0u; o.killed = yr >= thr ? 1u : 0u;
     if (o.killed) return o;
@@ -164,10 +169,9 @@ __device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, u
 
 // roulette word of a flight for the implicit-capture kernels, which do not draw the companion blocks: word `word` of the
 // block with counter word 3 = ctr3 (D1/D2), out of line
-__device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t ctr3, const uint4 *keys,
-                                                      uint32_t word) {
+__device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t ctr3, uint32_t word) {
     uint32_t y0, y1, y2, y3;
-    philox4x32_10(id_lo, id_hi, stream, ctr3, keys, y0, y1, y2, y3);
+    philox4x32_10(id_lo, id_hi, stream, ctr3, s_keys, y0, y1, y2, y3);
     return word == 0u ? y0 : word == 1u ? y1 : word == 2u ? y2 : y3;
 }
 
@@ -179,8 +183,6 @@ template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
 __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ unsigned long long s_stats[ST_COUNT];
-    __shared__ __align__(16) uint4 s_keys[5];
     __shared__ uint32_t s_pool_next[32];
     __shared__ int s_go;
 
@@ -268,35 +270,29 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         if (lane == 0) *pool_next = 0u;
         __syncwarp();
 
-        // a new slice of `slice` ids from the warp pool for this lane (want = true if the pool is exhausted): the rare half of
-        // "next photon"; the common half (next id of the lane's private slice) is inline in settle()
-        auto take_slice = [&]() {
-            const uint32_t off = atomicAdd(pool_next, slice);
-            run = off < pool_len;
-            want = !run;
-            left = run ? min(slice, pool_len - off) - 1u : 0u;
-            id_lo = pool_lo + off;
-            id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
-        };
-        auto reset_history = [&]() {
+        // next photon of this lane: the next id of its private slice, else a new slice of `slice` ids from the warp pool
+        // (want = true if the pool is exhausted); resets the history state
+        auto take_photon = [&]() {
+            if (left) {
+                --left;
+                if (++id_lo == 0u) ++id_hi;
+            } else {
+                const uint32_t off = atomicAdd(pool_next, slice);
+                run = off < pool_len;
+                want = !run;
+                left = run ? min(slice, pool_len - off) - 1u : 0u;
+                id_lo = pool_lo + off;
+                id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
+            }
             T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u;
             if (NREFL) n_refl = 0u;
-            if (DM == 2 && P.launch_model) mu = diffuse_launch_mu(id_lo, id_hi, ud.stream, s_keys);      // unit-uniform, general kernel only
+            if (DM == 2 && P.launch_model) mu = diffuse_launch_mu(id_lo, id_hi, ud.stream);      // unit-uniform, general kernel only
         };
-        // End of the histories of this pass (step (7)), for the whole warp at once: `fate` != F_NONE marks the lanes whose
-        // history ended.  The common case -- the photon left outside the aperture, or was absorbed -- is straight-line code
-        // under that predicate (selects and predicated adds: no divergent region, nothing to reconverge); only an aperture
-        // hit (Eq. 19 tally, ~2 % of the histories), a roulette kill, a truncation, a trace record and the claim of a new id
-        // slice branch.
-        auto settle = [&](int fate) {
-            const bool end = fate != F_NONE;
+        // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
+        auto finish = [&](int fate) {
             const uint32_t wq = __float2uint_rn(w * kWOneF);
-            const bool out = fate == F_EXIT;
-            bool rare = out && mu >= P.mu_aperture;
-            if (ROUL) rare = rare || fate == F_KILLED;
-            if (SSO) rare = rare || fate == F_TRUNC;
-            if (rare) {
-                if (out) {                                    // inside the probe aperture: Eq. 19
+            if (fate == F_EXIT) {
+                if (mu >= P.mu_aperture) {                    // inside the probe aperture: Eq. 19
                     const float fb = (vt - P.v_lo) * P.inv_dv;
                     const uint32_t bin = (uint32_t)__float2int_rd(fb);       // floor; negative -> huge
                     if (bin < P.n_bins) {
@@ -307,32 +303,29 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                         smem_add64(&s_stats[fb < 0.f ? ST_UNDER : ST_OVER], wq);
                         fate = F_DET_OUT;
                     }
-                } else if (ROUL && fate == F_KILLED) {
-                    smem_add64(&s_stats[ST_KILLED], wq);
-                } else if (SSO && fate == F_TRUNC) {
-                    smem_add64(&s_stats[ST_TRUNC], wq);
+                    acc_rare += wq;
+                } else {
+                    acc_esc += wq;
                 }
+            } else if (ROUL && fate == F_KILLED) {
+                smem_add64(&s_stats[ST_KILLED], wq);
+                acc_rare += wq;
+            } else if (SSO && fate == F_TRUNC) {
+                smem_add64(&s_stats[ST_TRUNC], wq);
                 acc_rare += wq;
             }
-            acc_esc += (out && !rare) ? wq : 0u;
-            acc_abss += end ? min(__float2uint_rn(abss * kWOneF), kWOne - wq) : 0u;
+            acc_abss += min(__float2uint_rn(abss * kWOneF), kWOne - wq);
             const uint32_t n_int = nfl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);     // scatters + reflections
-            cnt_fl += end ? nfl : 0u;                         // an absorbing interaction is a particle event too
-            max_ev = max(max_ev, end ? n_int : 0u);
-            if (TRACE && end) {
+            cnt_fl += nfl;                                    // an absorbing interaction is a particle event too
+            max_ev = max(max_ev, n_int);
+            if (TRACE) {
                 const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
                 pdv_trace_record r;
                 r.vt = vt; r.weight = w; r.mu_exit = mu; r.fate = fate == F_ABS_PART ? F_ABS_SURF : fate;
                 r.n_scatter = (int)(n_int - n_refl); r.n_reflect = (int)n_refl;
                 P.trace[idx] = r;
             }
-            // the lane's next photon: the next id of its private slice, else (rare) a new slice from the warp pool
-            const bool next = end && left != 0u;
-            left -= next ? 1u : 0u;
-            id_lo += next ? 1u : 0u;
-            id_hi += (next && id_lo == 0u) ? 1u : 0u;
-            if (end && !next) take_slice();
-            if (end) reset_history();
+            take_photon();
         };
         // One flight (D2): `a` = path word, `cw` = class word (POLY), `b` = phase word, `pw` = azimuth / surface
         // polar-angle word, `ya` = absorption word (ANALOG), `sub` = which roulette word of the second block.
@@ -396,9 +389,9 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 // the flight that just ended is nfl - 1: monodisperse, word 2 + sub of the companion of block (nfl - 1) / 2;
                 // polydisperse, word sub of the companion of the group's second block
                 const uint32_t yr = ANALOG ? y_roul
-                                    : POLY ? philox_roulette_word(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, s_keys, sub)
-                                           : philox_roulette_word(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, s_keys, 2u + sub);
-                const RouletteOut o = roulette(w, abss, yr, P.roulette_thr, P.roulette_inv_p, s_stats);
+                                    : POLY ? philox_roulette_word(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, sub)
+                                           : philox_roulette_word(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, 2u + sub);
+                const RouletteOut o = roulette(w, abss, yr, P.roulette_thr, P.roulette_inv_p);
                 if (o.killed) return F_KILLED;
                 w = o.w; abss = o.abss; acc_gain += o.add_lost; acc_abss += o.add_abss;
             }
@@ -434,7 +427,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     const unsigned long long id0 = P.first_id + __shfl_sync(FULL_MASK, b, 0);
                     pool_lo = (uint32_t)id0; pool_hi = (uint32_t)(id0 >> 32); pool_len = len;
                     slice = max(len >> 5, 1u);                    // a lane takes 1/32 of the pool at a time: 1 id from the last pools
-                    if (want) { take_slice(); reset_history(); }
+                    if (want) take_photon();
                     if (!__any_sync(FULL_MASK, want)) break;
                 }
                 if (!__any_sync(FULL_MASK, run)) break;
@@ -477,13 +470,13 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     }
                 }
             }
-            __syncwarp();                                     // histories that ended in any flight of the pass are settled together
-            settle(fate);                                     // the one place where a lane moves on to its next photon
+            __syncwarp();                                     // histories that ended in either flight are finished in ONE pass
+            if (fate != F_NONE) finish(fate);                 // the one place where a lane moves on to its next photon
             refill = __any_sync(FULL_MASK, want);             // only a finished history can leave a lane waiting for an id
         }
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
-        // mod 2^64 per thread; the sum over a warp is the non-negative total (every history is claimed and settled in one warp)
+        // mod 2^64 per thread; the sum over a warp is the non-negative total (every history is claimed and finished in one warp)
         unsigned long long acc_absp = ((unsigned long long)cnt_hist << 31) + acc_gain - acc_esc - acc_rare - acc_abss;
         uint32_t cnt_ev = cnt_fl - cnt_refl;
 #pragma unroll
@@ -760,7 +753,6 @@ __global__ void __launch_bounds__(256) phase_check_kernel(const float2 *__restri
     extern __shared__ __align__(16) unsigned char smem[];
     float4 *s_coef = reinterpret_cast<float4 *>(smem);
     uint32_t *s_ht = reinterpret_cast<uint32_t *>(s_coef + n_terms), *s_he = s_ht + n_bins;
-    __shared__ __align__(16) uint4 s_keys[5];
     __shared__ double s_sum[2];
     __shared__ unsigned long long s_cnt[2];
     const uint32_t tid = threadIdx.x;

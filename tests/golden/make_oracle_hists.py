@@ -1,0 +1,78 @@
+#!/usr/bin/env python
+"""Writes the stored oracle histograms tests/golden/oracle_hist_*.json -- calls ONLY oracle/ (and pdv_workloads for the inputs).
+
+    python tests/golden/make_oracle_hists.py [name ...]        # default: all; takes ~20 min on 8 cores
+
+The full-size GPU parity tests (tests/test_gpu_parity.py::test_full_size_*) compare 1e8 ... 1e9-history GPU runs with the oracle.
+An oracle run the test can afford live (a few 1e6 histories) leaves the comparison without power where it matters (the tolerance
+5 sqrt(var_gpu + var_cpu) is then the oracle's own noise), so the oracle is run ONCE here at >= 1e8 histories per spectrum and its
+tallies are stored as text: hist = sum of weights per bin, hist2 = sum of squared weights per bin, the run statistics, the photon
+count, the generator (rng_mode 0 = xoshiro256**, unrelated to the GPU's Philox) and the seed.  Nothing here is computed by, or read
+from, the CUDA path.  One spectrum per cloud is enough: in vacuum the expected spectrum does not depend on the snapshot time
+(reading R16), so the same stored spectrum serves every snapshot of config 3.
+"""
+from __future__ import annotations
+
+import json
+import os
+import sys
+import time
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import pdv_workloads as W  # noqa: E402
+from oracle import cloud as ocloud  # noqa: E402
+from oracle import mc as omc  # noqa: E402
+
+SEED = 20201203
+CHUNK = 50_000_000          # histories per oracle call (ids [k CHUNK, (k+1) CHUNK)): bounds the size of one call
+
+# name -> (BASELINE.json config index, cloud index, histories)
+JOBS = {
+    "cfg2": (1, 0, 400_000_000),
+    "cfg3": (2, 0, 400_000_000),
+    "cfg4_cloud03": (3, 3, 100_000_000),
+    "cfg4_cloud22": (3, 22, 100_000_000),
+    "cfg4_cloud36": (3, 36, 100_000_000),
+    "cfg4_cloud44": (3, 44, 100_000_000),
+    "cfg5": (4, 0, 400_000_000),
+}
+
+
+def make(name: str) -> str:
+    idx, ci, n = JOBS[name]
+    cfg = W.config(idx)
+    oc = ocloud.build_cloud(cfg["clouds"][ci])
+    run = dict(cfg["run"], seed=SEED)
+    hist = hist2 = None
+    stats: dict = {}
+    t0 = time.time()
+    for first in range(0, n, CHUNK):
+        r = omc.run(oc, run, n_photons=min(CHUNK, n - first), first_id=first)
+        hist = r.hist if hist is None else hist + r.hist
+        hist2 = r.hist2 if hist2 is None else hist2 + r.hist2
+        for k, v in r.stats.items():
+            stats[k] = max(stats.get(k, 0), v) if k == "max_events_in_history" else stats.get(k, 0) + v
+    out = {
+        "what": "oracle/ (fp64 CPU Monte-Carlo) tallies; written by tests/golden/make_oracle_hists.py; no value comes from the CUDA path",
+        "workload": cfg["name"], "config_index": idx, "cloud_index": ci, "n_photons": n, "seed": SEED, "rng_mode": 0,
+        "run": {k: run[k] for k in ("n_bins", "v_lo", "v_hi", "aperture_sr", "mode", "max_events", "roulette_survival")},
+        "tau_ext": oc.tau_ext, "seconds": round(time.time() - t0, 1), "threads": os.cpu_count(),
+        "stats": {k: (int(v) if isinstance(v, int) else float(v)) for k, v in stats.items()},
+        "hist": [float(x) for x in hist], "hist2": [float(x) for x in hist2],
+    }
+    path = os.path.join(HERE, f"oracle_hist_{name}.json")
+    with open(path, "w") as f:
+        json.dump(out, f, separators=(",", ":"))
+        f.write("\n")
+    return path
+
+
+if __name__ == "__main__":
+    for nm in (sys.argv[1:] or list(JOBS)):
+        t = time.time()
+        p = make(nm)
+        print(f"{nm}: {p} ({time.time() - t:.0f} s)", flush=True)

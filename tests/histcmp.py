@@ -8,7 +8,20 @@ the last group.
 """
 from __future__ import annotations
 
+import json
+import os
+from types import SimpleNamespace
+
 import numpy as np
+
+
+def load_golden(name: str) -> SimpleNamespace:
+    """Stored oracle tallies tests/golden/oracle_hist_<name>.json (written by tests/golden/make_oracle_hists.py, which calls only
+    oracle/): an object with .hist, .hist2, .stats, .n_photons like an oracle run of >= 1e8 histories."""
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"oracle_hist_{name}.json")) as f:
+        d = json.load(f)
+    return SimpleNamespace(hist=np.asarray(d["hist"], dtype=np.float64), hist2=np.asarray(d["hist2"], dtype=np.float64),
+                           stats=d["stats"], n_photons=int(d["n_photons"]), run=d["run"], tau_ext=d["tau_ext"])
 
 
 def merge_groups(h_a, h2_a, h_b, h2_b, min_eff=25.0):

@@ -15,7 +15,7 @@ import pdv_workloads as W
 from oracle import cloud as ocloud
 from oracle import mc as omc
 
-from histcmp import compare
+from histcmp import compare, load_golden
 
 pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("_library_is_built")]
 
@@ -154,15 +154,17 @@ def test_history_by_history_on_shared_philox_stream(P, idx, mode):
     out = same & (tr["fate"] <= 1)
     assert out.sum() > 0.3 * n
     dv = np.abs(rec["vt"][out] - tr["vt"][out])
-    # fp32 tolerance: one event moves v~ by 1/2 v dmu with dmu ~ 1e-6 (__cosf 2^-21.4 abs,
-    # sqrt.approx, fma rounding) => ~3e-3 m/s per event at v ~ 6 km/s.  The same dmu shifts the end of the next flight
-    # by dT ~ 1e-6 per event, which accumulates over a history (up to ~70 events) and is amplified where v(T) is
-    # logarithmic: in the top 3e-4 of the cloud's optical depth dv/dT ~ 8e5 m/s, so a rare history that scatters
-    # there moves by tens of m/s.  Bins are 11.7 m/s wide: median error << 1e-3 bin, 99.9 % below 2 % of a bin,
-    # fewer than 1e-4 of the histories off by more than 1 m/s.
-    assert np.median(dv) < 0.005 and np.quantile(dv, 0.999) < 0.25 and np.mean(dv > 1.0) < 1e-4 and dv.max() < 500.0
+    # fp32 tolerance ("History by history"): one event moves v~ by 1/2 v dmu with dmu ~ 1e-6 (cos.approx
+    # 2^-21.4 abs, sqrt.approx, lg2.approx, fma rounding) => ~3e-3 m/s per event at v ~ 6 km/s, a random walk over the ~10-20
+    # events of a history.  The same dmu shifts the end of the next flight by dT ~ 1e-6, and where v(T) is logarithmic (the
+    # top 3e-4 of the optical depth: dv/dT ~ 8e5 m/s) that is ~1 m/s: a few histories in 1e5 scatter there.  Bins are
+    # 11.7 m/s wide.  Measured at this size (profiles/README.md, round 2): median 1.5e-4 ... 2.7e-4, 99.9 % 0.03 ... 0.09,
+    # max 0.5 ... 2.5 m/s, max |d mu_exit| 6e-5 ... 2.8e-4.  max < 20 m/s and max |d mu_exit| < 1e-3 are the bounds the test
+    # was introduced with; the 99.9 % quantile was 0.05 for the first kernel (libm logf / sincosf) and is 0.15 since the
+    # kernel evaluates ln, cos and sqrt on the SFU (__cosf in commit a2d46aa; the bound was widened in 6a5f781).
+    assert np.median(dv) < 0.005 and np.quantile(dv, 0.999) < 0.15 and np.mean(dv > 1.0) < 1e-4 and dv.max() < 20.0
     dmu = np.abs(rec["mu_exit"][out] - tr["mu_exit"][out])
-    assert np.quantile(dmu, 0.9999) < 1e-3 and np.mean(dmu > 1e-3) < 2e-5
+    assert dmu.max() < 1e-3
     # identical decisions => near-identical histograms, far tighter than the statistical tolerance
     assert abs(r.hist.sum() - o.hist.sum()) < 2e-3 * o.hist.sum() + 5
     assert np.sum(np.abs(r.hist[0, 0] - o.hist)) < 0.01 * o.hist.sum() + 10
@@ -298,28 +300,32 @@ def test_empty_and_tiny_runs_and_empty_cloud(P):
 
 
 def test_closed_form_backscatter_histogram_on_gpu(P):
-    """Pin P2 evaluated on the GPU itself: all-backward scattering is not expressible through the boundary, so use
-    the pure-absorber limit instead (pin P1): a strongly absorbing index gives omega0 << 1 and the detected weight is
-    dominated by the direct surface reflection  N e^-tau R (2/pi) int exp(-tau/cos th) dth."""
+    """Pins P1 / P9 evaluated on the GPU itself, two-sided, with no reference implementation in the loop: tin spheres of
+    50 nm are almost pure absorbers at 1550 nm (x = 0.1: K_sca ~ x^4, K_abs ~ x, albedo 0.024), so the weight in the bins
+    just below v_fs is the direct surface reflection alone,
+        N e^-tau R (2/pi) int_0^{acos mu_a} exp(-tau / cos th) dth        (Beer-Lambert Eq. 7/10 down and up),
+    and photons that also scattered once near the surface add less than 1e-3 of it."""
     cfg = W.config(0)
-    params = dict(cfg["clouds"][0], area_mass=1.0 * W.MG_CM2)
+    params = dict(cfg["clouds"][0], diameters=[0.05e-6], area_mass=1.0 * W.MG_CM2)
     c = P.pdv_cloud_create(params)
-    tau = c.info()["tau_ext"]
-    n = 2_000_000
-    r = P.pdv_mc_run([c], cfg["t_snap"], n, 3, dict(cfg["run"], mode=1, single_scatter_only=1))
-    s = r.stats[0, 0]
-    # photons that reach the surface unscattered: Binomial(n, e^-tau) (Beer-Lambert, Eq. 7/10) -- counted as
-    # reflections + surface absorptions of histories without a particle event; here via the direct-reflection peak
+    info = c.info()
+    tau = info["tau_ext"]
+    assert 0.4 < tau < 2.0 and info["mean_albedo"] < 0.03
+    n = 8_000_000
     th = (np.arange(20000) + 0.5) / 20000 * math.acos(1 - 0.1 / (2 * math.pi))
     p_direct = math.exp(-tau) * 0.6 * (2 / math.pi) * np.sum(np.exp(-tau / np.cos(th))) * (th[1] - th[0])
     dv = 6000 / 512
     k_lo, k_hi = int(0.5 * (2 - 0.1 / (2 * math.pi)) * 2000 / dv), int(2000 / dv)
-    direct = r.hist[0, 0, k_lo:k_hi + 1].sum()
-    # single-scatter-only: besides direct reflection only one-scatter paths contribute; they add a little in these bins
-    o = _oracle(params, dict(cfg["run"], mode=1, single_scatter_only=1), n)
-    assert direct >= n * p_direct - 5 * math.sqrt(n * p_direct)
-    assert abs(direct - o.hist[k_lo:k_hi + 1].sum()) < 5 * math.sqrt(2 * direct)
-    assert s["truncated"] > 0
+    for mode in (0, 1):                             # implicit capture (weights 0.6) and analog (weights 1)
+        r = P.pdv_mc_run([c], cfg["t_snap"], n, 3 + mode, dict(cfg["run"], mode=mode))
+        s = r.stats[0, 0]
+        direct = r.hist[0, 0, k_lo:k_hi + 1].sum()
+        var = r.hist2[0, 0, k_lo:k_hi + 1].sum()
+        assert abs(direct - n * p_direct) < 5 * math.sqrt(var) + 1e-3 * n * p_direct, (mode, direct, n * p_direct)
+        # photons that reach the surface unscattered ~ Binomial(n, e^-tau) and leave (1 - R) of their weight there; the few
+        # that scattered first (albedo 0.024) add less than 1 %
+        assert float(s["absorbed_surface"]) == pytest.approx(0.4 * n * math.exp(-tau), rel=0.02)
+        assert r.conservation_residual()[0, 0] == 0.0
 
 
 # -------------------------------------------------------------------------------------------------- outputs
@@ -385,7 +391,7 @@ def test_photon_count_limit_of_the_fixed_point_tallies(P):
 
 def test_full_size_config2_in_bench_launch_configuration(P):
     """BASELINE.json configs[1] at full size (1e8 photons, default launch shape = what bench.py times): invariants
-    that hold at any size, plus parity against an oracle run the CPU can afford (4e7 histories)."""
+    that hold at any size, plus parity against the stored 4e8-history oracle run (tests/golden/oracle_hist_cfg2.json)."""
     cfg = W.config(1)
     c = P.pdv_cloud_create(cfg["clouds"][0])
     n = cfg["run"]["n_photons"]
@@ -395,9 +401,10 @@ def test_full_size_config2_in_bench_launch_configuration(P):
     # 1e8 * 2^31 exceeds 2^53: the double sum of exact Q31 terms may round in the last bits only
     assert abs(r.conservation_residual()[0, 0]) < 1e-6
     assert r.hist.sum() == pytest.approx(s["detected"], rel=1e-12)
-    n_o = 40_000_000
-    o = _oracle(cfg["clouds"][0], cfg["run"], n_o)
-    res = _assert_hist_parity(r.hist[0, 0], r.hist2[0, 0], n, o, min_ndf=200)
+    o = load_golden("cfg2")
+    n_o = o.n_photons
+    assert n_o >= 4 * n and o.run["n_bins"] == cfg["run"]["n_bins"]
+    res = _assert_hist_parity(r.hist[0, 0], r.hist2[0, 0], n, o, min_ndf=300)
     top_g = (s["detected"] + s["underflow"] + s["overflow"] + s["escaped"]) / n
     top_o = (o.stats["detected"] + o.stats["underflow"] + o.stats["overflow"] + o.stats["escaped"]) / n_o
     assert top_g == pytest.approx(top_o, rel=1e-3)                  # integrated backscatter, north_star
@@ -410,19 +417,23 @@ def test_full_size_configs_3_4_5(P):
     """The other BASELINE.json configs at their full photon counts in the default launch shape: config 3 (16 classes) as a
     slice of 4 of its 200 snapshots at 1e8 photons each, config 4 in full (48 clouds x 1e7), config 5 in full (1e9 photons,
     64-bit photon ids, roulette after 200 events).  Invariants that hold at any size, and parity of sampled outputs against
-    oracle runs the CPU can afford (the tolerance formula absorbs the oracle's larger sigma)."""
+    the stored oracle runs of 1e8 ... 4e8 histories (tests/golden/oracle_hist_*.json, written by make_oracle_hists.py from
+    oracle/ alone): at these sizes the 5 sigma band is the GPU's own noise, and reading R23 holds with 25 effective counts
+    for every config."""
     # ---- config 3
     cfg = W.config(2)
     c = P.pdv_cloud_create(cfg["clouds"][0])
     n = cfg["run"]["n_photons"]
     t4 = cfg["t_snap"][:2] + cfg["t_snap"][-2:]
     r = P.pdv_mc_run([c], t4, n, cfg["run"]["seed"], cfg["run"])
-    o = _oracle(cfg["clouds"][0], cfg["run"], 6_000_000)
+    o = load_golden("cfg3")
+    assert o.n_photons >= 4 * n
     for i in range(4):
         s = r.stats[0, i]
         assert s["histories"] == n and abs(r.conservation_residual()[0, i]) < 1e-6
-        _assert_hist_parity(r.hist[0, i], r.hist2[0, i], n, o, min_ndf=150)
-        assert s["particle_events"] / n == pytest.approx(o.stats["particle_events"] / o.n_photons, rel=3e-3)
+        _assert_hist_parity(r.hist[0, i], r.hist2[0, i], n, o, min_ndf=300)
+        _assert_stats_parity(s, n, o)
+        assert s["particle_events"] / n == pytest.approx(o.stats["particle_events"] / o.n_photons, rel=1e-3)
     res = compare(r.hist[0, 0], r.hist2[0, 0], n, r.hist[0, 3], r.hist2[0, 3], n)       # t = 0.5 us against t = 10 us (R16)
     assert res["worst"] < 5.0
     # ---- config 4
@@ -433,12 +444,13 @@ def test_full_size_configs_3_4_5(P):
     # 1e7 * 2^31 exceeds 2^53: the double sum of exact Q31 terms may round in the last bit
     assert np.all(r.stats["histories"] == n) and np.all(np.abs(r.conservation_residual()) < 1e-7)
     assert np.allclose(r.hist.sum(axis=2), r.stats["detected"], rtol=1e-12)
-    # sampled clouds, thin ... thick (tau 1.2, 0.9, 9.3, 18.6).  The thick ones get a larger oracle sample: their low-velocity
-    # bins are filled by a few long histories of very unequal weight, for which sum w^2 of 4e5 photons is itself uncertain
-    for i, n_o in ((3, 400_000), (22, 400_000), (36, 2_000_000), (44, 2_000_000)):
-        oo = _oracle(cfg["clouds"][i], cfg["run"], n_o)
-        _assert_hist_parity(r.hist[i, 0], r.hist2[i, 0], n, oo, min_ndf=5)
+    # sampled clouds, thin ... thick (tau 1.2, 0.9, 9.3, 18.6), each against 1e8 oracle histories
+    for i in (3, 22, 36, 44):
+        oo = load_golden(f"cfg4_cloud{i:02d}")
+        assert oo.n_photons >= 10 * n and oo.tau_ext == pytest.approx(clouds[i].info()["tau_ext"], rel=1e-9)
+        _assert_hist_parity(r.hist[i, 0], r.hist2[i, 0], n, oo, min_ndf=50)
         _assert_stats_parity(r.stats[i, 0], n, oo)
+        assert r.stats[i, 0]["particle_events"] / n == pytest.approx(oo.stats["particle_events"] / oo.n_photons, rel=3e-3)
     # ---- config 5
     cfg = W.config(4)
     c = P.pdv_cloud_create(cfg["clouds"][0])
@@ -449,12 +461,8 @@ def test_full_size_configs_3_4_5(P):
     s = r.stats[0, 0]
     assert s["histories"] == n and abs(r.conservation_residual()[0, 0]) < 1e-5
     assert r.hist.sum() == pytest.approx(s["detected"], rel=1e-12)
-    oo = _oracle(cfg["clouds"][0], cfg["run"], 3_000_000)
-    # The GPU side is 300x larger, so the oracle's bins are measured against the truth and their own sum w^2 must be a
-    # trustworthy variance: below v_fs the bins are filled by a few long histories of very unequal weight, and 25 effective
-    # counts are not enough for that (measured: the same 5.7-7.2 sigma appear when a 3e6-photon GPU run is compared with the
-    # 1e9 one).  Reading R23 with 100 effective counts per merged bin.
-    _assert_hist_parity(r.hist[0, 0], r.hist2[0, 0], n, oo, min_ndf=150, min_eff=100.0)
+    oo = load_golden("cfg5")                                      # 4e8 oracle histories
+    _assert_hist_parity(r.hist[0, 0], r.hist2[0, 0], n, oo, min_ndf=300)
     _assert_stats_parity(s, n, oo, same_game=False)
     top_g = (s["detected"] + s["underflow"] + s["overflow"] + s["escaped"]) / n
     top_o = (oo.stats["detected"] + oo.stats["underflow"] + oo.stats["overflow"] + oo.stats["escaped"]) / oo.n_photons
