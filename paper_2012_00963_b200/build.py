@@ -17,6 +17,17 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC,-O3", "-shared", "-cudart", "static"]
 
 
+def kernel_source_hash() -> str:
+    """sha256 over the sources of the CUDA kernels (csrc/pdv_kernels.cu, csrc/pdv_device.h): the key that ties an ncu capture
+    under profiles/ to the kernel it was taken from (bench.py prints a capture's counters only when the key matches)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("pdv_kernels.cu", "pdv_device.h"):
+        with open(os.path.join(CSRC, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def _nvcc() -> str:
     for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
         if cand and (os.path.sep not in cand or os.path.exists(cand)):

@@ -382,6 +382,38 @@ def test_two_device_output_runs_on_two_streams_are_independent(P):
                 assert np.array_equal(ds[k], tw.stats[0][k]), k
 
 
+@pytest.mark.parametrize("idx,n_snap,n_clouds,scaling", [(1, None, None, "strong"), (2, 5, None, "strong"), (3, None, 6, "strong"),
+                                                         (1, None, None, "weak")])
+def test_sharded_runs_reduce_to_the_single_run_bit_for_bit(P, idx, n_snap, n_clouds, scaling):
+    """SURVEY.md 8(e) on one GPU: the shares of a 3-rank job (paper_2012_00963_b200/_shard.py::plan, what bench.py --gpus N runs:
+    id ranges for one unit, whole units -- with their sub-streams of the whole job -- for several) are run one after the other
+    and reduced with reduce_job; the result must equal the one-call run of the job in every bit of hist, hist2 and stats."""
+    import torch
+    from paper_2012_00963_b200 import _shard
+    cfg = W.scaled(W.config(idx), 150_001, n_snap=n_snap, n_clouds=n_clouds)
+    run, n, world = cfg["run"], cfg["run"]["n_photons"], 3
+    clouds = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
+    nc, ns, nb = len(clouds), len(cfg["t_snap"]), run["n_bins"]
+    total = n * world if scaling == "weak" else n
+    whole = P.pdv_mc_run(clouds, cfg["t_snap"], total, 19, run)
+    acc_h = torch.zeros((nc * ns, nb), dtype=torch.float64)
+    acc_h2 = torch.zeros_like(acc_h)
+    parts = []
+    for rank in range(world):
+        pl = _shard.plan(nc, ns, n, rank, world, scaling)
+        r = P.pdv_mc_run([clouds[i] for i in pl["clouds"]], [cfg["t_snap"][j] for j in pl["snaps"]], pl["n_photons"], 19,
+                         dict(run, first_photon_id=pl["first_photon_id"], unit_streams=pl["unit_ids"]))
+        h, h2, st = _shard.reduce_job(torch.from_numpy(r.hist.reshape(-1, nb)), torch.from_numpy(r.hist2.reshape(-1, nb)),
+                                      r.stats.reshape(-1), pl["unit_ids"], nc * ns)
+        acc_h += h
+        acc_h2 += h2
+        parts.append(st)
+    st = _shard.merge_stats(parts)
+    assert np.array_equal(acc_h.numpy(), whole.hist.reshape(-1, nb)) and np.array_equal(acc_h2.numpy(), whole.hist2.reshape(-1, nb))
+    for k in st.dtype.names:
+        assert np.array_equal(st[k], whole.stats.reshape(-1)[k]), k
+
+
 def test_photon_count_limit_of_the_fixed_point_tallies(P):
     cfg = W.config(1)
     c = P.pdv_cloud_create(cfg["clouds"][0])

@@ -8,7 +8,7 @@ import socket
 import numpy as np
 import pytest
 
-from paper_2012_00963_b200._shard import ADDITIVE_STATS, allreduce_tallies, merge_stats, shard_photons, shard_units
+from paper_2012_00963_b200._shard import ADDITIVE_STATS, allreduce_tallies, merge_stats, plan, reduce_job, shard_photons, shard_units
 
 
 def test_shard_photons_tiles_the_id_range_exactly():
@@ -83,3 +83,91 @@ def test_merge_stats_sums_additive_fields_and_takes_the_max():
     for i, k in enumerate(ADDITIVE_STATS):
         assert np.all(m[k] == 11 * (i + 1))
     assert list(m["max_events_in_history"]) == [7, 9, 2]
+
+
+# ---------------------------------------------------------------------------------------------------------------------------
+# The sharding arithmetic bench.py runs (plan + reduce_job), on 2 gloo ranks.  The "tallies" of a unit are a deterministic
+# integer function of (unit id, photon id), as the library's are of (unit sub-stream, photon id): whatever the split, the
+# reduced job must equal the one-rank job bit for bit.
+def _fake_unit(unit, first, count, n_bins):
+    ids = np.arange(first, first + count, dtype=np.uint64)
+    key = ids * np.uint64(2654435761) + np.uint64(unit) * np.uint64(40503)
+    w = (key % np.uint64(2**31)).astype(np.float64) / 2.0**31
+    b = (key % np.uint64(n_bins)).astype(np.int64)
+    hist = np.bincount(b, weights=w, minlength=n_bins)
+    hist2 = np.bincount(b, weights=np.floor(w * w * 2.0**31) / 2.0**31, minlength=n_bins)
+    return hist, hist2, int((key % np.uint64(7)).sum()), int((key % np.uint64(97)).max()) if count else 0
+
+
+def _fake_job(n_clouds, n_snap, n_photons, n_bins, rank, world, scaling):
+    from paper_2012_00963_b200 import STATS_DTYPE
+    pl = plan(n_clouds, n_snap, n_photons, rank, world, scaling)
+    n_loc = len(pl["unit_ids"])
+    h, h2, st = np.zeros((n_loc, n_bins)), np.zeros((n_loc, n_bins)), np.zeros(n_loc, dtype=STATS_DTYPE)
+    for k, u in enumerate(pl["unit_ids"]):
+        h[k], h2[k], ev, mx = _fake_unit(u, pl["first_photon_id"], pl["n_photons"], n_bins)
+        st[k]["histories"], st[k]["particle_events"], st[k]["max_events_in_history"] = pl["n_photons"], ev, mx
+        st[k]["detected"] = h[k].sum()
+    return pl, h, h2, st
+
+
+def _job_worker(rank, world, port, cases, n_bins, out_dir):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    for ci, (nc, ns, n, scaling) in enumerate(cases):
+        pl, h, h2, st = _fake_job(nc, ns, n, n_bins, rank, world, scaling)
+        jh, jh2, jst = reduce_job(torch.from_numpy(h), torch.from_numpy(h2), st, pl["unit_ids"], nc * ns)
+        np.save(os.path.join(out_dir, f"job{ci}_h_{rank}.npy"), jh.numpy())
+        np.save(os.path.join(out_dir, f"job{ci}_h2_{rank}.npy"), jh2.numpy())
+        np.save(os.path.join(out_dir, f"job{ci}_st_{rank}.npy"), jst)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+CASES = [(1, 1, 100_003, "strong"),      # one unit: the id range is split (configs 2, 5)
+         (1, 7, 20_000, "strong"),       # one cloud, several snapshots: whole snapshots per rank (config 3)
+         (5, 1, 20_000, "strong"),       # several clouds, one snapshot: whole clouds per rank (config 4, the sweeps)
+         (3, 2, 10_000, "strong"),       # a grid: split along the clouds
+         (2, 3, 15_001, "weak")]         # every rank runs every unit on its own id range
+
+
+def test_plan_covers_the_job_exactly():
+    for nc, ns, n, scaling in CASES:
+        for world in (1, 2, 3, 8):
+            units, photons = {}, 0
+            for rank in range(world):
+                pl = plan(nc, ns, n, rank, world, scaling)
+                assert pl["unit_ids"] == [i * ns + j for i in pl["clouds"] for j in pl["snaps"]]
+                for u in pl["unit_ids"]:
+                    units.setdefault(u, []).append((pl["first_photon_id"], pl["n_photons"]))
+            assert sorted(units) == list(range(nc * ns))
+            for u, ranges in units.items():
+                ranges.sort()
+                at = 0
+                for first, count in ranges:                  # the id ranges of a unit tile [0, total) without gap or overlap
+                    assert first == at
+                    at += count
+                assert at == (n * world if scaling == "weak" else n)
+    with pytest.raises(ValueError):
+        plan(1, 1, 10, 0, 1, "both")
+
+
+def test_reduced_job_of_two_ranks_equals_the_one_rank_job_bit_for_bit(tmp_path):
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    n_bins, world = 48, 2
+    mp.spawn(_job_worker, args=(world, port, CASES, n_bins, str(tmp_path)), nprocs=world, join=True)
+    for ci, (nc, ns, n, scaling) in enumerate(CASES):
+        total = n * world if scaling == "weak" else n
+        _, h, h2, st = _fake_job(nc, ns, total, n_bins, 0, 1, "strong")          # the whole job on one rank
+        for rank in range(world):
+            assert np.array_equal(np.load(tmp_path / f"job{ci}_h_{rank}.npy"), h), (ci, rank)
+            assert np.array_equal(np.load(tmp_path / f"job{ci}_h2_{rank}.npy"), h2), (ci, rank)
+            jst = np.load(tmp_path / f"job{ci}_st_{rank}.npy")
+            for k in ("histories", "particle_events", "max_events_in_history", "detected"):
+                assert np.array_equal(jst[k], st[k]), (ci, rank, k)
