@@ -43,6 +43,8 @@ constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
 // (a pointer parameter would make it a generic address: window-base arithmetic at every call site, generic loads inside).
 __shared__ __align__(16) uint4 s_keys[5];                 // Philox round keys, two rounds per uint4
 __shared__ unsigned long long s_stats[ST_COUNT];          // per-unit statistics of the block (transport_kernel)
+__shared__ uint32_t s_roul_thr;                           // Russian roulette: survive iff the roulette word < s_roul_thr ...
+__shared__ float s_roul_inv_p;                            // ... and then w /= p
 
 // Philox4x32-10 block function.  The 10 round keys (k0_r, k1_r) are precomputed on the host and staged in shared memory,
 // two rounds per uint4: five broadcast LDS.128 per block instead of ten constant-bank loads (the ADU pipe that serves
@@ -118,8 +120,11 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
         }
         j = lo;
     } else {
-        uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base) - cv.guide_base;
-        PDV_BOUND(0, cell, cv.n_guide);
+        // cv.guide points guide_base cells BEFORE the table, so the clamped cell number indexes it directly
+        uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base);
+#ifdef PDV_DEBUG_BOUNDS
+        { uint32_t rel = cell - cv.guide_base; PDV_BOUND(0, rel, cv.n_guide); cell = rel + cv.guide_base; }
+#endif
         j = cv.guide[cell];
     }
     PDV_BOUND(1, j, cv.n_depth);
@@ -151,11 +156,11 @@ __device__ __noinline__ float lambert_mu(float pwf) { return fast_sqrt(pwf * 2.3
 // that w / p <= 1.  `yr` is the roulette word of the flight's second Philox block.  Everything by value: a reference
 // parameter would pin the caller's weight registers to local memory.
 struct RouletteOut { float w, abss; uint32_t add_lost, add_abss, killed; };
-__device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, uint32_t thr, float inv_p) {
+__device__ __forceinline__ RouletteOut roulette(float w, float abss, uint32_t yr) {
     RouletteOut o;
-    o.w = w; o.abss = abss; o.add_lost = 0u; o.add_abss = 0u; o.killed = yr >= thr ? 1u : 0u;
+    o.w = w; o.abss = abss; o.add_lost = 0u; o.add_abss = 0u; o.killed = yr >= s_roul_thr ? 1u : 0u;
     if (o.killed) return o;
-    const float wn = fminf(w * inv_p, 1.f);
+    const float wn = fminf(w * s_roul_inv_p, 1.f);
     const uint32_t q0 = __float2uint_rn(w * kWOneF), q1 = __float2uint_rn(wn * kWOneF);
     const uint32_t gain = q1 > q0 ? q1 - q0 : 0u;
     smem_add64(&s_stats[ST_GAINED], gain);
@@ -167,13 +172,17 @@ __device__ __noinline__ RouletteOut roulette(float w, float abss, uint32_t yr, u
     return o;
 }
 
-// roulette word of a flight for the implicit-capture kernels, which do not draw the companion blocks: word `word` of the
-// block with counter word 3 = ctr3 (D1/D2), out of line
-__device__ __noinline__ uint32_t philox_roulette_word(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t ctr3, uint32_t word) {
+// One game for the implicit-capture kernels, which do not draw the companion blocks: the roulette word is word `word` of the
+// block with counter word 3 = ctr3 (D1/D2).  ONE out-of-line function (block + game), nine register arguments: a
+// game runs at about one lane of the warp, so every instruction of it, call sequence included, costs a whole issue slot
+// (config 5: a game per 415 flights took 8 % of the kernel's issue slots as two calls with pointer arguments).
+__device__ __noinline__ RouletteOut roulette_with_draw(uint32_t id_lo, uint32_t id_hi, uint32_t stream, uint32_t ctr3, uint32_t word,
+                                                       float w, float abss) {
     uint32_t y0, y1, y2, y3;
     philox4x32_10(id_lo, id_hi, stream, ctr3, s_keys, y0, y1, y2, y3);
-    return word == 0u ? y0 : word == 1u ? y1 : word == 2u ? y2 : y3;
+    return roulette(w, abss, word == 0u ? y0 : word == 1u ? y1 : word == 2u ? y2 : y3);
 }
+__device__ __noinline__ RouletteOut roulette_with_word(float w, float abss, uint32_t yr) { return roulette(w, abss, yr); }
 
 
 // History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
@@ -191,6 +200,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
     unsigned long long *s_hist2 = s_hist + P.n_bins;
     unsigned char *s_blob = smem + 16u * (size_t)P.n_bins;
     if (tid < 5) s_keys[tid] = make_uint4(P.key0[2 * tid], P.key1[2 * tid], P.key0[2 * tid + 1], P.key1[2 * tid + 1]);
+    if (ROUL && tid == 0) { s_roul_thr = P.roulette_thr; s_roul_inv_p = P.roulette_inv_p; }
 
     for (uint32_t visit = 0; visit < P.n_units; ++visit) {
         const uint32_t u = P.units[(P.block_start[blockIdx.x] + visit) % P.n_units].visit;
@@ -222,7 +232,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cv.thr = reinterpret_cast<const uint32_t *>(s_blob + h->off_thr);
             cv.albedo = reinterpret_cast<const float *>(s_blob + h->off_albedo);
             cv.albthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_albthr);
-            cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide);
+            cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide) - h->guide_base;
             cv.cguide = s_blob + h->off_cguide;
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
@@ -255,12 +265,13 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         uint32_t cnt_hist = 0u, cnt_fl = 0u, cnt_refl = 0u, max_ev = 0u;
 
         // ---- lane state: one photon history (step (1)) ---------------------------------------------
-        // nfl = flights flown so far = Philox draw index of the next flight (D1); n_refl = reflections of this
-        // history, carried only by the variants that read it (NREFL).
+        // nfl = flights flown so far = Philox draw index of the next flight (D1); refl0 = the thread's reflection
+        // counter at the start of this history, kept only by the variants that read a history's own reflection count (NREFL).
         // run: the lane flies a photon; want: it needs a photon id (neither: the unit is drained, the lane is done).
         bool run = false, want = true;
         float T = 0.f, mu = -1.f, vt = 0.f, w = 1.f, abss = 0.f;
-        uint32_t nfl = 0u, n_refl = 0u, id_lo = 0u, id_hi = 0u;
+        uint32_t nfl = 0u, refl0 = 0u, id_lo = 0u, id_hi = 0u;
+#define N_REFL (cnt_refl - refl0)      /* reflections of this history: the thread's counter minus its value at the history's start */
         // ---- the warp's pool of photon ids: [pool_lo/hi, + pool_len), warp-uniform registers; the hand-out cursor lives in
         // shared memory so that a lane can take a slice of ids from inside the divergent end-of-history code with one shared
         // atomic.  Pools are claimed from the unit's global cursor by lane 0 (guided sizes): ~1e4 times fewer global
@@ -285,7 +296,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
             }
             T = 0.f; mu = -1.f; vt = 0.f; w = 1.f; abss = 0.f; nfl = 0u;
-            if (NREFL) n_refl = 0u;
+            if (NREFL) refl0 = cnt_refl;
             if (DM == 2 && P.launch_model) mu = diffuse_launch_mu(id_lo, id_hi, ud.stream);      // unit-uniform, general kernel only
         };
         // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
@@ -322,7 +333,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 const unsigned long long idx = (((unsigned long long)id_hi << 32) | id_lo) - P.first_id;
                 pdv_trace_record r;
                 r.vt = vt; r.weight = w; r.mu_exit = mu; r.fate = fate == F_ABS_PART ? F_ABS_SURF : fate;
-                r.n_scatter = (int)(n_int - n_refl); r.n_reflect = (int)n_refl;
+                r.n_scatter = (int)(n_int - N_REFL); r.n_reflect = (int)N_REFL;
                 P.trace[idx] = r;
             }
             take_photon();
@@ -337,7 +348,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             const float Tn = fmaf(-mu, s, T);
             if (Tn < 0.f) return F_EXIT;                      // leaves through the top (step (6))
             const bool surf = Tn >= cv.tau_ext;               // reaches the free surface
-            if (SSO && !surf && nfl != n_refl) return F_TRUNC;    // single-scatter-only: cut at the 2nd particle event
+            if (SSO && !surf && nfl != N_REFL) return F_TRUNC;    // single-scatter-only: cut at the 2nd particle event
             // ---------------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ------
             T = fminf(Tn, cv.tau_ext);
             float vh;                                         // = v_fs / 2 at the surface
@@ -383,15 +394,17 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             vt = fmaf(mu_new - mu, vh, vt);                   // Eq. 4 (vh = v/2)
             mu = mu_new;
             ++nfl;
-            cnt_refl += surf ? 1u : 0u;
-            if (NREFL) n_refl += surf ? 1u : 0u;
-            if (ROUL && nfl - n_refl >= P.max_events && w <= P.roulette_p) {       // Russian roulette (rare path)
+            // cnt_refl += surf, as ONE predicated add on the predicate the flight already has (the compiler's own version of
+            // this conditional increment was an add, a predicated move and a move)
+            asm("{\n\t.reg .pred p;\n\tsetp.ge.f32 p, %1, %2;\n\t@p add.u32 %0, %0, 1;\n\t}" : "+r"(cnt_refl) : "f"(Tn), "f"(cv.tau_ext));
+            // Russian roulette (rare path): flights >= particle events, so one integer compare keeps every flight before the
+            // max_events-th out of the detailed test
+            if (ROUL && nfl >= P.max_events && nfl - N_REFL >= P.max_events && w <= P.roulette_p) {
                 // the flight that just ended is nfl - 1: monodisperse, word 2 + sub of the companion of block (nfl - 1) / 2;
                 // polydisperse, word sub of the companion of the group's second block
-                const uint32_t yr = ANALOG ? y_roul
-                                    : POLY ? philox_roulette_word(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, sub)
-                                           : philox_roulette_word(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, 2u + sub);
-                const RouletteOut o = roulette(w, abss, yr, P.roulette_thr, P.roulette_inv_p);
+                const RouletteOut o = ANALOG ? roulette_with_word(w, abss, y_roul)
+                                      : POLY ? roulette_with_draw(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, sub, w, abss)
+                                             : roulette_with_draw(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, 2u + sub, w, abss);
                 if (o.killed) return F_KILLED;
                 w = o.w; abss = o.abss; acc_gain += o.add_lost; acc_abss += o.add_abss;
             }
