@@ -49,6 +49,8 @@ class _Params(C.Structure):
         ("mode", C.c_int32), ("max_events", C.c_int32), ("p_roulette", C.c_double),
         ("single_scatter_only", C.c_int32), ("rng_mode", C.c_int32), ("seed", C.c_uint64),
         ("stream", C.c_uint32), ("launch_model", C.c_int32),
+        ("gas", C.c_int32), ("zeta_edge", C.POINTER(C.c_double)), ("class_cum", C.POINTER(C.c_double)),
+        ("gas_L", C.POINTER(C.c_double)), ("t_snap", C.c_double),
     ]
 
 
@@ -117,7 +119,7 @@ class OracleResult:
 
 def run(cloud: OracleCloud, run_opts: dict, *, n_photons: int | None = None, first_id: int = 0, stream: int = 0,
         seed: int | None = None, rng_mode: int = 0, n_threads: int | None = None, analytic_profile: bool = False,
-        exact_mie: dict | None = None, trace: bool = False, launch_model: int = 0) -> OracleResult:
+        exact_mie: dict | None = None, trace: bool = False, launch_model: int = 0, gas: dict | None = None) -> OracleResult:
     """Run the oracle Monte-Carlo for one (cloud, snapshot) unit.
 
     run_opts: the "run" dictionary of a pdv_workloads config (n_bins, v_lo, v_hi, aperture_sr, mode,
@@ -126,6 +128,8 @@ def run(cloud: OracleCloud, run_opts: dict, *, n_photons: int | None = None, fir
     on the exact Mie function; requires rng_mode 0.
     launch_model 1: diffuse (Lambertian) illumination of the cloud top instead of the paper's collimated beam -- exists
     only for the invariance pin of the multiple-scattering core (tests/test_oracle_mc.py), rng_mode 0.
+    gas: the tables of oracle/gas.py::build_tables for this (cloud, snapshot) unit -- ejecta decelerated by a gas
+    (SURVEY.md 8(f) row f4); None: the paper's vacuum.
     """
     lib = _load()
     n = int(run_opts["n_photons"] if n_photons is None else n_photons)
@@ -135,7 +139,7 @@ def run(cloud: OracleCloud, run_opts: dict, *, n_photons: int | None = None, fir
     p_cum = np.ascontiguousarray(np.cumsum(cloud.p_class), dtype=np.float64)
     p_cum[-1] = 1.0
     omega0 = np.ascontiguousarray(cloud.omega0, dtype=np.float64)
-    T_edge = np.ascontiguousarray(cloud.T_edge, dtype=np.float64)
+    T_edge = np.ascontiguousarray(cloud.T_edge if gas is None else gas["T_edge"], dtype=np.float64)
     dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
     p = _Params()
     p.n_classes, p.K, p.n_depth = cloud.n_classes, phase.shape[1] - 1, T_edge.size - 1
@@ -171,6 +175,16 @@ def run(cloud: OracleCloud, run_opts: dict, *, n_photons: int | None = None, fir
     if launch_model and rng_mode != 0:
         raise ValueError("launch_model 1 (diffuse illumination, pins only) needs rng_mode 0")
     p.launch_model = int(launch_model)
+    if gas is not None:
+        if analytic_profile:
+            raise ValueError("the closed-form depth profile exists for the vacuum case only")
+        g_zeta = np.ascontiguousarray(gas["zeta_edge"], dtype=np.float64)
+        g_cum = np.ascontiguousarray(gas["class_cum"], dtype=np.float64)
+        g_L = np.ascontiguousarray(gas["L"], dtype=np.float64)
+        if g_zeta.size != T_edge.size or g_cum.shape != (T_edge.size - 1, cloud.n_classes) or g_L.size != cloud.n_classes:
+            raise ValueError("gas tables do not match the cloud")
+        keep += [g_zeta, g_cum, g_L]
+        p.gas, p.zeta_edge, p.class_cum, p.gas_L, p.t_snap = 1, dp(g_zeta), dp(g_cum), dp(g_L), float(gas["t"])
     hist = np.zeros(p.n_bins)
     hist2 = np.zeros(p.n_bins)
     st = _Stats()

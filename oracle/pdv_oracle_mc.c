@@ -75,6 +75,12 @@ typedef struct {
     int32_t launch_model;     /* 0: the paper's collimated beam, u = (0,0,-1) (reading R1); 1: diffuse (Lambertian) illumination of
                                * the cloud top, pdf of the polar cosine proportional to it -- used only by the invariance pin
                                * (mean-chord-length theorem), rng_mode 0 only */
+    /* ---- gas environment (readings R35-R38 of oracle/gas.py, NOT from the paper) ---- */
+    int32_t gas;              /* 1: T_edge belongs to the depth bins uniform in the height zeta above the free surface */
+    const double *zeta_edge;  /* [n_depth+1] heights of the bin edges, zeta_top ... 0 */
+    const double *class_cum;  /* [n_depth][n_classes] cumulative class hit probabilities inside each bin, last = 1 */
+    const double *gas_L;      /* [n_classes] drag length L_c = 4 rho0 d_c / (3 C_d rho_g); +inf: no drag */
+    double t_snap;            /* snapshot time t */
 } oracle_params;
 
 typedef struct {
@@ -223,6 +229,26 @@ static double velocity_at(const oracle_params *p, double T) {
     return p->v_max - (lo + frac) * dv;
 }
 
+/* Gas environment (R36, R37): the interaction at optical depth T lies in depth bin `lo` at height zeta (T linear in zeta inside
+ * the bin); the class is picked with the bin's own probabilities; the class-c particle found there moves with
+ * v_fs + (L_c/t)(1 - exp(-zeta/L_c)) -- the closed form of the drag law du/dt = -u^2/L_c (R35). */
+static double gas_interaction(const oracle_params *p, double T, double xi_class, int *c_out) {
+    int lo = 0, hi = p->n_depth;                   /* T_edge[lo] <= T < T_edge[hi] */
+    while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (p->T_edge[mid] <= T) lo = mid; else hi = mid;
+    }
+    double frac = (T - p->T_edge[lo]) / (p->T_edge[lo + 1] - p->T_edge[lo]);
+    double zeta = p->zeta_edge[lo] + frac * (p->zeta_edge[lo + 1] - p->zeta_edge[lo]);
+    const double *cum = p->class_cum + (size_t)lo * p->n_classes;
+    int c = 0;
+    while (c < p->n_classes - 1 && xi_class >= cum[c]) ++c;
+    *c_out = c;
+    double L = p->gas_L[c];
+    double u = isinf(L) ? zeta / p->t_snap : -(L / p->t_snap) * expm1(-zeta / L);
+    return p->v_fs + u;
+}
+
 static int pick_class(const oracle_params *p, double xi) {
     int c = 0;
     while (c < p->n_classes - 1 && xi >= p->p_cum[c]) ++c;
@@ -326,8 +352,9 @@ static void run_history(const oracle_params *p, uint64_t id, tally_t *ty, oracle
             n_refl += 1; ty->st.surface_reflections += 1;
         } else {                                   /* particle interaction at depth Tn */
             if (p->single_scatter_only && n_sc >= 1) { ty->st.truncated += w; fate = 4; break; }
-            v_here = velocity_at(p, Tn);
-            int c = pick_class(p, d.xi_class);
+            int c;
+            if (p->gas) v_here = gas_interaction(p, Tn, d.xi_class, &c);
+            else { v_here = velocity_at(p, Tn); c = pick_class(p, d.xi_class); }
             if (p->mode == 1) {
                 if (d.xi_absorb >= p->omega0[c]) { ty->st.absorbed_particles += w; fate = 2; w = 0.0;
                                                    ty->st.particle_events += 1; break; }
