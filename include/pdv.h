@@ -69,6 +69,16 @@ typedef struct {
                                     1: the closed form of the truncated Eq. 20,
                                        v = v_fs - (v_fs/beta) ln(E + (1 - E) T/tau_ext), E = exp(-beta (vmax_ratio - 1))
                                        (R26) -- profile_kind 0 only; no table error, one logarithm per event */
+    /* ---- gas environment.  The paper treats the vacuum only and names this case as future work in one
+     * sentence without an equation, so what follows is a reading that is NOT the paper's (R35-R38):
+     * the gas ahead of the free surface moves with it (velocity v_fs, density gas_density); a particle of diameter d feels the
+     * quasi-steady drag of a constant coefficient on its velocity u relative to the gas, du/dt = -u^2/L with
+     * L = 4 density d / (3 drag_coefficient gas_density), hence u(t) = u0/(1 + u0 t/L) and the height above the free surface
+     * zeta(t) = L ln(1 + u0 t/L).  Small particles stop first, the cloud sorts itself by size, and the spectrum depends on the
+     * snapshot time: pdv_mc_run builds the depth tables of every (cloud, snapshot) unit at run time. */
+    double gas_density;          /* rho_g, kg/m^3; 0: vacuum (the paper; every other field keeps its meaning and the run is bit-identical
+                                    to one without these two fields) */
+    double drag_coefficient;     /* C_d > 0 when gas_density > 0 (0.5 is typical of spheres at high Reynolds number) */
 } pdv_cloud_params;
 
 #define PDV_MAX_CLASSES 32
@@ -110,6 +120,16 @@ pdv_status pdv_cloud_get_info(const pdv_cloud *cloud, pdv_cloud_info *out);
  * T_edge: [n_depth_bins+1], T at velocity v_max - j (v_max - v_fs)/n_depth_bins. */
 pdv_status pdv_cloud_get_tables(const pdv_cloud *cloud, double *k_ext, double *k_sca, double *g, double *p_class,
                                 double *phase, double *T_edge);
+
+/* Host (double) depth tables of the (cloud, snapshot time t) unit of a cloud in a gas environment (gas_density > 0), as
+ * pdv_mc_run builds them (R36, R37): n = n_depth_bins bins uniform in the height zeta above the free surface.
+ *   zeta_edge [n+1]  heights of the bin edges, from the cloud top zeta_top(t) = max_c L_c ln(1 + u_max t / L_c) down to 0
+ *   T_edge    [n+1]  vertical optical depth from the top at the edges, 0 ... tau_ext (T linear in zeta inside a bin)
+ *   class_cum [n][n_classes]  cumulative probabilities that an interaction inside the bin hits class 0..c (last = 1)
+ *   drag_length [n_classes]   L_c
+ * Any pointer may be NULL to skip it.  PDV_E_INVALID for a vacuum cloud or t <= 0.  No device is needed. */
+pdv_status pdv_cloud_gas_tables(const pdv_cloud *cloud, double t, double *zeta_edge, double *T_edge, double *class_cum,
+                                double *drag_length);
 
 /* ---- Monte-Carlo run: PAPER.md section II.B steps (1)-(7) (174-183) ---------------------------------- */
 typedef struct {

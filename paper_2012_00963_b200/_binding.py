@@ -18,7 +18,7 @@ PDV_MAX_CLASSES = 32
 PDV_MAX_BINS = 8192
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
-           "pdv_cloud_get_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
+           "pdv_cloud_get_tables", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
            "pdv_last_launch_info", "pdv_last_error", "pdv_version")
 
 
@@ -36,7 +36,7 @@ class CloudParams(C.Structure):
                 ("m_re", C.c_double), ("m_im", C.c_double), ("wavelength", C.c_double),
                 ("surface_reflectivity", C.c_double), ("surface_model", C.c_int32),
                 ("n_phase_bins", C.c_int32), ("n_depth_bins", C.c_int32), ("phase_model", C.c_int32),
-                ("depth_model", C.c_int32)]
+                ("depth_model", C.c_int32), ("gas_density", C.c_double), ("drag_coefficient", C.c_double)]
 
 
 class CloudInfo(C.Structure):
@@ -93,6 +93,7 @@ def lib() -> C.CDLL:
         L.pdv_cloud_destroy.restype = None
         L.pdv_cloud_get_info.argtypes = [vp, C.POINTER(CloudInfo)]
         L.pdv_cloud_get_tables.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.pdv_cloud_gas_tables.argtypes = [vp, C.c_double, vp, vp, vp, vp]
         L.pdv_mc_run.argtypes = [C.POINTER(vp), C.c_int32, dp, C.c_int32, C.c_uint64, C.c_uint64, C.POINTER(RunOpts),
                                  vp, vp, vp, vp]
         L.pdv_mc_trace.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint64, C.POINTER(RunOpts), vp, vp, vp, vp, vp]
@@ -170,6 +171,14 @@ class Cloud:
                                                          ("k_ext", "k_sca", "g", "p_class", "phase", "T_edge")]))
         return out
 
+    def gas_tables(self, t: float) -> dict:
+        """Host depth tables of the (cloud, snapshot time t) unit of a cloud in a gas environment (pdv_cloud_gas_tables)."""
+        i = self.info()
+        nc, nd = i["n_classes"], i["n_depth_bins"]
+        out = dict(zeta_edge=np.zeros(nd + 1), T_edge=np.zeros(nd + 1), class_cum=np.zeros((nd, nc)), L=np.zeros(nc))
+        _check(lib().pdv_cloud_gas_tables(self.handle, float(t), *[out[k].ctypes.data for k in ("zeta_edge", "T_edge", "class_cum", "L")]))
+        return out
+
 
 def pdv_cloud_create(params: dict) -> Cloud:
     """params: a cloud dictionary as in pdv_workloads._cloud (SI units).  Either explicit `diameters` +
@@ -202,6 +211,8 @@ def pdv_cloud_create(params: dict) -> Cloud:
     p.n_phase_bins, p.n_depth_bins = int(params.get("n_phase_bins", 0)), int(params.get("n_depth_bins", 0))
     p.phase_model = int(params.get("phase_model", 0))
     p.depth_model = int(params.get("depth_model", 0))
+    p.gas_density = float(params.get("gas_density", 0.0))
+    p.drag_coefficient = float(params.get("drag_coefficient", 0.5 if p.gas_density > 0.0 else 0.0))
     h = C.c_void_p(None)
     _check(lib().pdv_cloud_create(C.byref(p), C.byref(h)))
     return Cloud(h.value)

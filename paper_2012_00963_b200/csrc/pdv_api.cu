@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <limits>
 #include <mutex>
 #include <new>
 #include <string>
@@ -63,22 +64,26 @@ uint32_t to_thr32(double p) {            // smallest integer t with t/2^32 >= p,
     return (uint32_t)v;
 }
 
-void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
+// Device image of a cloud (gu == nullptr: the paper's vacuum, depth rows in v/2) or of one (cloud, snapshot) unit in a gas
+// environment (gu: its tables; depth rows in the height zeta, per-bin class thresholds, per-class drag constants).
+void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasUnit *gu = nullptr) {
     const int nc = h.n_classes, K = h.K, nd = h.n_depth;
+    const std::vector<double> &T_src = gu ? gu->T_edge : h.T_edge;
     int steps = 0;
     while ((1 << steps) < nc) ++steps;
     const int n_pad = 1 << steps;
     // fp32 depth edges, T_0 = 0 at the cloud top ... T_nd = tau_ext at the free surface, non-decreasing
     std::vector<float> Tf(nd + 1);
-    for (int j = 0; j <= nd; ++j) Tf[j] = (float)h.T_edge[j];
+    for (int j = 0; j <= nd; ++j) Tf[j] = (float)T_src[j];
     Tf[0] = 0.f;
     for (int j = 1; j <= nd; ++j) if (Tf[j] < Tf[j - 1]) Tf[j] = Tf[j - 1];
     // depth rows (layout: pdv_device.h).  Half velocities: the Doppler update is  v~ += (mu' - mu) v/2  (Eq. 4).
     const double dv = (h.v_max - h.v_fs) / nd;
-    std::vector<float> slope(nd + 1, 0.f);                    // d(v/2)/dT inside bin j; 0 for an empty bin
+    std::vector<float> slope(nd + 1, 0.f);                    // d(v/2)/dT (gas: dzeta/dT) inside bin j; 0 for an empty bin
     for (int j = 0; j < nd; ++j) {
         const double dT = (double)Tf[j + 1] - (double)Tf[j];
-        slope[j] = dT > 0.0 ? (float)(-0.5 * dv / dT) : 0.f;
+        const double dy = gu ? gu->zeta_edge[j + 1] - gu->zeta_edge[j] : -0.5 * dv;
+        slope[j] = dT > 0.0 ? (float)(dy / dT) : 0.f;
     }
     // guide over (float bits >> shift): the coarsest shift for which no cell straddles two bin edges
     float t_min = 0.f;
@@ -153,6 +158,11 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     const uint32_t n_cg = nc > 1 ? 1u << (32 - cg_shift) : 16u;
     hd.off_cguide = (uint32_t)off; off = align16(off + n_cg);
     hd.cguide_shift = cg_shift;
+    if (gu) {
+        hd.gas = 1; hd.gas_steps = (uint32_t)steps;
+        hd.off_gthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * (size_t)nd * n_pad);
+        hd.off_gcls = (uint32_t)off; off = align16(off + sizeof(float) * 2 * n_pad);
+    }
     hd.blob_bytes = (uint32_t)off;
     hd.n_classes = nc; hd.K = K; hd.n_depth = nd; hd.n_guide = n_guide; hd.guide_base = base;
     hd.guide_shift = shift; hd.depth_bisect = bisect;
@@ -192,7 +202,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
     float *rows = reinterpret_cast<float *>(blob.data() + hd.off_rows);
     for (int j = 0; j < nd; ++j) {
         rows[4 * j + 0] = Tf[j + 1];
-        rows[4 * j + 1] = j + 1 == nd ? hd.vh_fs : (float)(0.5 * (h.v_max - (j + 1) * dv));
+        rows[4 * j + 1] = gu ? (float)gu->zeta_edge[j + 1] : (j + 1 == nd ? hd.vh_fs : (float)(0.5 * (h.v_max - (j + 1) * dv)));
         rows[4 * j + 2] = slope[j];
         rows[4 * j + 3] = slope[j + 1];
     }
@@ -206,6 +216,21 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob) {
         albt[c] = to_thr32(om);
     }
     std::memcpy(blob.data() + hd.off_guide, guide.data(), sizeof(uint16_t) * n_guide);
+    if (gu) {
+        uint32_t *gt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_gthr);
+        for (int j = 0; j < nd; ++j)
+            for (int c = 0; c < n_pad; ++c) {
+                double v = 4294967295.0;
+                if (c < nc - 1) v = std::ceil(gu->class_cum[(size_t)j * nc + c] * 4294967296.0 - 0.5);
+                gt[(size_t)j * n_pad + c] = v <= 0.0 ? 0u : (v >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)v);
+            }
+        float *gc = reinterpret_cast<float *>(blob.data() + hd.off_gcls);
+        for (int c = 0; c < n_pad; ++c) {
+            const double L = c < nc ? gu->L[c] : std::numeric_limits<double>::infinity();
+            gc[2 * c + 0] = std::isinf(L) ? (float)(0.5 / gu->t) : (float)(0.5 * L / gu->t);
+            gc[2 * c + 1] = std::isinf(L) ? 0.f : (float)(-1.0 / L);
+        }
+    }
     unsigned char *cg = blob.data() + hd.off_cguide;          // class guide (layout: pdv_device.h)
     for (uint32_t g = 0; nc > 1 && g < n_cg; ++g) {
         int below, inside;
@@ -395,6 +420,13 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
             odd = odd || hd.depth_bisect == 1u || hd.surface_model != 0u;
         }
         kv.dm = odd || (n_closed != 0 && n_closed != n_clouds) ? 2 : (n_closed ? 1 : 0);
+        bool any_gas = false;
+        for (int i = 0; i < n_clouds; ++i) any_gas = any_gas || clouds[i]->host.gas();
+        if (any_gas) {                 // gas units: their own instantiations (dm 3), vacuum clouds of the launch ride along with L = infinity
+            if (odd || n_closed) return fail(PDV_E_UNSUPPORTED, "a launch with a gas cloud supports neither single_scatter_only, pdv_mc_trace, launch_model 1, "
+                                                                "surface_model 1, depth_model 1 nor a depth table that needs bisection");
+            kv.dm = 3;
+        }
     }
 
     const DeviceInfo &di = device_info(device);
@@ -430,6 +462,15 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     return PDV_OK;
 }
 
+// Draws per pass of a unit (UnitDesc::draws_per_pass) from its estimated flights per history.
+uint32_t draws_per_pass(double flights, bool poly) {
+    // measured (profiles/README.md, round 2): config 2 (10 flights per history) and config 3 (20) lose 1 % / 7 % with 2 draws,
+    // config 5 (56 flights; estimated 139) gains 2 % with 2 and 2.4 % with 3, config 4 (its work is in the units of 50 ... 500
+    // flights) gains 1.4 % / 4.3 % / 5.2 % with 2 / 3 / 4
+    (void)poly;
+    return flights >= 150.0 ? 4u : flights >= 60.0 ? 3u : flights >= 35.0 ? 2u : 1u;
+}
+
 // Estimated flights (particle events + reflections + the exit flight) of one history in a cloud of vertical optical thickness
 // tau: only the RATIOS between the units of a launch matter (they place the blocks, see RunParams::block_start), and a wrong
 // estimate costs a few more unit visits, never a wrong result.  Measured on the configs of BASELINE.json: 4.9 (tau 1.25), 9.8
@@ -442,7 +483,7 @@ double estimated_flights(double tau, double mean_albedo, const pdv_run_opts *o) 
     return f;
 }
 
-pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, const uint32_t *unit_streams,
+pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *t_snap, int n_snap, const uint32_t *unit_streams,
                     uint64_t n_photons, uint64_t seed, const pdv_run_opts *o, double *hist, double *hist2,
                     pdv_run_stats *stats, pdv_trace_record *records, void *cuda_stream) {
     const int n_units = n_clouds * n_snap;
@@ -455,10 +496,33 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     int device = 0;
     CU(cudaGetDevice(&device), "cudaGetDevice");
     size_t max_blob = 0;
+    bool any_gas = false;
     for (int i = 0; i < n_clouds; ++i) {
         pdv_status s = ensure_on_device(clouds[i], device);
         if (s != PDV_OK) return s;
         max_blob = std::max(max_blob, clouds[i]->blob.size());
+        any_gas = any_gas || clouds[i]->host.gas();
+    }
+    // Gas environment (R38): the depth tables depend on the snapshot time, so every (cloud, snapshot) unit gets its
+    // own device image, built here and copied with the unit table
+    std::vector<unsigned char> gas_images;
+    std::vector<size_t> gas_off;
+    if (any_gas) {
+        if (!t_snap) return fail(PDV_E_UNSUPPORTED, "gas clouds need snapshot times (not available through pdv_mc_trace)");
+        max_blob = 0;
+        std::vector<unsigned char> img;
+        for (int i = 0; i < n_clouds; ++i)
+            for (int j = 0; j < n_snap; ++j) {
+                GasUnit gu;
+                build_gas_unit(clouds[i]->host, t_snap[j], gu);
+                build_blob(clouds[i]->host, img, &gu);
+                DevCloudHeader hd;
+                std::memcpy(&hd, img.data(), sizeof(hd));
+                if (hd.depth_bisect == 1u) return fail(PDV_E_UNSUPPORTED, "gas unit: depth table too irregular for the one-probe guide (use fewer n_depth_bins)");
+                gas_off.push_back(gas_images.size());
+                gas_images.insert(gas_images.end(), img.begin(), img.end());
+                max_blob = std::max(max_blob, img.size());
+            }
     }
     RunPlan plan;
     pdv_status s = make_plan(clouds, n_clouds, n_units, n_photons, seed, o, trace, device, plan, max_blob);
@@ -476,6 +540,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
     const size_t zero_bytes = off;
     const size_t o_units = off; off = align16(off + sizeof(UnitDesc) * (size_t)n_units);
     const size_t o_start = off; off = align16(off + sizeof(uint32_t) * (size_t)grid);
+    const size_t o_gas = off;   off = align16(off + gas_images.size());
     const size_t table_bytes = off - o_units;
     const size_t o_oh = off;    off = align16(off + 8 * nb * n_units);
     const size_t o_oh2 = off;   off = align16(off + (hist2 ? 8 * nb * n_units : 0));
@@ -508,12 +573,13 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
             for (int j = 0; j < n_snap; ++j) {
                 const size_t k = (size_t)i * n_snap + j;
                 UnitDesc &u = units[k];
-                u.cloud_blob = clouds[i]->d_blob;
+                u.cloud_blob = any_gas ? ws + o_gas + gas_off[k] : clouds[i]->d_blob;
                 u.stream = unit_streams ? unit_streams[k] : (uint32_t)k;
                 // threads expected on this unit: its share of the grid, at least one block
                 const double threads = std::max(1.0, cost[k] / total * grid) * plan.shape.block;
                 u.chunk = (uint32_t)std::min(std::max(std::floor((double)n_photons / (threads * 4.0)), 1.0), 128.0);
                 u.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
+                u.draws_per_pass = draws_per_pass(cost[k], clouds[i]->host.n_classes > 1);
             }
         for (int k = 0; k < n_units; ++k) units[k].visit = ord[k];
         double cum = 0.0;                                          // cost line: unit ord[k] covers [cum, cum + cost)
@@ -524,6 +590,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, co
             block_start[b] = (uint32_t)k;
         }
     }
+    if (any_gas) std::memcpy(table.data() + (o_gas - o_units), gas_images.data(), gas_images.size());
     pdv_trace_record *d_trace = nullptr;
     if (trace && n_photons) CU(cudaMalloc(&d_trace, sizeof(pdv_trace_record) * n_photons), "cudaMalloc(trace)");
     auto cleanup = [&]() { if (d_trace) cudaFree(d_trace); };
@@ -667,6 +734,20 @@ pdv_status pdv_cloud_get_tables(const pdv_cloud *c, double *k_ext, double *k_sca
     return PDV_OK;
 }
 
+pdv_status pdv_cloud_gas_tables(const pdv_cloud *c, double t, double *zeta_edge, double *T_edge, double *class_cum, double *drag_length) {
+    g_err.clear();
+    if (!c) return fail(PDV_E_INVALID, "cloud is NULL");
+    if (!c->host.gas()) return fail(PDV_E_INVALID, "the cloud is in vacuum (gas_density = 0): it has no per-snapshot tables");
+    if (!(t > 0.0) || !std::isfinite(t)) return fail(PDV_E_INVALID, "t must be > 0");
+    GasUnit gu;
+    build_gas_unit(c->host, t, gu);
+    if (zeta_edge) std::memcpy(zeta_edge, gu.zeta_edge.data(), 8 * gu.zeta_edge.size());
+    if (T_edge) std::memcpy(T_edge, gu.T_edge.data(), 8 * gu.T_edge.size());
+    if (class_cum) std::memcpy(class_cum, gu.class_cum.data(), 8 * gu.class_cum.size());
+    if (drag_length) std::memcpy(drag_length, gu.L.data(), 8 * gu.L.size());
+    return PDV_OK;
+}
+
 pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const double *t_snap, int32_t n_snap,
                       uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
                       double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream) {
@@ -681,7 +762,7 @@ pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const do
     if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
     if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
     if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
-    return run_impl(clouds, n_clouds, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
+    return run_impl(clouds, n_clouds, t_snap, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
 }
 
 pdv_status pdv_mc_trace(const pdv_cloud *cloud, uint32_t unit, uint64_t n_photons, uint64_t seed,
@@ -694,7 +775,7 @@ pdv_status pdv_mc_trace(const pdv_cloud *cloud, uint32_t unit, uint64_t n_photon
     if (opts->output_on_device) return fail(PDV_E_INVALID, "pdv_mc_trace writes host buffers only");
     if (n_photons > (1ull << 28)) return fail(PDV_E_INVALID, "pdv_mc_trace: at most 2^28 histories");
     const pdv_cloud *cl[1] = {cloud};
-    return run_impl(cl, 1, 1, &unit, n_photons, seed, opts, hist, hist2, stats, records, cuda_stream);
+    return run_impl(cl, 1, nullptr, 1, &unit, n_photons, seed, opts, hist, hist2, stats, records, cuda_stream);
 }
 
 pdv_status pdv_spectrogram(const double *hist, int32_t n_snap, int32_t n_bins, uint64_t n_photons,

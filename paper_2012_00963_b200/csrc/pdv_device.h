@@ -72,6 +72,14 @@ struct DevCloudHeader {
     uint32_t off_cguide;       // class guide: 2^(32 - cguide_shift) bytes, see above
     float an_c0, an_c1, an_c2, an_c3;   // closed-form depth model (pdv_cloud_params.depth_model 1)
     uint32_t cguide_shift;     // 24 ... 20
+    // Gas environment (R35-R37; one image per (cloud, snapshot) unit): the depth rows hold the HEIGHT zeta above the
+    // free surface instead of v/2 (y = zeta_{j+1}, z / w = dzeta/dT inside bins j / j+1), bins uniform in zeta;
+    // gas thresholds u32 [n_depth][n_pad]: row j = cumulative class pick probabilities inside bin j as 32-bit thresholds
+    // (c = #{k : thr[j][k] <= cw}, padded with 0xffffffff to n_pad = 2^gas_steps entries, found by gas_steps bisection steps);
+    // gas class constants float2 [n_pad]: (L_c / (2 t), -1 / L_c), or (1 / (2 t), 0) for a class without drag, so that half the
+    // class-c particle velocity at zeta is  v_fs/2 + x (1 - e^{y zeta})   resp.   v_fs/2 + x zeta.
+    uint32_t gas;              // 1: this image is a gas unit
+    uint32_t off_gthr, off_gcls, gas_steps;
     uint32_t pad[1];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
@@ -84,6 +92,12 @@ struct UnitDesc {
     // ids at a time; chunk_per_remaining = 1 / (2 * threads expected to work on the unit)
     uint32_t chunk;
     float chunk_per_remaining;
+    // Random draws (Philox blocks of a one-class cloud = 2 flights each, block pairs of a polydisperse one = 3 flights each)
+    // a lane flies between two end-of-history passes of its warp.  1 for short histories; more when histories are long: the
+    // end-of-history pass then runs at one or two lanes, and running it less often costs fewer issue slots than the lanes
+    // that wait for it.
+    uint32_t draws_per_pass;
+    uint32_t pad;
 };
 
 struct RunParams {

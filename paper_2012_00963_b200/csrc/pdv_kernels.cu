@@ -26,11 +26,9 @@ __shared__ unsigned int s_dbg[8];
 #define PDV_BOUND(cat, idx, limit) do { } while (0)
 #endif
 
-#ifndef PDV_BLOCKS_MONO
-#define PDV_BLOCKS_MONO 1
-#endif
-#ifndef PDV_GROUPS_POLY
-#define PDV_GROUPS_POLY 1
+// experiment builds only: force UnitDesc::draws_per_pass
+#ifndef PDV_FORCE_DRAWS
+#define PDV_FORCE_DRAWS 0
 #endif
 // Register budget of transport_kernel: PDV_LB_THREADS x PDV_LB_BLOCKS resident threads per SM (pdv_device.h).
 namespace pdv {
@@ -97,6 +95,10 @@ __device__ __forceinline__ void smem_add64(unsigned long long *p, uint32_t v) {
 }
 
 struct CloudView {               // per-unit scalars and shared-memory table pointers
+    const uint32_t *gthr;        // gas units: per-bin class thresholds [n_depth][1 << gas_steps]
+    const float2 *gcls;          // gas units: per-class (L / 2t, -1 / L)
+    uint32_t gas_steps;
+    float vh_fs;
     const float2 *phase;
     const float4 *rows;
     const uint32_t *thr, *albthr;
@@ -130,6 +132,26 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
     PDV_BOUND(1, j, cv.n_depth);
     const float4 r = cv.rows[j];
     return fmaf(Tc - r.x, Tc < r.x ? r.z : r.w, r.y);
+}
+
+// Gas unit (R35-R37): height zeta above the free surface at vertical optical depth Tc and the depth bin it lies in.
+// Same one-probe rows as depth_half_velocity (y = zeta at the lower edge of bin j, z / w = dzeta/dT in bins j / j+1).
+__device__ __forceinline__ float gas_height(const CloudView &cv, float Tc, uint32_t &bin) {
+    const uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base);
+    const uint32_t j = cv.guide[cell];
+    const float4 r = cv.rows[j];
+    const bool lower = !(Tc < r.x);
+    bin = min(j + (lower ? 1u : 0u), cv.n_depth - 1u);
+    return fmaf(Tc - r.x, lower ? r.w : r.z, r.y);
+}
+// half the velocity RELATIVE to the free surface of the class particle found at height zeta:  (L/2t)(1 - e^{-zeta/L}), the closed
+// form of the drag law du/dt = -u^2/L; g = (L/2t, -1/L), or (1/2t, 0) for a class without drag.  1 - e^x by its series for
+// |x| < 1/16 (fp32 cancellation), by ex2 otherwise.
+__device__ __forceinline__ float gas_half_velocity(float2 g, float zeta) {
+    const float x = g.y * zeta;
+    const float series = x * fmaf(x, fmaf(x, fmaf(x, 1.f / 24.f, 1.f / 6.f), 0.5f), 1.f);       // e^x - 1
+    const float em1 = fabsf(x) < 0.0625f ? series : exp2f(x * 1.4426950408889634f) - 1.f;
+    return g.y == 0.f ? g.x * zeta : -g.x * em1;
 }
 
 // ---- rare paths kept out of line: the flight loop stays small, and the compiler cannot fold their conditions into the
@@ -237,9 +259,13 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
             cv.depth_bisect = h->depth_bisect; cv.cg_shift = h->cguide_shift;
+            cv.gthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_gthr);
+            cv.gcls = reinterpret_cast<const float2 *>(s_blob + h->off_gcls);
+            cv.gas_steps = h->gas_steps; cv.vh_fs = h->vh_fs;
             cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
+        const uint32_t draws = PDV_FORCE_DRAWS ? PDV_FORCE_DRAWS : ud.draws_per_pass;
         const float albedo0 = cv.albedo[0];               // monodisperse: the only class
         const uint32_t albthr0 = cv.albthr[0];
 
@@ -248,6 +274,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         //   1  closed form of the exponential profile (pdv_cloud_params.depth_model 1): v/2 = an0 + an1 lg2(an2 + an3 T),
         //      exactly v_fs / 2 at T = tau_ext
         //   2  general: per unit, any of guide probe / bisection of a pathological table / closed form, either surface law
+        //   3  gas environment (row f4): every unit carries its own image; depth rows give the height, class pick per depth
+        //      bin, velocity from the closed form of the drag law; the paper's surface law
         float an0 = 0.f, an1 = 0.f, an2 = 1.f, an3 = 0.f;
         bool closed = DM == 1;
         if (DM != 0) {
@@ -352,12 +380,24 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             // ---------------- interaction at depth T = min(T', tau_ext): particle (steps (4)-(5)) or free surface ------
             T = fminf(Tn, cv.tau_ext);
             float vh;                                         // = v_fs / 2 at the surface
-            if (DM == 1 || (DM == 2 && closed)) vh = fmaf(an1, fast_lg2(fmaf(an3, T, an2)), an0);
-            else vh = depth_half_velocity<DM == 2>(cv, T);
             uint32_t c = 0u;
             float alb = albedo0;
             uint32_t albt = albthr0;
-            if (POLY) {
+            if (DM == 3) {
+                // gas unit: height of the event, class by the probabilities of its depth bin (bisection of the bin's
+                // thresholds), velocity of that class at that height
+                uint32_t bin;
+                const float zeta = gas_height(cv, T, bin);
+                if (POLY) {
+                    const uint32_t *t = cv.gthr + (bin << cv.gas_steps);
+                    for (uint32_t st = 1u << cv.gas_steps >> 1; st > 0u; st >>= 1) c += t[c + st - 1u] <= cw ? st : 0u;
+                    c = min(c, cv.n_classes - 1u);
+                    if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
+                }
+                vh = cv.vh_fs + gas_half_velocity(cv.gcls[c], zeta);
+            } else if (DM == 1 || (DM == 2 && closed)) vh = fmaf(an1, fast_lg2(fmaf(an3, T, an2)), an0);
+            else vh = depth_half_velocity<DM == 2>(cv, T);
+            if (POLY && DM != 3) {
                 // c = #{j : thr[j] <= cw} through the class guide (pdv_device.h); thr is padded with 0xffffffff
                 const uint32_t e = cv.cguide[cw >> cv.cg_shift];
                 c = e & 0x7Fu;
@@ -451,11 +491,11 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 // word made of their low bytes (a.byte0, b.byte0, a.byte1, a.byte2 from the top: neither the 23 path bits nor
                 // the 22 phase bits reach the two leading ones) and, with several size classes, a class word.
                 // One class: one Philox4x32-10 block feeds two flights.  Several classes: two blocks feed three flights.
-                // A pass flies PDV_BLOCKS_MONO blocks / PDV_GROUPS_POLY groups: the end-of-history code below runs at the few
+                // A pass flies `draws` blocks / groups (UnitDesc::draws_per_pass: 1 unless histories are long): the end-of-history code below runs at the few
                 // lanes whose history ended, so it is entered once per several flights; those lanes wait meanwhile ------
                 if (POLY) {
 #pragma unroll 1
-                    for (int grp = 0; grp < PDV_GROUPS_POLY && fate == F_NONE; ++grp) {
+                    for (uint32_t grp = 0; grp < draws && fate == F_NONE; ++grp) {
                         const uint32_t b2 = 2u * (nfl / 3u);      // nfl is a multiple of 3 here: blocks b2 and b2 + 1
                         uint32_t w0, w1, w2, w3, w4, w5, w6, w7, ya0 = 0u, ya1 = 0u, ya2 = 0u, ya3 = 0u, yr0 = 0u, yr1 = 0u, yr2 = 0u, yr3 = 0u;
                         philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2, s_keys, w0, w1, w2, w3);
@@ -473,7 +513,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     }
                 } else {
 #pragma unroll 1
-                    for (int blk = 0; blk < PDV_BLOCKS_MONO && fate == F_NONE; ++blk) {
+                    for (uint32_t blk = 0; blk < draws && fate == F_NONE; ++blk) {
                         const uint32_t draw = nfl >> 1;
                         uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
                         philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
@@ -573,7 +613,8 @@ static cudaError_t launch_dm(int dm, const RunParams &rp, LaunchShape s, cudaStr
     if constexpr (C || D) {
         return launch_t<A, B, C, D, E, 2>(rp, s, st);
     } else {
-        return dm == 0 ? launch_t<A, B, C, D, E, 0>(rp, s, st) : dm == 1 ? launch_t<A, B, C, D, E, 1>(rp, s, st) : launch_t<A, B, C, D, E, 2>(rp, s, st);
+        return dm == 0 ? launch_t<A, B, C, D, E, 0>(rp, s, st) : dm == 1 ? launch_t<A, B, C, D, E, 1>(rp, s, st)
+             : dm == 3 ? launch_t<A, B, C, D, E, 3>(rp, s, st) : launch_t<A, B, C, D, E, 2>(rp, s, st);
     }
 }
 template <bool A, bool B, bool C, bool D, bool E>
@@ -581,7 +622,8 @@ static cudaError_t occ_dm(int dm, int block, int smem, int *out) {
     if constexpr (C || D) {
         return occ_t<A, B, C, D, E, 2>(block, smem, out);
     } else {
-        return dm == 0 ? occ_t<A, B, C, D, E, 0>(block, smem, out) : dm == 1 ? occ_t<A, B, C, D, E, 1>(block, smem, out) : occ_t<A, B, C, D, E, 2>(block, smem, out);
+        return dm == 0 ? occ_t<A, B, C, D, E, 0>(block, smem, out) : dm == 1 ? occ_t<A, B, C, D, E, 1>(block, smem, out)
+             : dm == 3 ? occ_t<A, B, C, D, E, 3>(block, smem, out) : occ_t<A, B, C, D, E, 2>(block, smem, out);
     }
 }
 #define PDV_D0(FN, A, B, C, D, ...) (v.roulette ? FN<A, B, C, D, true>(v.dm, __VA_ARGS__) : FN<A, B, C, D, false>(v.dm, __VA_ARGS__))

@@ -12,6 +12,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <limits>
 #include <complex>
 #include <thread>
 #include <utility>
@@ -226,6 +227,9 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     if (p.phase_model != 0 && p.phase_model != 1) return bad("phase_model must be 0 or 1");
     if (p.depth_model != 0 && p.depth_model != 1) return bad("depth_model must be 0 or 1");
     if (p.depth_model == 1 && p.profile_kind != 0) return bad("depth_model 1 (closed form) needs the exponential profile (profile_kind 0)");
+    if (!(p.gas_density >= 0.0) || !std::isfinite(p.gas_density)) return bad("gas_density must be >= 0");
+    if (p.gas_density > 0.0 && !(p.drag_coefficient > 0.0 && std::isfinite(p.drag_coefficient))) return bad("drag_coefficient must be > 0 in a gas");
+    if (p.gas_density > 0.0 && p.depth_model == 1) return bad("depth_model 1 (closed form) exists for the vacuum only");
     const int K = p.n_phase_bins == 0 ? 1024 : p.n_phase_bins;
     const int nd = p.n_depth_bins == 0 ? 1024 : p.n_depth_bins;
     if (!is_pow2(K) || K < 16 || K > 4096) return bad("n_phase_bins must be a power of two in [16, 4096]");
@@ -250,6 +254,8 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     h.v_fs = p.v_fs; h.v_max = p.vmax_ratio * p.v_fs; h.R = p.surface_reflectivity; h.surface_model = p.surface_model;
     h.m_re = p.m_re; h.m_im = p.m_im; h.wavelength = p.wavelength; h.phase_model = p.phase_model;
     h.depth_model = p.depth_model; h.beta = p.profile_kind == 0 ? p.beta : 0.0;
+    h.gas_density = p.gas_density; h.drag_coefficient = p.drag_coefficient; h.density = p.density; h.profile_kind = p.profile_kind;
+    if (p.profile_kind == 1) { h.prof_v.assign(p.prof_v, p.prof_v + p.n_prof); h.prof_cum.assign(p.prof_cum_mass, p.prof_cum_mass + p.n_prof); }
     h.diameter.assign(p.diameter, p.diameter + p.n_classes);
     h.weight.resize(p.n_classes);
     for (int c = 0; c < p.n_classes; ++c) h.weight[c] = p.number_weight[c] / wsum;
@@ -328,6 +334,65 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     for (int j = 1; j <= nd; ++j) if (h.T_edge[j] < h.T_edge[j - 1]) h.T_edge[j] = h.T_edge[j - 1];
     out = std::move(h);
     return PDV_OK;
+}
+
+// Fraction of the ejecta mass whose ejection velocity exceeds v0 (Eq. 20 truncated to [v_fs, v_max] and renormalised, or the
+// tabulated profile): 1 at v_fs, 0 at v_max and above.
+static double mass_fraction_above(const HostCloud &h, double v0) {
+    if (v0 >= h.v_max) return 0.0;
+    if (v0 <= h.v_fs) return 1.0;
+    if (h.profile_kind == 0) {
+        const double bv = h.beta / h.v_fs;
+        return std::expm1(bv * (h.v_max - v0)) / std::expm1(bv * (h.v_max - h.v_fs));
+    }
+    const int n = (int)h.prof_v.size();
+    const double v = std::min(std::max(v0, h.prof_v[0]), h.prof_v[n - 1]);
+    int seg = 0;
+    while (seg < n - 2 && h.prof_v[seg + 1] <= v) ++seg;
+    const double f = (v - h.prof_v[seg]) / (h.prof_v[seg + 1] - h.prof_v[seg]);
+    const double cm = h.prof_cum[seg] + f * (h.prof_cum[seg + 1] - h.prof_cum[seg]);
+    return (h.prof_cum[n - 1] - cm) / (h.prof_cum[n - 1] - h.prof_cum[0]);
+}
+
+// Gas environment (R35-R37).  Class c (drag length L_c) at time t: a particle ejected with relative velocity u0 sits
+// at zeta = L_c ln(1 + u0 t/L_c); those above zeta have u0 > (L_c/t)(e^{zeta/L_c} - 1), so the class carries the optical depth
+// tau_ext P_c mass_fraction_above(v_fs + u0_c(zeta)) above that height.
+void build_gas_unit(const HostCloud &h, double t, GasUnit &out) {
+    const int nc = h.n_classes, nd = h.n_depth;
+    const double u_max = h.v_max - h.v_fs, inf = std::numeric_limits<double>::infinity();
+    out.t = t;
+    out.L.resize(nc);
+    double top = 0.0;
+    for (int c = 0; c < nc; ++c) {
+        out.L[c] = h.gas() ? 4.0 * h.density * h.diameter[c] / (3.0 * h.drag_coefficient * h.gas_density) : inf;
+        const double z = std::isinf(out.L[c]) ? u_max * t : out.L[c] * std::log1p(u_max * t / out.L[c]);
+        top = std::max(top, z);
+    }
+    out.zeta_edge.resize(nd + 1); out.T_edge.resize(nd + 1); out.class_cum.assign((size_t)nd * nc, 0.0);
+    std::vector<double> prev(nc, 0.0), cur(nc);
+    for (int j = 0; j <= nd; ++j) {
+        const double z = j == nd ? 0.0 : top * (1.0 - (double)j / nd);
+        out.zeta_edge[j] = z;
+        double T = 0.0;
+        for (int c = 0; c < nc; ++c) {
+            const double u0 = std::isinf(out.L[c]) ? z / t : (out.L[c] / t) * std::expm1(z / out.L[c]);
+            cur[c] = j == nd ? h.tau_ext * h.p_class[c] : h.tau_ext * h.p_class[c] * mass_fraction_above(h, h.v_fs + u0);
+            T += cur[c];
+        }
+        out.T_edge[j] = j == 0 ? 0.0 : T;
+        if (j > 0) {
+            if (out.T_edge[j] < out.T_edge[j - 1]) out.T_edge[j] = out.T_edge[j - 1];
+            double dT = 0.0;
+            for (int c = 0; c < nc; ++c) dT += cur[c] - prev[c];
+            double cum = 0.0;
+            for (int c = 0; c < nc; ++c) {
+                cum += dT > 0.0 ? (cur[c] - prev[c]) / dT : h.p_class[c];
+                out.class_cum[(size_t)(j - 1) * nc + c] = c == nc - 1 ? 1.0 : cum;
+            }
+        }
+        prev = cur;
+    }
+    out.T_edge[nd] = std::max(out.T_edge[nd - 1], h.tau_ext);
 }
 
 }  // namespace pdv

@@ -22,7 +22,21 @@ struct HostCloud {
     double beta = 0;
     double m_re = 0, m_im = 0, wavelength = 0;       // kept for pdv_phase_sampling_check
     int phase_model = 0;
+    // gas environment (pdv_cloud_params.gas_density > 0; R35-R38): what the per-snapshot tables are built from
+    double gas_density = 0, drag_coefficient = 0, density = 0;
+    int profile_kind = 0;
+    std::vector<double> prof_v, prof_cum;            // profile_kind 1
+    bool gas() const { return gas_density > 0.0; }
 };
+
+// Depth tables of one (cloud, snapshot) unit in a gas environment: bins uniform in the height zeta above the free surface.
+struct GasUnit {
+    std::vector<double> zeta_edge, T_edge;           // [n_depth+1]: zeta_top ... 0, 0 ... tau_ext
+    std::vector<double> class_cum;                   // [n_depth][n_classes]
+    std::vector<double> L;                           // [n_classes] drag lengths (infinity: no drag)
+    double t = 0;
+};
+void build_gas_unit(const HostCloud &h, double t, GasUnit &out);
 
 // Mie coefficients a_n, b_n (n = 1..n_max) of a homogeneous sphere, size parameter x, relative index m.
 void mie_coefficients(double x, double m_re, double m_im, std::vector<double> &a_re, std::vector<double> &a_im,

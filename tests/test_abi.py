@@ -146,3 +146,22 @@ def test_product_does_not_import_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", src, re.M), f
                 assert "pdv_oracle" not in src and "oracle/" not in src.replace("shares nothing with oracle/", ""), f
+
+
+@pytest.mark.parametrize("idx,n_depth", [(1, 1024), (2, 256)])
+def test_host_gas_tables_agree_with_the_oracle(idx, n_depth):
+    """Row f4 (R35-R37): the product's per-snapshot depth tables of a cloud in a gas environment (C++,
+    csrc/pdv_optics.cpp::build_gas_unit) against the oracle's (numpy, oracle/gas.py) -- two implementations of the same
+    reading, no shared code.  No GPU needed."""
+    from oracle import gas as ogas
+    params = dict(W.config(idx)["clouds"][0], gas_density=5.0, drag_coefficient=0.5, n_depth_bins=n_depth)
+    c = P.pdv_cloud_create(params)
+    oc = ocloud.build_cloud(params)
+    for t in (0.7e-6, 9e-6):
+        a, b = c.gas_tables(t), ogas.build_tables(oc, params, t, n_depth)
+        assert np.allclose(a["zeta_edge"], b["zeta_edge"], rtol=1e-12, atol=1e-15 * b["zeta_edge"][0])
+        assert np.allclose(a["T_edge"], b["T_edge"], rtol=0, atol=1e-12 * oc.tau_ext)
+        assert np.allclose(a["class_cum"], b["class_cum"], rtol=0, atol=1e-9)
+        assert np.allclose(a["L"], b["L"], rtol=1e-14)
+    with pytest.raises(P.PdvError):                      # a vacuum cloud has no per-snapshot tables
+        P.pdv_cloud_create(W.config(idx)["clouds"][0]).gas_tables(1e-6)
