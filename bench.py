@@ -317,7 +317,7 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
         dist.all_reduce(e2e_c, op=dist.ReduceOp.SUM)
     blob_bytes = max(info["smem_bytes"] - 16 * nb, 0)                           # largest cloud image staged per block
-    h2d = nc * blob_bytes + 32 * n_units + 4 * info["grid"] + 8 * n_units_job * nb   # tables + unit table + block starts + hist (spectrogram)
+    h2d = nc * blob_bytes + 24 * n_units + 4 * info["grid"] + 8 * n_units_job * nb   # tables + unit table + block starts + hist (spectrogram)
     d2h = 2 * 8 * n_units * nb + n_units * P.STATS_DTYPE.itemsize + 4 * n_units_job * nb
     for c in clouds:
         c.destroy()

@@ -380,6 +380,18 @@ pdv_status check_opts(const pdv_run_opts *o) {
     return PDV_OK;
 }
 
+// Estimated flights (particle events + reflections + the exit flight) of one history in a cloud of vertical optical thickness
+// tau: only the RATIOS between the units of a launch matter (they place the blocks, see RunParams::block_start), and a wrong
+// estimate costs a few more unit visits, never a wrong result.  Measured on the configs of BASELINE.json: 4.9 (tau 1.25), 9.8
+// (1.87), 20 (4.1), 45 (9.3), 92 (18.7) -- the mean path of a slab grows linearly with its thickness.
+double estimated_flights(double tau, double mean_albedo, const pdv_run_opts *o) {
+    double f = 2.3 + 4.8 * tau;
+    if (o->max_events > 0) { const double m = 1.25 * o->max_events; f = m * (1.0 - std::exp(-f / m)); }
+    if (o->mode == 1) f = 1.0 / (1.0 / f + std::max(0.0, 1.0 - mean_albedo));      // analog histories end by absorption
+    if (o->single_scatter_only) f = std::min(f, 3.0);
+    return f;
+}
+
 // Fills the run parameters and the launch shape.  `ws` layout: next_id | hist | hist2 | stats | units.
 pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, uint64_t n_photons, uint64_t seed,
                      const pdv_run_opts *o, bool trace, int device, RunPlan &plan, size_t max_blob) {
@@ -408,6 +420,17 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     kv.sso = o->single_scatter_only != 0;
     kv.trace = trace;
     kv.roulette = o->max_events > 0;
+    {   // long histories?  cost-weighted mean of the estimated flights per history over the clouds of the launch
+        double sum = 0.0, sum2 = 0.0;
+        for (int i = 0; i < n_clouds; ++i) {
+            const HostCloud &h = clouds[i]->host;
+            double om = 0.0;
+            for (int c = 0; c < h.n_classes; ++c) om += h.p_class[c] * h.k_sca[c] / h.k_ext[c];
+            const double f = estimated_flights(h.tau_ext, om, o);
+            sum += f; sum2 += f * f;
+        }
+        kv.long_hist = sum > 0.0 && sum2 / sum >= 45.0;
+    }
     // dm 0: every cloud uses the one-probe depth table and the paper's surface law; 1: every cloud uses the closed-form
     // depth model and the paper's surface law; 2 (general kernel): anything else, decided per unit at run time
     {
@@ -436,7 +459,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         return fail(PDV_E_UNSUPPORTED, "cloud tables + histogram exceed the shared memory of one block");
     // 1024 resident threads per SM (64 registers each): two blocks of 512 when their shared memory fits twice, else one of 1024
     int block = o->threads_per_block, per_sm = 0;
-    // polydisperse clouds: one block of PDV_LB_THREADS_POLY threads per SM (80 registers each), see pdv_device.h
+    // polydisperse clouds: their tables leave room for one block per SM: PDV_LB_THREADS_POLY threads (pdv_device.h)
     if (kv.poly) block = block == 0 ? PDV_LB_THREADS_POLY : std::min(block, PDV_LB_THREADS_POLY);
     if (block == 0) block = 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024 ? 512 : 1024;
     {
@@ -445,7 +468,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         static std::vector<std::pair<Key, int>> cache;       // occupancy queries are not free either
         std::lock_guard<std::mutex> lk(mu);
         for (const auto &e : cache)
-            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.dm == kv.dm &&
+            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.dm == kv.dm && e.first.v.long_hist == kv.long_hist &&
                 e.first.block == block && e.first.smem == smem && e.first.device == device) { per_sm = e.second; break; }
         if (per_sm == 0) {
             CU(transport_max_blocks_per_sm(kv, block, smem, &per_sm), "occupancy query");
@@ -460,27 +483,6 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     if (useful < grid) grid = std::max(1LL, useful);
     plan.shape.grid = (int)grid; plan.shape.block = block; plan.shape.smem = smem;
     return PDV_OK;
-}
-
-// Draws per pass of a unit (UnitDesc::draws_per_pass) from its estimated flights per history.
-uint32_t draws_per_pass(double flights, bool poly) {
-    // measured (profiles/README.md, round 2): config 2 (10 flights per history) and config 3 (20) lose 1 % / 7 % with 2 draws,
-    // config 5 (56 flights; estimated 139) gains 2 % with 2 and 2.4 % with 3, config 4 (its work is in the units of 50 ... 500
-    // flights) gains 1.4 % / 4.3 % / 5.2 % with 2 / 3 / 4
-    (void)poly;
-    return flights >= 150.0 ? 4u : flights >= 60.0 ? 3u : flights >= 35.0 ? 2u : 1u;
-}
-
-// Estimated flights (particle events + reflections + the exit flight) of one history in a cloud of vertical optical thickness
-// tau: only the RATIOS between the units of a launch matter (they place the blocks, see RunParams::block_start), and a wrong
-// estimate costs a few more unit visits, never a wrong result.  Measured on the configs of BASELINE.json: 4.9 (tau 1.25), 9.8
-// (1.87), 20 (4.1), 45 (9.3), 92 (18.7) -- the mean path of a slab grows linearly with its thickness.
-double estimated_flights(double tau, double mean_albedo, const pdv_run_opts *o) {
-    double f = 2.3 + 4.8 * tau;
-    if (o->max_events > 0) { const double m = 1.25 * o->max_events; f = m * (1.0 - std::exp(-f / m)); }
-    if (o->mode == 1) f = 1.0 / (1.0 / f + std::max(0.0, 1.0 - mean_albedo));      // analog histories end by absorption
-    if (o->single_scatter_only) f = std::min(f, 3.0);
-    return f;
 }
 
 pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *t_snap, int n_snap, const uint32_t *unit_streams,
@@ -579,7 +581,6 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *
                 const double threads = std::max(1.0, cost[k] / total * grid) * plan.shape.block;
                 u.chunk = (uint32_t)std::min(std::max(std::floor((double)n_photons / (threads * 4.0)), 1.0), 128.0);
                 u.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
-                u.draws_per_pass = draws_per_pass(cost[k], clouds[i]->host.n_classes > 1);
             }
         for (int k = 0; k < n_units; ++k) units[k].visit = ord[k];
         double cum = 0.0;                                          // cost line: unit ord[k] covers [cum, cum + cost)

@@ -7,13 +7,16 @@
 
 // transport_kernel is compiled for PDV_LB_THREADS threads per block at most and PDV_LB_BLOCKS resident blocks per SM
 // (its register budget = 65536 / (PDV_LB_THREADS * PDV_LB_BLOCKS)).  The polydisperse instantiations, whose tables leave room
-// for one block per SM anyway, are compiled for PDV_LB_THREADS_POLY threads: 80 registers instead of 64 with spills; measured
-// 1024 / 896 / 768 / 640 threads on config 3: 1.45 / 1.48 / 1.52 / 1.44e11 events/s.
+// for one block per SM anyway, are compiled for PDV_LB_THREADS_POLY threads.  Round 1 (kernel v10, 80 registers): 1024 / 896 /
+// 768 / 640 threads on config 3: 1.45 / 1.48 / 1.52 / 1.44e11 events/s.  Round 2 (76 registers after the per-history bookkeeping
+// went; it now fits 64 registers without a spill): 768 / 896 / 960 / 1024 threads: config 5 280.7 / 276.4 / 275.0 / 273.1 ms,
+// Figs. 13-15 sweep (one draw per pass) 75.6 / 74.2 / 74.3 / 73.4 ms, config 3 at 4e6 photons per snapshot 76.4 / 75.7 / 75.5 /
+// 74.9 ms -- 1024 threads = 32 warps per SM, as for one class.
 #ifndef PDV_LB_THREADS
 #define PDV_LB_THREADS 1024
 #endif
 #ifndef PDV_LB_THREADS_POLY
-#define PDV_LB_THREADS_POLY 768
+#define PDV_LB_THREADS_POLY 1024
 #endif
 #ifndef PDV_LB_BLOCKS
 #define PDV_LB_BLOCKS 1
@@ -92,12 +95,6 @@ struct UnitDesc {
     // ids at a time; chunk_per_remaining = 1 / (2 * threads expected to work on the unit)
     uint32_t chunk;
     float chunk_per_remaining;
-    // Random draws (Philox blocks of a one-class cloud = 2 flights each, block pairs of a polydisperse one = 3 flights each)
-    // a lane flies between two end-of-history passes of its warp.  1 for short histories; more when histories are long: the
-    // end-of-history pass then runs at one or two lanes, and running it less often costs fewer issue slots than the lanes
-    // that wait for it.
-    uint32_t draws_per_pass;
-    uint32_t pad;
 };
 
 struct RunParams {
@@ -127,7 +124,10 @@ struct RunParams {
 struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
-struct KernelVariant { bool poly, analog, sso, trace, roulette; int dm; };   // dm: see transport_kernel   // template instantiation of transport_kernel
+// long_hist: the launch's histories are long (cost-weighted mean of the estimated flights per history >= 45): a one-class
+// kernel then flies several random draws between two end-of-history passes -- that pass runs at one or two lanes when histories
+// are long, and running it less often costs fewer issue slots than the lanes that wait for it (measured: profiles/README.md)
+struct KernelVariant { bool poly, analog, sso, trace, roulette; int dm; bool long_hist; };   // dm: see transport_kernel   // template instantiation of transport_kernel
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,

@@ -26,9 +26,12 @@ __shared__ unsigned int s_dbg[8];
 #define PDV_BOUND(cat, idx, limit) do { } while (0)
 #endif
 
-// experiment builds only: force UnitDesc::draws_per_pass
-#ifndef PDV_FORCE_DRAWS
-#define PDV_FORCE_DRAWS 0
+// Draws per pass of the LONG instantiations (experiment builds may override): see transport_kernel
+#ifndef PDV_DRAWS_LONG_MONO
+#define PDV_DRAWS_LONG_MONO 4
+#endif
+#ifndef PDV_DRAWS_LONG_POLY
+#define PDV_DRAWS_LONG_POLY 1
 #endif
 // Register budget of transport_kernel: PDV_LB_THREADS x PDV_LB_BLOCKS resident threads per SM (pdv_device.h).
 namespace pdv {
@@ -210,8 +213,15 @@ __device__ __noinline__ RouletteOut roulette_with_word(float w, float abss, uint
 // History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
 enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
 __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
+    // Random draws (Philox blocks of a one-class cloud = 2 flights each, block pairs of a polydisperse one = 3 flights each) a
+    // lane flies between two end-of-history passes of its warp: 1, or 4 in the LONG instantiations of the one-class kernel,
+    // which the host picks for launches whose histories are long (KernelVariant::long_hist; config 4: 130.5 -> 124 ms).
+    // Polydisperse kernels always fly one draw (measured at 896 threads: config 5 275.9 / 272.4 / 274.0 ms, Figs. 13-15
+    // sweep 74.2 / 78.2 / 77.8 ms with 1 / 2 / 3 draws).  A compile-time constant: as a run-time loop bound it cost a
+    // register and spilled (config 2 3.81 -> 4.12 ms, config 3 +14 %).
+    constexpr uint32_t draws = LONG ? (POLY ? PDV_DRAWS_LONG_POLY : PDV_DRAWS_LONG_MONO) : 1;
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ uint32_t s_pool_next[32];
@@ -265,7 +275,6 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
-        const uint32_t draws = PDV_FORCE_DRAWS ? PDV_FORCE_DRAWS : ud.draws_per_pass;
         const float albedo0 = cv.albedo[0];               // monodisperse: the only class
         const uint32_t albthr0 = cv.albthr[0];
 
@@ -491,7 +500,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 // word made of their low bytes (a.byte0, b.byte0, a.byte1, a.byte2 from the top: neither the 23 path bits nor
                 // the 22 phase bits reach the two leading ones) and, with several size classes, a class word.
                 // One class: one Philox4x32-10 block feeds two flights.  Several classes: two blocks feed three flights.
-                // A pass flies `draws` blocks / groups (UnitDesc::draws_per_pass: 1 unless histories are long): the end-of-history code below runs at the few
+                // A pass flies `draws` blocks / groups (1 unless histories are long): the end-of-history code below runs at the few
                 // lanes whose history ended, so it is entered once per several flights; those lanes wait meanwhile ------
                 if (POLY) {
 #pragma unroll 1
@@ -580,11 +589,11 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
 
 // ------------------------------------------------------------------------------------------------------------
 // The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
 static cudaError_t ensure_smem(int smem) {
     static int smem_set = 48 * 1024;
     if (smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM>,
+        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         smem_set = smem;
@@ -592,19 +601,19 @@ static cudaError_t ensure_smem(int smem) {
     return cudaSuccess;
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
 static cudaError_t launch_t(const RunParams &rp, LaunchShape s, cudaStream_t st) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM>(s.smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>(s.smem);
     if (e != cudaSuccess) return e;
-    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM><<<s.grid, s.block, s.smem, st>>>(rp);
+    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG><<<s.grid, s.block, s.smem, st>>>(rp);
     return cudaGetLastError();
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
 static cudaError_t occ_t(int block, int smem, int *out) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM>(smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>(smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM>, block, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>, block, smem);
 }
 
 // DM = 0 / 1 exist for the production variants only; single-scatter-only and trace runs always take the general kernel.
@@ -632,11 +641,21 @@ static cudaError_t occ_dm(int dm, int block, int smem, int *out) {
 #define PDV_D3(FN, A, ...) (v.analog ? PDV_D2(FN, A, true, __VA_ARGS__) : PDV_D2(FN, A, false, __VA_ARGS__))
 #define PDV_DISPATCH(FN, ...) (v.poly ? PDV_D3(FN, true, __VA_ARGS__) : PDV_D3(FN, false, __VA_ARGS__))
 
+// LONG instantiations exist for the production variants of the one-class depth-table kernel only (implicit capture, no
+// single-scatter cut, no trace, DM 0): the thick sweeps of config 4.
+static bool long_variant(const KernelVariant &v) { return v.long_hist && !v.poly && !v.analog && !v.sso && !v.trace && v.dm == 0; }
+
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st) {
+    if (long_variant(v)) {
+        return v.roulette ? launch_t<false, false, false, false, true, 0, true>(rp, shape, st) : launch_t<false, false, false, false, false, 0, true>(rp, shape, st);
+    }
     return PDV_DISPATCH(launch_dm, rp, shape, st);
 }
 
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out) {
+    if (long_variant(v)) {
+        return v.roulette ? occ_t<false, false, false, false, true, 0, true>(block, smem, out) : occ_t<false, false, false, false, false, 0, true>(block, smem, out);
+    }
     return PDV_DISPATCH(occ_dm, block, smem, out);
 }
 
