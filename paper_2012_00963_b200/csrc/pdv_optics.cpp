@@ -14,6 +14,10 @@
 #include <cmath>
 #include <limits>
 #include <complex>
+#include <cstring>
+#include <deque>
+#include <memory>
+#include <mutex>
 #include <thread>
 #include <utility>
 
@@ -210,6 +214,33 @@ pdv_status lognormal_classes(double d_median, double sigma_ln, int n, double *di
 
 static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
+// Process-wide memo of the per-class optics (efficiencies + inverse-CDF phase table), keyed by the exact bits of
+// (size parameter, refractive index, K): the clouds of a parameter sweep differ in area mass and velocity profile and share
+// their size classes (Figs. 7-8, 13-15: 14 clouds = 2 size distributions), and a table costs ~0.4 ms of host
+// time.  A hit returns exactly what a recomputation would.  At most 4096 tables (8 KB each at K = 1024), oldest dropped first.
+namespace {
+struct ClassOptics { double k_ext, k_sca, g; std::vector<double> M; };
+struct OpticsKey {
+    uint64_t x, m_re, m_im; int K;
+    bool operator==(const OpticsKey &o) const { return x == o.x && m_re == o.m_re && m_im == o.m_im && K == o.K; }
+};
+uint64_t bits_of(double v) { uint64_t u; std::memcpy(&u, &v, 8); return u; }
+std::mutex g_memo_mu;
+std::deque<std::pair<OpticsKey, std::shared_ptr<const ClassOptics>>> g_memo;
+
+std::shared_ptr<const ClassOptics> memo_find(const OpticsKey &k) {
+    std::lock_guard<std::mutex> lk(g_memo_mu);
+    for (const auto &e : g_memo) if (e.first == k) return e.second;
+    return nullptr;
+}
+void memo_store(const OpticsKey &k, std::shared_ptr<const ClassOptics> v) {
+    std::lock_guard<std::mutex> lk(g_memo_mu);
+    for (const auto &e : g_memo) if (e.first == k) return;
+    if (g_memo.size() >= 4096) g_memo.pop_front();
+    g_memo.emplace_back(k, std::move(v));
+}
+}  // namespace
+
 pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::string &err) {
     auto bad = [&](const char *msg) { err = msg; return PDV_E_INVALID; };
     if (!(p.area_mass >= 0.0) || !std::isfinite(p.area_mass)) return bad("area_mass must be >= 0");
@@ -262,17 +293,24 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
     h.k_ext.resize(p.n_classes); h.k_sca.resize(p.n_classes); h.g.resize(p.n_classes); h.p_class.resize(p.n_classes);
     h.phase.resize((size_t)p.n_classes * (K + 1));
     double s_ext = 0.0, s_d3 = 0.0, s_d2 = 0.0;
+    std::vector<int> computed;                           // classes whose optics were computed in this call (not copied, not memoised)
     std::vector<int> todo;                               // classes whose phase table is still to be computed
     std::vector<std::pair<int, int>> copies;
     for (int c = 0; c < p.n_classes; ++c) {
         const double d = h.diameter[c], x = kPi * d / p.wavelength;
         int same = -1;                                   // identical diameters share a table
         for (int e = 0; e < c; ++e) if (h.diameter[e] == d) { same = e; break; }
+        const OpticsKey key{bits_of(x), bits_of(p.m_re), bits_of(p.m_im), K};
+        std::shared_ptr<const ClassOptics> hit = (same < 0 && p.phase_model == 0) ? memo_find(key) : nullptr;
         if (same >= 0) {
             h.k_ext[c] = h.k_ext[same]; h.k_sca[c] = h.k_sca[same]; h.g[c] = h.g[same];
             copies.emplace_back(c, same);                // the table itself is copied once it exists, below
+        } else if (hit) {
+            h.k_ext[c] = hit->k_ext; h.k_sca[c] = hit->k_sca; h.g[c] = hit->g;
+            std::copy(hit->M.begin(), hit->M.end(), h.phase.begin() + (size_t)c * (K + 1));
         } else {
             mie_efficiencies(x, p.m_re, p.m_im, &h.k_ext[c], &h.k_sca[c], &h.g[c]);
+            computed.push_back(c);
             double *M = &h.phase[(size_t)c * (K + 1)];
             if (p.phase_model == 1) {
                 for (int k = 0; k <= K; ++k) M[k] = -1.0 + 2.0 * (double)k / (double)K;
@@ -300,6 +338,15 @@ pdv_status build_host_cloud(const pdv_cloud_params &p, HostCloud &out, std::stri
         for (int t = 1; t < n_thr; ++t) pool.emplace_back(work, t);
         work(0);
         for (auto &th : pool) th.join();
+    }
+    if (p.phase_model == 0) {                             // remember what was computed here (Mie tables only)
+        auto remember = [&](int c) {
+            auto v = std::make_shared<ClassOptics>();
+            v->k_ext = h.k_ext[c]; v->k_sca = h.k_sca[c]; v->g = h.g[c];
+            v->M.assign(h.phase.begin() + (size_t)c * (K + 1), h.phase.begin() + (size_t)(c + 1) * (K + 1));
+            memo_store(OpticsKey{bits_of(kPi * h.diameter[c] / p.wavelength), bits_of(p.m_re), bits_of(p.m_im), K}, std::move(v));
+        };
+        for (int c : computed) remember(c);
     }
     for (const auto &cs : copies)
         std::copy(h.phase.begin() + (size_t)cs.second * (K + 1), h.phase.begin() + (size_t)(cs.second + 1) * (K + 1),
