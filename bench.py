@@ -420,7 +420,7 @@ def main():
         for idx in (0, 2, 3, 4, 5):
             if idx == args.config:
                 continue
-            o = time_workload(P, torch, dist, _workload(idx), args, steps=2, warmup=3, e2e_steps=1, rank=rank, world=world, local=local,
+            o = time_workload(P, torch, dist, _workload(idx), args, steps=2, warmup=3, e2e_steps=2, rank=rank, world=world, local=local,
                               clk=clk, want_peaks=peaks)
             if o is not None:
                 others.append({"workload": o["config"]["workload"], "config_index": idx, "value": o["value"], "unit": UNIT,

@@ -461,7 +461,10 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     int block = o->threads_per_block, per_sm = 0;
     // polydisperse clouds: their tables leave room for one block per SM: PDV_LB_THREADS_POLY threads (pdv_device.h)
     if (kv.poly) block = block == 0 ? PDV_LB_THREADS_POLY : std::min(block, PDV_LB_THREADS_POLY);
-    if (block == 0) block = 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024 ? 512 : 1024;
+    // one class: 1024 resident threads per SM either way.  Several units: two blocks of 512 when their shared memory fits twice
+    // (finer grain where blocks move from unit to unit: config 4 123.9 ms against 135.3 with one block of 1024); ONE unit: one
+    // block of 1024 (half as many stagings, flushes and warp pools: config 2 3.73 ms against 3.81)
+    if (block == 0) block = (n_units > 1 && 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024) ? 512 : 1024;
     {
         struct Key { KernelVariant v; int block, smem, device; };
         static std::mutex mu;
