@@ -73,8 +73,10 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     while ((1 << steps) < nc) ++steps;
     const int n_pad = 1 << steps;
     // fp32 depth edges, T_0 = 0 at the cloud top ... T_nd = tau_ext at the free surface, non-decreasing
+    // The device carries optical depths in units of ln 2: a flight is then  T' = T + mu lg2(xi)  -- the SFU's base-2 logarithm
+    // without the multiplication by ln 2 (pdv_device.h).  Everything below (slopes, guide, tau_ext, closed form) is in those units.
     std::vector<float> Tf(nd + 1);
-    for (int j = 0; j <= nd; ++j) Tf[j] = (float)T_src[j];
+    for (int j = 0; j <= nd; ++j) Tf[j] = (float)(T_src[j] / 0.6931471805599453);
     Tf[0] = 0.f;
     for (int j = 1; j <= nd; ++j) if (Tf[j] < Tf[j - 1]) Tf[j] = Tf[j - 1];
     // depth rows (layout: pdv_device.h).  Half velocities: the Doppler update is  v~ += (mu' - mu) v/2  (Eq. 4).
@@ -122,6 +124,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     std::memset(&hd, 0, sizeof(hd));
     size_t off = sizeof(DevCloudHeader);
     hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * 2 * (size_t)nc * K);
+    off += 80;                                                // the block writes its Philox round keys in front of the rows (pdv_device.h)
     hd.off_rows = (uint32_t)off;   off = align16(off + sizeof(float) * 4 * (size_t)nd);
     hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * n_pad);
@@ -464,7 +467,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     // one class: 1024 resident threads per SM either way.  Several units: two blocks of 512 when their shared memory fits twice
     // (finer grain where blocks move from unit to unit: config 4 123.9 ms against 135.3 with one block of 1024); ONE unit: one
     // block of 1024 (half as many stagings, flushes and warp pools: config 2 3.73 ms against 3.81)
-    if (block == 0) block = (n_units > 1 && 2 * (size_t)(smem + 1024 + 256) <= di.smem_optin + 1024) ? 512 : 1024;
+    if (block == 0) block = (n_units > 1 && 2 * (size_t)(smem + 1024 + 18432) <= di.smem_optin + 1024) ? 512 : 1024;   // 18 KB: the kernel's static shared memory (warp queues)
     {
         struct Key { KernelVariant v; int block, smem, device; };
         static std::mutex mu;

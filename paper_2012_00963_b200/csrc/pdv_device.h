@@ -44,6 +44,8 @@ enum StatSlot {
 // D_K sample M[k] + (M[k+1]-M[k]) frac with frac = the 12 bits of b below the index bits: one 64-bit load,
 // one FFMA.
 //
+// UNITS: every optical depth of the image (rows.x, tau_ext, the guide's float bits, an_c3) is in units of ln 2, T / ln 2: the
+// kernel's free flight is then  T' = T + mu lg2(xi)  with the SFU's base-2 logarithm and no multiplication by ln 2.
 // Depth rows (one float4 per depth bin j, bins uniform in v, j = 0 at the cloud top):
 //   x = T_{j+1}                      vertical optical depth of the LOWER edge of bin j
 //   y = v(T_{j+1}) / 2               half the particle velocity at that edge (the Doppler update uses v/2)
@@ -67,7 +69,7 @@ struct DevCloudHeader {
     uint32_t guide_base;       // (float bits of T) >> guide_shift of guide cell 0
     uint32_t guide_shift;
     uint32_t depth_bisect;     // 0: one guide probe; 1: bisect the rows; 2: closed form  v/2 = an_c0 + an_c1 lg2(an_c2 + an_c3 T)
-    float tau_ext, vh_fs;      // vh_fs = v_fs / 2
+    float tau_ext, vh_fs;      // tau_ext in units of ln 2 (see above); vh_fs = v_fs / 2
     float R_f;                 // surface reflectivity
     uint32_t R_thr;            // analog mode: reflected iff xi_absorb word < R_thr
     uint32_t surface_model;

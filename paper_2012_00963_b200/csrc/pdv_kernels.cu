@@ -73,6 +73,20 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
+// The flight loop reads the round keys from a copy that each block keeps in the 80 bytes in front of its depth rows: the rows'
+// base address is in a register anyway, while s_keys (static shared memory) costs three uniform-datapath instructions per pass
+// to address (S2UR SR_CgaCtaId, UMOV, ULEA); as constant-bank operands the keys became five LDCU.128 per block (measured
+// slower on the polydisperse kernels).
+#define PHILOX_MAIN(c0, c1, c2, c3, o0, o1, o2, o3) philox4x32_10(c0, c1, c2, c3, reinterpret_cast<const uint4 *>(cv.rows) - 5, o0, o1, o2, o3)
+
+// threadIdx.x read where it is used: the address of a warp's shared state is then computed inside the rare path that needs it
+// instead of being hoisted into every pass (or kept in a register the polydisperse kernels do not have)
+__device__ __forceinline__ uint32_t opaque_tid() {
+    uint32_t t;
+    asm volatile("mov.u32 %0, %%tid.x;" : "=r"(t));
+    return t;
+}
+
 __device__ __forceinline__ float fast_sqrt(float x) {
     float r;
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
@@ -97,6 +111,23 @@ __device__ __forceinline__ void smem_add64(unsigned long long *p, uint32_t v) {
     if (old + v < old) atomicAdd(q + 1, 1u);
 }
 
+// Per-warp shared state.  pool_next: hand-out cursor of the warp's pool of photon ids.  q / qn: the warp's DETECTION QUEUE.  A
+// history that leaves inside the probe aperture (2 % of the histories, about one lane of a warp in every third pass) only
+// pushes (v~, Q31 weight) here -- one shared atomic and one 64-bit store; the warp tallies the queue into the block's
+// histogram (Eq. 19) with all 32 lanes once 32 entries are waiting, and when the unit is drained.  The tally itself -- bin, two
+// carry-propagating pairs of shared atomics -- took 35 instructions at 1.2 lanes, 5 % of the kernel's issue slots.
+// A pass pushes at most 32 entries and the queue is emptied before the next pass whenever it holds 32 or more: 64 slots.
+struct WarpShared {
+    uint2 q[64];
+    uint32_t qn, pool_next, pad[2];
+};
+
+__device__ __forceinline__ uint32_t lds_u16(uint32_t saddr) {
+    uint16_t v;
+    asm("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(saddr));
+    return v;
+}
+
 struct CloudView {               // per-unit scalars and shared-memory table pointers
     const uint32_t *gthr;        // gas units: per-bin class thresholds [n_depth][1 << gas_steps]
     const float2 *gcls;          // gas units: per-class (L / 2t, -1 / L)
@@ -106,7 +137,7 @@ struct CloudView {               // per-unit scalars and shared-memory table poi
     const float4 *rows;
     const uint32_t *thr, *albthr;
     const float *albedo;
-    const uint16_t *guide;
+    uint32_t guide_s;            // shared-memory address of the depth guide, minus 2 * guide_base
     const unsigned char *cguide;
     uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, depth_bisect, cg_shift;
     float tau_ext, R_f, one_minus_R;
@@ -125,12 +156,14 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
         }
         j = lo;
     } else {
-        // cv.guide points guide_base cells BEFORE the table, so the clamped cell number indexes it directly
+        // cv.guide_s is the shared-memory address of the guide minus guide_base cells, so the clamped cell number indexes it
+        // directly (as an integer the compiler cannot see through: it turned the pre-offset POINTER back into a subtraction of
+        // guide_base per flight)
         uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base);
 #ifdef PDV_DEBUG_BOUNDS
         { uint32_t rel = cell - cv.guide_base; PDV_BOUND(0, rel, cv.n_guide); cell = rel + cv.guide_base; }
 #endif
-        j = cv.guide[cell];
+        j = lds_u16(cv.guide_s + 2u * cell);
     }
     PDV_BOUND(1, j, cv.n_depth);
     const float4 r = cv.rows[j];
@@ -141,7 +174,7 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
 // Same one-probe rows as depth_half_velocity (y = zeta at the lower edge of bin j, z / w = dzeta/dT in bins j / j+1).
 __device__ __forceinline__ float gas_height(const CloudView &cv, float Tc, uint32_t &bin) {
     const uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base);
-    const uint32_t j = cv.guide[cell];
+    const uint32_t j = lds_u16(cv.guide_s + 2u * cell);
     const float4 r = cv.rows[j];
     const bool lower = !(Tc < r.x);
     bin = min(j + (lower ? 1u : 0u), cv.n_depth - 1u);
@@ -213,6 +246,37 @@ __device__ __noinline__ RouletteOut roulette_with_word(float w, float abss, uint
 // History fates inside the kernel (pdv_trace_record.fate: 6 is reported as 2).
 enum : int { F_NONE = -1, F_DETECTED = 0, F_EXIT = 1, F_ABS_SURF = 2, F_KILLED = 3, F_TRUNC = 4, F_DET_OUT = 5, F_ABS_PART = 6 };
 
+extern __shared__ __align__(16) unsigned char smem[];        // [hist u64 n_bins | hist2 u64 n_bins | cloud blob]
+__shared__ WarpShared s_warp[32];
+
+// Tally of one detection (Eq. 19): bin of v~, weight and squared weight in Q31 into the block's private histogram
+__device__ __forceinline__ int tally_detection(float vt, uint32_t wq, uint32_t n_bins, float v_lo, float inv_dv) {
+    unsigned long long *s_hist = reinterpret_cast<unsigned long long *>(smem);
+    const float fb = (vt - v_lo) * inv_dv;
+    const uint32_t bin = (uint32_t)__float2int_rd(fb);       // floor; negative -> huge
+    if (bin < n_bins) {
+        smem_add64(&s_hist[bin], wq);
+        smem_add64(&s_hist[n_bins + bin], mul_q31(wq, wq));
+        return F_DETECTED;
+    }
+    smem_add64(&s_stats[fb < 0.f ? ST_UNDER : ST_OVER], wq);
+    return F_DET_OUT;
+}
+
+// The warp (all 32 lanes) tallies its detection queue and empties it.  Out of line: a few times per thousand passes.
+__device__ __noinline__ void drain_queue(uint32_t n_bins, float v_lo, float inv_dv) {
+    WarpShared &ws = s_warp[threadIdx.x >> 5];
+    __syncwarp();
+    const uint32_t nq = ws.qn;
+    for (uint32_t i = threadIdx.x & 31u; i < nq; i += 32u) {
+        const uint2 e = ws.q[i];
+        tally_detection(__uint_as_float(e.x), e.y, n_bins, v_lo, inv_dv);
+    }
+    __syncwarp();
+    if ((threadIdx.x & 31u) == 0u) ws.qn = 0u;
+    __syncwarp();
+}
+
 template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
 __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     // Random draws (Philox blocks of a one-class cloud = 2 flights each, block pairs of a polydisperse one = 3 flights each) a
@@ -223,9 +287,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
     // register and spilled (config 2 3.81 -> 4.12 ms, config 3 +14 %).
     constexpr uint32_t draws = LONG ? (POLY ? PDV_DRAWS_LONG_POLY : PDV_DRAWS_LONG_MONO) : 1;
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
-    extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ uint32_t s_pool_next[32];
     __shared__ int s_go;
+    constexpr bool QUEUE = !TRACE;                            // aperture hits go through the warp's detection queue
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u;
     unsigned long long *s_hist = reinterpret_cast<unsigned long long *>(smem);
@@ -264,7 +327,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cv.thr = reinterpret_cast<const uint32_t *>(s_blob + h->off_thr);
             cv.albedo = reinterpret_cast<const float *>(s_blob + h->off_albedo);
             cv.albthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_albthr);
-            cv.guide = reinterpret_cast<const uint16_t *>(s_blob + h->off_guide) - h->guide_base;
+            cv.guide_s = (uint32_t)__cvta_generic_to_shared(s_blob + h->off_guide) - 2u * h->guide_base;
+            asm volatile("" : "+r"(cv.guide_s));
             cv.cguide = s_blob + h->off_cguide;
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
@@ -275,6 +339,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
+        if (tid < 5) const_cast<uint4 *>(reinterpret_cast<const uint4 *>(cv.rows) - 5)[tid] = s_keys[tid];     // see PHILOX_MAIN
+        __syncthreads();
         const float albedo0 = cv.albedo[0];               // monodisperse: the only class
         const uint32_t albthr0 = cv.albthr[0];
 
@@ -305,7 +371,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         // nfl = flights flown so far = Philox draw index of the next flight (D1); refl0 = the thread's reflection
         // counter at the start of this history, kept only by the variants that read a history's own reflection count (NREFL).
         // run: the lane flies a photon; want: it needs a photon id (neither: the unit is drained, the lane is done).
-        bool run = false, want = true;
+        bool run = false;
+        uint32_t need = 1u;
         float T = 0.f, mu = -1.f, vt = 0.f, w = 1.f, abss = 0.f;
         uint32_t nfl = 0u, refl0 = 0u, id_lo = 0u, id_hi = 0u;
 #define N_REFL (cnt_refl - refl0)      /* reflections of this history: the thread's counter minus its value at the history's start */
@@ -314,20 +381,23 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         // atomic.  Pools are claimed from the unit's global cursor by lane 0 (guided sizes): ~1e4 times fewer global
         // atomics than one claim per lane -- the single-address L2 atomic rate was what bounded the drain of a unit.
         uint32_t pool_lo = 0u, pool_hi = 0u, pool_len = 0u, slice = 1u, left = 0u;
-        uint32_t *pool_next = &s_pool_next[tid >> 5];
-        if (lane == 0) *pool_next = 0u;
+        WarpShared &ws = s_warp[tid >> 5];
+        uint32_t *pool_next = &ws.pool_next;
+        if (lane == 0) { ws.pool_next = 0u; ws.qn = 0u; }
         __syncwarp();
+        // need: bit 0 = the lane waits for a photon id, bit 1 = the warp's detection queue is half full
 
         // next photon of this lane: the next id of its private slice, else a new slice of `slice` ids from the warp pool
         // (want = true if the pool is exhausted); resets the history state
         auto take_photon = [&]() {
             if (left) {
-                --left;
-                if (++id_lo == 0u) ++id_hi;
+                // --left, ++id (64 bits) -- as predicated PTX: the compiler's version added, compared, undid and moved (7 instructions)
+                asm("{\n\t.reg .pred q;\n\tsub.u32 %2, %2, 1;\n\tadd.u32 %0, %0, 1;\n\tsetp.eq.u32 q, %0, 0;\n\t@q add.u32 %1, %1, 1;\n\t}"
+                    : "+r"(id_lo), "+r"(id_hi), "+r"(left));
             } else {
-                const uint32_t off = atomicAdd(pool_next, slice);
+                const uint32_t off = atomicAdd(POLY ? &s_warp[opaque_tid() >> 5].pool_next : pool_next, slice);
                 run = off < pool_len;
-                want = !run;
+                need = (need & ~1u) | (run ? 0u : 1u);
                 left = run ? min(slice, pool_len - off) - 1u : 0u;
                 id_lo = pool_lo + off;
                 id_hi = pool_hi + (id_lo < pool_lo ? 1u : 0u);
@@ -339,17 +409,16 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         // end of a history (step (7)): Eq. 19 tally or escape, per-history bookkeeping in Q31, then the lane's next photon
         auto finish = [&](int fate) {
             const uint32_t wq = __float2uint_rn(w * kWOneF);
-            if (fate == F_EXIT) {
+            // without analog absorption, roulette and the single-scatter cut every history ends by leaving through the top
+            if ((!ANALOG && !ROUL && !SSO) || fate == F_EXIT) {
                 if (mu >= P.mu_aperture) {                    // inside the probe aperture: Eq. 19
-                    const float fb = (vt - P.v_lo) * P.inv_dv;
-                    const uint32_t bin = (uint32_t)__float2int_rd(fb);       // floor; negative -> huge
-                    if (bin < P.n_bins) {
-                        smem_add64(&s_hist[bin], wq);
-                        smem_add64(&s_hist2[bin], mul_q31(wq, wq));
-                        fate = F_DETECTED;
+                    if (QUEUE) {
+                        WarpShared &wq_ = POLY ? s_warp[opaque_tid() >> 5] : ws;
+                        const uint32_t slot = atomicAdd(&wq_.qn, 1u);
+                        wq_.q[slot] = make_uint2(__float_as_uint(vt), wq);
+                        if (slot >= 31u) need |= 2u;
                     } else {
-                        smem_add64(&s_stats[fb < 0.f ? ST_UNDER : ST_OVER], wq);
-                        fate = F_DET_OUT;
+                        fate = tally_detection(vt, wq, P.n_bins, P.v_lo, P.inv_dv);
                     }
                     acc_rare += wq;
                 } else {
@@ -362,7 +431,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 smem_add64(&s_stats[ST_TRUNC], wq);
                 acc_rare += wq;
             }
-            acc_abss += min(__float2uint_rn(abss * kWOneF), kWOne - wq);
+            // weight left in the surface: implicit capture, (1 - R) x the weights that reached it; analog, the absorbed weight
+            acc_abss += min(__float2uint_rn(abss * (ANALOG ? kWOneF : cv.one_minus_R * kWOneF)), kWOne - wq);
             const uint32_t n_int = nfl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);     // scatters + reflections
             cnt_fl += nfl;                                    // an absorbing interaction is a particle event too
             max_ev = max(max_ev, n_int);
@@ -380,9 +450,9 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         // Returns F_NONE while the history goes on.
         auto flight = [&](uint32_t a, uint32_t cw, uint32_t b, uint32_t pw, uint32_t ya, uint32_t y_roul, uint32_t sub) -> int {
             // ---------------- free flight: s = -ln(xi), xi in (0,1]; T' = T - mu s (Eq. 7/10, step (3)) ---------------
+            // T is carried in units of ln 2 (so are the depth tables): -mu s / ln 2 = mu lg2(xi)
             const float xi = 2.0f - __uint_as_float(0x3F800000u | (a >> 9));
-            const float s = fast_lg2(xi) * -0.69314718056f;
-            const float Tn = fmaf(-mu, s, T);
+            const float Tn = fmaf(mu, fast_lg2(xi), T);
             if (Tn < 0.f) return F_EXIT;                      // leaves through the top (step (6))
             const bool surf = Tn >= cv.tau_ext;               // reaches the free surface
             if (SSO && !surf && nfl != N_REFL) return F_TRUNC;    // single-scatter-only: cut at the 2nd particle event
@@ -422,7 +492,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     return surf ? F_ABS_SURF : F_ABS_PART;
                 }
             } else {                                          // implicit capture: Eq. 11 in expectation
-                if (surf) abss = fmaf(w, cv.one_minus_R, abss);
+                if (surf) abss += w;                          // the surface keeps (1 - R) of it: multiplied in when the history ends
                 w *= surf ? cv.R_f : alb;
             }
             // cos(theta) from D_K (Eq. 13-14): M[k] + (M[k+1] - M[k]) frac in one 64-bit load and one FFMA
@@ -432,7 +502,9 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             const float ct = fmaf(m.y, __uint2float_rn(b & cv.frac_mask), m.x);
             // one cosine serves both: cos(phi), phi = 2 pi pw / 2^32 (Eq. 15), or cos(theta'), theta' = (pi/2) pw / 2^32
             const float pwf = __uint2float_rn(pw);
-            const float cosv = __cosf(pwf * (surf ? 3.65729519818e-10f : 1.46291807927e-9f));
+            float ang = pwf * 1.46291807927e-9f;              // 2 pi / 2^32 ...
+            if (surf) ang *= 0.25f;                           // ... or (pi/2) / 2^32
+            const float cosv = __cosf(ang);
             const float sq = fast_sqrt(fabsf(fmaf(-ct, ct, 1.f) * fmaf(-mu, mu, 1.f)));
             // z row of Eq. 16 (Eq. 17 at |mu| = 1).  Rounding may leave |mu| one ulp above 1: harmless, the next square root
             // takes |(1 - ct^2)(1 - mu^2)|
@@ -451,21 +523,25 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             if (ROUL && nfl >= P.max_events && nfl - N_REFL >= P.max_events && w <= P.roulette_p) {
                 // the flight that just ended is nfl - 1: monodisperse, word 2 + sub of the companion of block (nfl - 1) / 2;
                 // polydisperse, word sub of the companion of the group's second block
-                const RouletteOut o = ANALOG ? roulette_with_word(w, abss, y_roul)
-                                      : POLY ? roulette_with_draw(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, sub, w, abss)
-                                             : roulette_with_draw(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, 2u + sub, w, abss);
+                const float ab = ANALOG ? abss : abss * cv.one_minus_R;
+                const RouletteOut o = ANALOG ? roulette_with_word(w, ab, y_roul)
+                                      : POLY ? roulette_with_draw(id_lo, id_hi, ud.stream, 4u * ((nfl - 1u) / 3u) + 3u, sub, w, ab)
+                                             : roulette_with_draw(id_lo, id_hi, ud.stream, 2u * ((nfl - 1u) >> 1) + 1u, 2u + sub, w, ab);
                 if (o.killed) return F_KILLED;
                 w = o.w; abss = o.abss; acc_gain += o.add_lost; acc_abss += o.add_abss;
             }
             return F_NONE;
         };
 
-        bool refill = true;                                   // warp-uniform: some lane waits for a photon id
         for (;;) {
-            if (refill) {
-                // ---- some lane found the warp pool empty: refill it from the unit's cursor (guided self-scheduling: a warp
-                // claims clamp(remaining / (2 warps), 32, 32 chunk) ids, sized from a fresh look at the cursor) and
-                // hand ids to the waiting lanes; lanes still waiting when the unit is drained are done
+            if (QUEUE && __any_sync(FULL_MASK, need & 2u)) {  // the detection queue is half full: tally it
+                drain_queue(P.n_bins, P.v_lo, P.inv_dv);
+                need &= ~2u;
+            }
+            if (__any_sync(FULL_MASK, need & 1u)) {
+                // ---- some lane found the warp pool empty (or the unit starts): refill it from the unit's cursor (guided
+                // self-scheduling: a warp claims clamp(remaining / (2 warps), 32, 32 chunk) ids, sized from a fresh look at the
+                // cursor) and hand ids to the waiting lanes; lanes still waiting when the unit is drained are done
                 for (;;) {
                     unsigned long long b = 0ull;
                     uint32_t len = 0u;
@@ -485,15 +561,16 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     }
                     len = __shfl_sync(FULL_MASK, len, 0);
                     __syncwarp();                                 // lane 0's cursor reset is visible to the takes below
-                    if (len == 0u) { want = false; break; }
+                    if (len == 0u) { need &= ~1u; break; }
                     const unsigned long long id0 = P.first_id + __shfl_sync(FULL_MASK, b, 0);
                     pool_lo = (uint32_t)id0; pool_hi = (uint32_t)(id0 >> 32); pool_len = len;
                     slice = max(len >> 5, 1u);                    // a lane takes 1/32 of the pool at a time: 1 id from the last pools
-                    if (want) take_photon();
-                    if (!__any_sync(FULL_MASK, want)) break;
+                    if (need & 1u) take_photon();
+                    if (!__any_sync(FULL_MASK, need & 1u)) break;
                 }
                 if (!__any_sync(FULL_MASK, run)) break;
             }
+            do {                                              // passes until a lane waits for a photon id
             int fate = F_NONE;
             if (run) {
                 // -------- random numbers (step (3); D1/D2).  A flight reads a path word a, a phase word b, an azimuth
@@ -507,8 +584,8 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     for (uint32_t grp = 0; grp < draws && fate == F_NONE; ++grp) {
                         const uint32_t b2 = 2u * (nfl / 3u);      // nfl is a multiple of 3 here: blocks b2 and b2 + 1
                         uint32_t w0, w1, w2, w3, w4, w5, w6, w7, ya0 = 0u, ya1 = 0u, ya2 = 0u, ya3 = 0u, yr0 = 0u, yr1 = 0u, yr2 = 0u, yr3 = 0u;
-                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2, s_keys, w0, w1, w2, w3);
-                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 2u, s_keys, w4, w5, w6, w7);
+                        PHILOX_MAIN(id_lo, id_hi, ud.stream, 2u * b2, w0, w1, w2, w3);
+                        PHILOX_MAIN(id_lo, id_hi, ud.stream, 2u * b2 + 2u, w4, w5, w6, w7);
                         if (ANALOG) {                                 // companion blocks: absorption words, roulette words
                             philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 1u, s_keys, ya0, ya1, ya2, ya3);
                             if (ROUL) philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 3u, s_keys, yr0, yr1, yr2, yr3);
@@ -525,7 +602,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                     for (uint32_t blk = 0; blk < draws && fate == F_NONE; ++blk) {
                         const uint32_t draw = nfl >> 1;
                         uint32_t x0, x1, x2, x3, y0 = 0u, y1 = 0u, y2 = 0u, y3 = 0u;
-                        philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw, s_keys, x0, x1, x2, x3);
+                        PHILOX_MAIN(id_lo, id_hi, ud.stream, 2u * draw, x0, x1, x2, x3);
                         if (ANALOG) philox4x32_10(id_lo, id_hi, ud.stream, 2u * draw + 1u, s_keys, y0, y1, y2, y3);
                         fate = flight(x0, 0u, x1, __byte_perm(x0, x1, 0x0412), y0, y2, 0u);
                         if (fate == F_NONE) fate = flight(x2, 0u, x3, __byte_perm(x2, x3, 0x0412), y1, y3, 1u);
@@ -534,8 +611,9 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             }
             __syncwarp();                                     // histories that ended in either flight are finished in ONE pass
             if (fate != F_NONE) finish(fate);                 // the one place where a lane moves on to its next photon
-            refill = __any_sync(FULL_MASK, want);             // only a finished history can leave a lane waiting for an id
+            } while (!__any_sync(FULL_MASK, need));           // only a finished history can leave a lane waiting for an id
         }
+        if (QUEUE) drain_queue(P.n_bins, P.v_lo, P.inv_dv);
 
         // ---- block flush: per-thread counters -> warp -> shared -> global; histogram -> global ------------------
         // mod 2^64 per thread; the sum over a warp is the non-negative total (every history is claimed and finished in one warp)
@@ -591,7 +669,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
 // The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
 template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
 static cudaError_t ensure_smem(int smem) {
-    static int smem_set = 48 * 1024;
+    static int smem_set = 48 * 1024 - (int)sizeof(WarpShared) * 32 - 2048;      // static + dynamic above 48 KB needs the opt-in
     if (smem > smem_set) {
         cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -646,17 +724,39 @@ static cudaError_t occ_dm(int dm, int block, int smem, int *out) {
 static bool long_variant(const KernelVariant &v) { return v.long_hist && !v.poly && !v.analog && !v.sso && !v.trace && v.dm == 0; }
 
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st) {
+#ifdef PDV_FEW
+    if (!long_variant(v)) {
+        if (v.analog || v.sso || v.trace || v.dm != 0) return cudaErrorNotSupported;
+        if (!v.poly) return v.roulette ? cudaErrorNotSupported : launch_t<false, false, false, false, false, 0>(rp, shape, st);
+        return v.roulette ? launch_t<true, false, false, false, true, 0>(rp, shape, st) : launch_t<true, false, false, false, false, 0>(rp, shape, st);
+    }
+#endif
     if (long_variant(v)) {
         return v.roulette ? launch_t<false, false, false, false, true, 0, true>(rp, shape, st) : launch_t<false, false, false, false, false, 0, true>(rp, shape, st);
     }
+#ifdef PDV_FEW
+    return cudaErrorNotSupported;
+#else
     return PDV_DISPATCH(launch_dm, rp, shape, st);
+#endif
 }
 
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out) {
+#ifdef PDV_FEW
+    if (!long_variant(v)) {
+        if (v.analog || v.sso || v.trace || v.dm != 0) return cudaErrorNotSupported;
+        if (!v.poly) return v.roulette ? cudaErrorNotSupported : occ_t<false, false, false, false, false, 0>(block, smem, out);
+        return v.roulette ? occ_t<true, false, false, false, true, 0>(block, smem, out) : occ_t<true, false, false, false, false, 0>(block, smem, out);
+    }
+#endif
     if (long_variant(v)) {
         return v.roulette ? occ_t<false, false, false, false, true, 0, true>(block, smem, out) : occ_t<false, false, false, false, false, 0, true>(block, smem, out);
     }
+#ifdef PDV_FEW
+    return cudaErrorNotSupported;
+#else
     return PDV_DISPATCH(occ_dm, block, smem, out);
+#endif
 }
 
 // ---- finalize: Q31 integers -> doubles (H12 input; stats) ------------------------------------------------------
