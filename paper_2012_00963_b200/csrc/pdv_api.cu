@@ -126,7 +126,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * 2 * (size_t)nc * K);
     off += 80;                                                // the block writes its Philox round keys in front of the rows (pdv_device.h)
     hd.off_rows = (uint32_t)off;   off = align16(off + sizeof(float) * 4 * (size_t)nd);
-    hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * n_pad);
+    hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * 2 * PDV_MAX_CLASSES);     // thr[32] | thr24[32] (pdv_device.h)
     hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * n_pad);
     hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
     hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
@@ -181,6 +181,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     while ((1 << hd.log2K) < K) ++hd.log2K;
     hd.tau_ext = Tf[nd]; hd.vh_fs = (float)(0.5 * h.v_fs);
     hd.R_f = (float)h.R;
+    hd.omr_q31 = (float)((1.0 - (double)hd.R_f) * 2147483648.0);
     hd.R_thr = to_thr32(h.R);
     hd.surface_model = (uint32_t)h.surface_model;
     const uint32_t shiftK = 32u - hd.log2K;                   // K <= 4096: shiftK >= 20
@@ -212,8 +213,16 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     uint32_t *thr = reinterpret_cast<uint32_t *>(blob.data() + hd.off_thr);
     float *alb = reinterpret_cast<float *>(blob.data() + hd.off_albedo);
     uint32_t *albt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_albthr);
+    for (int c = 0; c < PDV_MAX_CLASSES; ++c) {
+        // thr24: for a class word whose low byte is replaced by 0x80 (first and second flight of a group, D2),
+        //   thr <= (W & ~0xff | 0x80)   <=>   W >= 256 ceil((thr - 128) / 256),
+        // so those flights compare the raw word W with thr24 and mask nothing
+        const uint32_t t = c < n_pad ? thr_v[c] : 0xFFFFFFFFu;
+        const uint64_t t24 = t < 128u ? 0u : ((uint64_t)t - 128u + 255u) / 256u;
+        thr[c] = t;
+        thr[PDV_MAX_CLASSES + c] = t24 >= (1u << 24) ? 0xFFFFFFFFu : (uint32_t)(t24 << 8);
+    }
     for (int c = 0; c < n_pad; ++c) {
-        thr[c] = thr_v[c];
         const double om = c < nc ? h.k_sca[c] / h.k_ext[c] : 0.0;
         alb[c] = (float)std::min(std::max(om, 0.0), 1.0);
         albt[c] = to_thr32(om);

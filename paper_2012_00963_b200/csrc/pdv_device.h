@@ -62,6 +62,9 @@ enum StatSlot {
 // every cell but the flagged ones, which walk on.  The host takes the coarsest guide of 2^8 ... 2^12 cells in which no cell
 // holds two thresholds (config 3: 2^10); if even 2^12 cells leave flagged ones (config 5: the two smallest classes, hit with
 // probability 1.7e-6 and 2.7e-5) it stays at 2^12 and one flight in 4096 walks.
+// Class thresholds: two tables of PDV_MAX_CLASSES words.  thr[j] = 32-bit threshold of the cumulative pick probability (padded with
+// 0xffffffff); thr24[j] = 256 ceil((thr[j] - 128) / 256): a class word W whose low byte counts as 0x80 (first and second flight
+// of a three-flight group, D2) satisfies  thr[j] <= (W & ~0xff | 0x80)  exactly when  W >= thr24[j].
 struct DevCloudHeader {
     uint32_t blob_bytes;       // multiple of 16
     uint32_t n_classes, K, log2K, n_depth, n_guide;
@@ -85,7 +88,7 @@ struct DevCloudHeader {
     // class-c particle velocity at zeta is  v_fs/2 + x (1 - e^{y zeta})   resp.   v_fs/2 + x zeta.
     uint32_t gas;              // 1: this image is a gas unit
     uint32_t off_gthr, off_gcls, gas_steps;
-    uint32_t pad[1];
+    float omr_q31;             // (1 - R_f) 2^31: weight that reached the surface -> Q31 weight left in it
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 

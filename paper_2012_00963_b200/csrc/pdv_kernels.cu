@@ -50,7 +50,16 @@ __shared__ float s_roul_inv_p;                            // ... and then w /= p
 // Philox4x32-10 block function.  The 10 round keys (k0_r, k1_r) are precomputed on the host and staged in shared memory,
 // two rounds per uint4: five broadcast LDS.128 per block instead of ten constant-bank loads (the ADU pipe that serves
 // LDC was a third busy with the keys alone).
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint4 *keys,
+struct SharedKeys {              // the five key vectors at a shared-memory address held in a register
+    uint32_t saddr;
+    __device__ __forceinline__ uint4 operator[](int i) const {
+        uint4 k;
+        asm("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(k.x), "=r"(k.y), "=r"(k.z), "=r"(k.w) : "r"(saddr + 16u * (uint32_t)i));
+        return k;
+    }
+};
+template <class Keys>
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const Keys keys,
                                               uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3) {
 #pragma unroll
     for (int r = 0; r < 10; r += 2) {
@@ -77,7 +86,9 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 // base address is in a register anyway, while s_keys (static shared memory) costs three uniform-datapath instructions per pass
 // to address (S2UR SR_CgaCtaId, UMOV, ULEA); as constant-bank operands the keys became five LDCU.128 per block (measured
 // slower on the polydisperse kernels).
-#define PHILOX_MAIN(c0, c1, c2, c3, o0, o1, o2, o3) philox4x32_10(c0, c1, c2, c3, reinterpret_cast<const uint4 *>(cv.rows) - 5, o0, o1, o2, o3)
+// cv.rows_s is that address as an integer the compiler cannot see through (else it may move it to a uniform register and pay a
+// move per load: config 4 +2.5 %).
+#define PHILOX_MAIN(c0, c1, c2, c3, o0, o1, o2, o3) philox4x32_10(c0, c1, c2, c3, SharedKeys{cv.rows_s - 80u}, o0, o1, o2, o3)
 
 // threadIdx.x read where it is used: the address of a warp's shared state is then computed inside the rare path that needs it
 // instead of being hoisted into every pass (or kept in a register the polydisperse kernels do not have)
@@ -122,6 +133,16 @@ struct WarpShared {
     uint32_t qn, pool_next, pad[2];
 };
 
+__device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
+    float4 v;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t saddr) {
+    uint32_t v;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(saddr));
+    return v;
+}
 __device__ __forceinline__ uint32_t lds_u16(uint32_t saddr) {
     uint16_t v;
     asm("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(saddr));
@@ -134,13 +155,14 @@ struct CloudView {               // per-unit scalars and shared-memory table poi
     uint32_t gas_steps;
     float vh_fs;
     const float2 *phase;
-    const float4 *rows;
+    const float4 *rows;          // depth rows (general kernel's bisection); the hot path loads them through rows_s
+    uint32_t rows_s;             // shared-memory address of the depth rows; the block's Philox round keys sit 80 bytes in front
     const uint32_t *thr, *albthr;
     const float *albedo;
     uint32_t guide_s;            // shared-memory address of the depth guide, minus 2 * guide_base
-    const unsigned char *cguide;
+    uint32_t cg_s;               // shared-memory address of the class guide
     uint32_t n_classes, K, shiftK, frac_mask, n_depth, n_guide, guide_base, guide_shift, depth_bisect, cg_shift;
-    float tau_ext, R_f, one_minus_R;
+    float tau_ext, R_f, one_minus_R, omr_q31;
     uint32_t R_thr, surface_model;
 };
 
@@ -166,7 +188,7 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
         j = lds_u16(cv.guide_s + 2u * cell);
     }
     PDV_BOUND(1, j, cv.n_depth);
-    const float4 r = cv.rows[j];
+    const float4 r = lds_f4(cv.rows_s + 16u * j);
     return fmaf(Tc - r.x, Tc < r.x ? r.z : r.w, r.y);
 }
 
@@ -175,7 +197,7 @@ __device__ __forceinline__ float depth_half_velocity(const CloudView &cv, float 
 __device__ __forceinline__ float gas_height(const CloudView &cv, float Tc, uint32_t &bin) {
     const uint32_t cell = max(__float_as_uint(Tc) >> cv.guide_shift, cv.guide_base);
     const uint32_t j = lds_u16(cv.guide_s + 2u * cell);
-    const float4 r = cv.rows[j];
+    const float4 r = lds_f4(cv.rows_s + 16u * j);
     const bool lower = !(Tc < r.x);
     bin = min(j + (lower ? 1u : 0u), cv.n_depth - 1u);
     return fmaf(Tc - r.x, lower ? r.w : r.z, r.y);
@@ -324,19 +346,21 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             const DevCloudHeader *h = reinterpret_cast<const DevCloudHeader *>(s_blob);
             cv.phase = reinterpret_cast<const float2 *>(s_blob + h->off_phase);
             cv.rows = reinterpret_cast<const float4 *>(s_blob + h->off_rows);
+            cv.rows_s = (uint32_t)__cvta_generic_to_shared(cv.rows);
+            asm volatile("" : "+r"(cv.rows_s));
             cv.thr = reinterpret_cast<const uint32_t *>(s_blob + h->off_thr);
             cv.albedo = reinterpret_cast<const float *>(s_blob + h->off_albedo);
             cv.albthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_albthr);
             cv.guide_s = (uint32_t)__cvta_generic_to_shared(s_blob + h->off_guide) - 2u * h->guide_base;
             asm volatile("" : "+r"(cv.guide_s));
-            cv.cguide = s_blob + h->off_cguide;
+            cv.cg_s = (uint32_t)__cvta_generic_to_shared(s_blob + h->off_cguide);
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
             cv.depth_bisect = h->depth_bisect; cv.cg_shift = h->cguide_shift;
             cv.gthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_gthr);
             cv.gcls = reinterpret_cast<const float2 *>(s_blob + h->off_gcls);
             cv.gas_steps = h->gas_steps; cv.vh_fs = h->vh_fs;
-            cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f;
+            cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f; cv.omr_q31 = h->omr_q31;
             cv.R_thr = h->R_thr; cv.surface_model = h->surface_model;
         }
         if (tid < 5) const_cast<uint4 *>(reinterpret_cast<const uint4 *>(cv.rows) - 5)[tid] = s_keys[tid];     // see PHILOX_MAIN
@@ -432,7 +456,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 acc_rare += wq;
             }
             // weight left in the surface: implicit capture, (1 - R) x the weights that reached it; analog, the absorbed weight
-            acc_abss += min(__float2uint_rn(abss * (ANALOG ? kWOneF : cv.one_minus_R * kWOneF)), kWOne - wq);
+            acc_abss += min(__float2uint_rn(abss * (ANALOG ? kWOneF : cv.omr_q31)), kWOne - wq);
             const uint32_t n_int = nfl - (ANALOG && fate == F_ABS_PART ? 1u : 0u);     // scatters + reflections
             cnt_fl += nfl;                                    // an absorbing interaction is a particle event too
             max_ev = max(max_ev, n_int);
@@ -448,7 +472,10 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
         // One flight (D2): `a` = path word, `cw` = class word (POLY), `b` = phase word, `pw` = azimuth / surface
         // polar-angle word, `ya` = absorption word (ANALOG), `sub` = which roulette word of the second block.
         // Returns F_NONE while the history goes on.
+        // `cw`: flights 0 and 1 of a group pass the RAW word (its low byte counts as 0x80: compared with thr24, pdv_device.h),
+        // flight 2 the assembled 32-bit class word (compared with thr)
         auto flight = [&](uint32_t a, uint32_t cw, uint32_t b, uint32_t pw, uint32_t ya, uint32_t y_roul, uint32_t sub) -> int {
+            const uint32_t thr_tab = sub == 2u ? 0u : (uint32_t)PDV_MAX_CLASSES;
             // ---------------- free flight: s = -ln(xi), xi in (0,1]; T' = T - mu s (Eq. 7/10, step (3)) ---------------
             // T is carried in units of ln 2 (so are the depth tables): -mu s / ln 2 = mu lg2(xi)
             const float xi = 2.0f - __uint_as_float(0x3F800000u | (a >> 9));
@@ -468,6 +495,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                 uint32_t bin;
                 const float zeta = gas_height(cv, T, bin);
                 if (POLY) {
+                    if (sub != 2u) cw = (cw & 0xFFFFFF00u) | 0x80u;
                     const uint32_t *t = cv.gthr + (bin << cv.gas_steps);
                     for (uint32_t st = 1u << cv.gas_steps >> 1; st > 0u; st >>= 1) c += t[c + st - 1u] <= cw ? st : 0u;
                     c = min(c, cv.n_classes - 1u);
@@ -478,10 +506,10 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             else vh = depth_half_velocity<DM == 2>(cv, T);
             if (POLY && DM != 3) {
                 // c = #{j : thr[j] <= cw} through the class guide (pdv_device.h); thr is padded with 0xffffffff
-                const uint32_t e = cv.cguide[cw >> cv.cg_shift];
+                const uint32_t e = lds_u8(cv.cg_s + (cw >> cv.cg_shift));
                 c = e & 0x7Fu;
-                c += cv.thr[c] <= cw ? 1u : 0u;
-                if (e & 0x80u) c = class_walk(cv.thr, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
+                c += cv.thr[thr_tab + c] <= cw ? 1u : 0u;
+                if (e & 0x80u) c = class_walk(cv.thr + thr_tab, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
                 c = min(c, cv.n_classes - 1u);
                 if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
             }
@@ -591,10 +619,10 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
                             if (ROUL) philox4x32_10(id_lo, id_hi, ud.stream, 2u * b2 + 3u, s_keys, yr0, yr1, yr2, yr3);
                         }
                         // class words: 24 bits of w2 and of w5, and (w2.byte0, w5.byte0, w6 bits 23..8) for the third flight
-                        fate = flight(w0, (w2 & 0xFFFFFF00u) | 0x80u, w1, __byte_perm(w0, w1, 0x0412), ya0, yr0, 0u);
-                        if (fate == F_NONE) fate = flight(w3, (w5 & 0xFFFFFF00u) | 0x80u, w4, __byte_perm(w3, w4, 0x0412), ya1, yr1, 1u);
-                        if (fate == F_NONE)
-                            fate = flight(w6, (w2 << 24) | ((w5 & 0xFFu) << 16) | ((w6 >> 8) & 0xFFFFu), w7, __byte_perm(w6, w7, 0x0412),
+                        fate = flight(w0, w2, w1, __byte_perm(w0, w1, 0x0412), ya0, yr0, 0u);
+                        if (fate == F_NONE) fate = flight(w3, w5, w4, __byte_perm(w3, w4, 0x0412), ya1, yr1, 1u);
+                        if (fate == F_NONE)       // (w2.byte0, w5.byte0, w6.byte2, w6.byte1) from the top
+                            fate = flight(w6, __byte_perm(__byte_perm(w6, w2, 0x4021), w5, 0x3410), w7, __byte_perm(w6, w7, 0x0412),
                                           ya2, yr2, 2u);
                     }
                 } else {
