@@ -248,7 +248,9 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
         int below, inside;
         cell_counts(cg_shift, g, below, inside);
         cg[g] = (unsigned char)(below | (inside > 1 ? 0x80 : 0));
+        if (inside > 1) ++hd.cguide_flagged;
     }
+    std::memcpy(blob.data(), &hd, sizeof(hd));
 }
 
 // Device images of destroyed clouds are kept for the next cloud instead of going back to the driver: cudaFree was measured at
@@ -441,7 +443,15 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
             const double f = estimated_flights(h.tau_ext, om, o);
             sum += f; sum2 += f * f;
         }
-        kv.long_hist = sum > 0.0 && sum2 / sum >= 45.0;
+        kv.alt = sum > 0.0 && sum2 / sum >= 45.0;
+    }
+    if (kv.poly) {       // several classes: alt = every class guide of the launch is clean
+        kv.alt = true;
+        for (int i = 0; i < n_clouds; ++i) {
+            DevCloudHeader hd;
+            std::memcpy(&hd, clouds[i]->blob.data(), sizeof(hd));
+            kv.alt = kv.alt && hd.cguide_flagged == 0u;
+        }
     }
     // dm 0: every cloud uses the one-probe depth table and the paper's surface law; 1: every cloud uses the closed-form
     // depth model and the paper's surface law; 2 (general kernel): anything else, decided per unit at run time
@@ -483,7 +493,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         static std::vector<std::pair<Key, int>> cache;       // occupancy queries are not free either
         std::lock_guard<std::mutex> lk(mu);
         for (const auto &e : cache)
-            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.dm == kv.dm && e.first.v.long_hist == kv.long_hist &&
+            if (e.first.v.poly == kv.poly && e.first.v.analog == kv.analog && e.first.v.sso == kv.sso && e.first.v.trace == kv.trace && e.first.v.roulette == kv.roulette && e.first.v.dm == kv.dm && e.first.v.alt == kv.alt &&
                 e.first.block == block && e.first.smem == smem && e.first.device == device) { per_sm = e.second; break; }
         if (per_sm == 0) {
             CU(transport_max_blocks_per_sm(kv, block, smem, &per_sm), "occupancy query");

@@ -89,6 +89,8 @@ struct DevCloudHeader {
     uint32_t gas;              // 1: this image is a gas unit
     uint32_t off_gthr, off_gcls, gas_steps;
     float omr_q31;             // (1 - R_f) 2^31: weight that reached the surface -> Q31 weight left in it
+    uint32_t cguide_flagged;   // number of class-guide cells that hold several thresholds (0: an entry is the class count itself)
+    uint32_t pad[3];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 
@@ -129,10 +131,12 @@ struct RunParams {
 struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
-// long_hist: the launch's histories are long (cost-weighted mean of the estimated flights per history >= 45): a one-class
-// kernel then flies several random draws between two end-of-history passes -- that pass runs at one or two lanes when histories
-// are long, and running it less often costs fewer issue slots than the lanes that wait for it (measured: profiles/README.md)
-struct KernelVariant { bool poly, analog, sso, trace, roulette; int dm; bool long_hist; };   // dm: see transport_kernel   // template instantiation of transport_kernel
+// alt: run the second production instantiation (transport_kernel's ALT).  One-class launches: the histories are long
+// (cost-weighted mean of the estimated flights per history >= 45), a lane then flies several random draws between two
+// end-of-history passes -- that pass runs at one or two lanes when histories are long, and running it less often costs fewer
+// issue slots than the lanes that wait for it (measured: profiles/README.md).  Polydisperse launches: no class-guide cell of
+// any cloud holds two thresholds (DevCloudHeader::cguide_flagged == 0 everywhere).
+struct KernelVariant { bool poly, analog, sso, trace, roulette; int dm; bool alt; };   // dm: see transport_kernel
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,

@@ -26,12 +26,9 @@ __shared__ unsigned int s_dbg[8];
 #define PDV_BOUND(cat, idx, limit) do { } while (0)
 #endif
 
-// Draws per pass of the LONG instantiations (experiment builds may override): see transport_kernel
+// Draws per pass of the long-history instantiations of the one-class kernel (experiment builds may override): see transport_kernel
 #ifndef PDV_DRAWS_LONG_MONO
 #define PDV_DRAWS_LONG_MONO 4
-#endif
-#ifndef PDV_DRAWS_LONG_POLY
-#define PDV_DRAWS_LONG_POLY 1
 #endif
 // Register budget of transport_kernel: PDV_LB_THREADS x PDV_LB_BLOCKS resident threads per SM (pdv_device.h).
 namespace pdv {
@@ -299,15 +296,18 @@ __device__ __noinline__ void drain_queue(uint32_t n_bins, float v_lo, float inv_
     __syncwarp();
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool ALT = false>
 __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
-    // Random draws (Philox blocks of a one-class cloud = 2 flights each, block pairs of a polydisperse one = 3 flights each) a
-    // lane flies between two end-of-history passes of its warp: 1, or 4 in the LONG instantiations of the one-class kernel,
-    // which the host picks for launches whose histories are long (KernelVariant::long_hist; config 4: 130.5 -> 124 ms).
-    // Polydisperse kernels always fly one draw (measured at 896 threads: config 5 275.9 / 272.4 / 274.0 ms, Figs. 13-15
-    // sweep 74.2 / 78.2 / 77.8 ms with 1 / 2 / 3 draws).  A compile-time constant: as a run-time loop bound it cost a
-    // register and spilled (config 2 3.81 -> 4.12 ms, config 3 +14 %).
-    constexpr uint32_t draws = LONG ? (POLY ? PDV_DRAWS_LONG_POLY : PDV_DRAWS_LONG_MONO) : 1;
+    // ALT: the second production instantiation of the implicit-capture depth-table kernels (KernelVariant::alt).
+    // One class -- LONG histories: a lane flies 4 random draws (Philox blocks = 2 flights each) between two end-of-history
+    // passes of its warp instead of 1; the host picks it for launches whose histories are long (config 4).  A compile-time
+    // constant: as a run-time loop bound it cost a register and spilled (config 2 +8 %).
+    // Several classes -- CLEAN class guides: no guide cell of any cloud of the launch holds two thresholds, so an entry IS
+    // the class count below its cell (no flag bit to mask or test) and the out-of-line walk with its BSSY / BRA / BSYNC is
+    // compiled out of every flight.  (More draws per pass never paid for polydisperse kernels: 1 / 2 / 3 draws at 896 threads
+    // gave config 5 275.9 / 272.4 / 274.0 ms, Figs. 13-15 sweep 74.2 / 78.2 / 77.8 ms.)
+    constexpr uint32_t draws = ALT && !POLY ? PDV_DRAWS_LONG_MONO : 1;
+    constexpr bool WALK = !(ALT && POLY);                     // class-guide cells may hold several thresholds
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     __shared__ int s_go;
     constexpr bool QUEUE = !TRACE;                            // aperture hits go through the warp's detection queue
@@ -507,9 +507,9 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
             if (POLY && DM != 3) {
                 // c = #{j : thr[j] <= cw} through the class guide (pdv_device.h); thr is padded with 0xffffffff
                 const uint32_t e = lds_u8(cv.cg_s + (cw >> cv.cg_shift));
-                c = e & 0x7Fu;
+                c = WALK ? e & 0x7Fu : e;
                 c += cv.thr[thr_tab + c] <= cw ? 1u : 0u;
-                if (e & 0x80u) c = class_walk(cv.thr + thr_tab, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
+                if (WALK && (e & 0x80u)) c = class_walk(cv.thr + thr_tab, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
                 c = min(c, cv.n_classes - 1u);
                 if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
             }
@@ -695,11 +695,11 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, P
 
 // ------------------------------------------------------------------------------------------------------------
 // The dynamic shared memory limit of an instantiation is only ever raised (it is a per-function attribute).
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool ALT = false>
 static cudaError_t ensure_smem(int smem) {
     static int smem_set = 48 * 1024 - (int)sizeof(WarpShared) * 32 - 2048;      // static + dynamic above 48 KB needs the opt-in
     if (smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>,
+        cudaError_t e = cudaFuncSetAttribute(transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         smem_set = smem;
@@ -707,19 +707,19 @@ static cudaError_t ensure_smem(int smem) {
     return cudaSuccess;
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool ALT = false>
 static cudaError_t launch_t(const RunParams &rp, LaunchShape s, cudaStream_t st) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>(s.smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT>(s.smem);
     if (e != cudaSuccess) return e;
-    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG><<<s.grid, s.block, s.smem, st>>>(rp);
+    transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT><<<s.grid, s.block, s.smem, st>>>(rp);
     return cudaGetLastError();
 }
 
-template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool LONG = false>
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool ALT = false>
 static cudaError_t occ_t(int block, int smem, int *out) {
-    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>(smem);
+    cudaError_t e = ensure_smem<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT>(smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, LONG>, block, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT>, block, smem);
 }
 
 // DM = 0 / 1 exist for the production variants only; single-scatter-only and trace runs always take the general kernel.
@@ -747,19 +747,20 @@ static cudaError_t occ_dm(int dm, int block, int smem, int *out) {
 #define PDV_D3(FN, A, ...) (v.analog ? PDV_D2(FN, A, true, __VA_ARGS__) : PDV_D2(FN, A, false, __VA_ARGS__))
 #define PDV_DISPATCH(FN, ...) (v.poly ? PDV_D3(FN, true, __VA_ARGS__) : PDV_D3(FN, false, __VA_ARGS__))
 
-// LONG instantiations exist for the production variants of the one-class depth-table kernel only (implicit capture, no
-// single-scatter cut, no trace, DM 0): the thick sweeps of config 4.
-static bool long_variant(const KernelVariant &v) { return v.long_hist && !v.poly && !v.analog && !v.sso && !v.trace && v.dm == 0; }
+// ALT instantiations exist for the production variants of the depth-table kernels only (implicit capture, no single-scatter
+// cut, no trace, DM 0): long histories of one-class clouds (the thick sweeps of config 4), clean class guides of polydisperse ones.
+static bool alt_variant(const KernelVariant &v) { return v.alt && !v.analog && !v.sso && !v.trace && v.dm == 0; }
 
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st) {
 #ifdef PDV_FEW
-    if (!long_variant(v)) {
+    if (!alt_variant(v)) {
         if (v.analog || v.sso || v.trace || v.dm != 0) return cudaErrorNotSupported;
         if (!v.poly) return v.roulette ? cudaErrorNotSupported : launch_t<false, false, false, false, false, 0>(rp, shape, st);
         return v.roulette ? launch_t<true, false, false, false, true, 0>(rp, shape, st) : launch_t<true, false, false, false, false, 0>(rp, shape, st);
     }
 #endif
-    if (long_variant(v)) {
+    if (alt_variant(v)) {
+        if (v.poly) return v.roulette ? launch_t<true, false, false, false, true, 0, true>(rp, shape, st) : launch_t<true, false, false, false, false, 0, true>(rp, shape, st);
         return v.roulette ? launch_t<false, false, false, false, true, 0, true>(rp, shape, st) : launch_t<false, false, false, false, false, 0, true>(rp, shape, st);
     }
 #ifdef PDV_FEW
@@ -771,13 +772,14 @@ cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape s
 
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out) {
 #ifdef PDV_FEW
-    if (!long_variant(v)) {
+    if (!alt_variant(v)) {
         if (v.analog || v.sso || v.trace || v.dm != 0) return cudaErrorNotSupported;
         if (!v.poly) return v.roulette ? cudaErrorNotSupported : occ_t<false, false, false, false, false, 0>(block, smem, out);
         return v.roulette ? occ_t<true, false, false, false, true, 0>(block, smem, out) : occ_t<true, false, false, false, false, 0>(block, smem, out);
     }
 #endif
-    if (long_variant(v)) {
+    if (alt_variant(v)) {
+        if (v.poly) return v.roulette ? occ_t<true, false, false, false, true, 0, true>(block, smem, out) : occ_t<true, false, false, false, false, 0, true>(block, smem, out);
         return v.roulette ? occ_t<false, false, false, false, true, 0, true>(block, smem, out) : occ_t<false, false, false, false, false, 0, true>(block, smem, out);
     }
 #ifdef PDV_FEW
