@@ -9,6 +9,7 @@
 #include <mutex>
 #include <new>
 #include <string>
+#include <deque>
 #include <vector>
 
 #include "pdv_device.h"
@@ -254,29 +255,45 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
 }
 
 // Device images of destroyed clouds are kept for the next cloud instead of going back to the driver: cudaFree was measured at
-// 0.5 ... 750 ms for the 14 images of a sweep (it synchronises the device and may unmap memory).  At most 64 buffers / 64 MiB.
+// 0.5 ... 750 ms for the 14 images of a sweep (it synchronises the device and may unmap memory).  Buffers come in power-of-two
+// sizes from 64 KiB, so the image of one workload fits the buffer another left behind.  At most 256 buffers / 256 MiB; when
+// that is full the OLDEST buffer goes back to the driver and the new one stays -- a loop that creates and destroys the same
+// clouds never reaches cudaMalloc / cudaFree after its first turn, whatever ran before it (round 2: the 14-cloud sweep at the
+// end of bench.py's default run took 426 ms per end-to-end step instead of 66, the cache being full of smaller buffers).
 struct BlobCache {
     struct Entry { unsigned char *p; size_t bytes; int device; };
     std::mutex mu;
-    std::vector<Entry> free_list;
+    std::deque<Entry> free_list;                               // oldest first
     size_t total = 0;
-    unsigned char *take(size_t bytes, int device) {           // smallest cached buffer that is large enough
-        std::lock_guard<std::mutex> lk(mu);
-        int best = -1;
-        for (int i = 0; i < (int)free_list.size(); ++i)
-            if (free_list[i].device == device && free_list[i].bytes >= bytes && (best < 0 || free_list[i].bytes < free_list[best].bytes)) best = i;
-        if (best < 0) return nullptr;
-        unsigned char *p = free_list[best].p;
-        total -= free_list[best].bytes;
-        free_list.erase(free_list.begin() + best);
-        return p;
+    static size_t capacity_for(size_t bytes) {
+        size_t cap = (size_t)64 << 10;
+        while (cap < bytes) cap <<= 1;
+        return cap;
     }
-    bool give(unsigned char *p, size_t bytes, int device) {
+    unsigned char *take(size_t cap, int device) {             // a cached buffer of exactly this capacity
         std::lock_guard<std::mutex> lk(mu);
-        if (free_list.size() >= 64 || total + bytes > ((size_t)64 << 20)) return false;
-        free_list.push_back({p, bytes, device});
-        total += bytes;
-        return true;
+        for (size_t i = free_list.size(); i-- > 0;)
+            if (free_list[i].device == device && free_list[i].bytes == cap) {
+                unsigned char *p = free_list[i].p;
+                total -= cap;
+                free_list.erase(free_list.begin() + (long)i);
+                return p;
+            }
+        return nullptr;
+    }
+    void give(unsigned char *p, size_t cap, int device) {
+        std::vector<unsigned char *> evict;
+        {
+            std::lock_guard<std::mutex> lk(mu);
+            free_list.push_back({p, cap, device});
+            total += cap;
+            while (free_list.size() > 256 || total > ((size_t)256 << 20)) {
+                evict.push_back(free_list.front().p);
+                total -= free_list.front().bytes;
+                free_list.pop_front();
+            }
+        }
+        for (unsigned char *q : evict) cudaFree(q);
     }
 };
 BlobCache g_blob_cache;
@@ -285,15 +302,16 @@ pdv_status ensure_on_device(const pdv_cloud *c, int device) {
     std::lock_guard<std::mutex> lk(c->mu);
     if (c->d_blob && c->device == device) return PDV_OK;
     if (c->d_blob) return fail(PDV_E_INVALID, "cloud was uploaded to another CUDA device");
-    unsigned char *d = g_blob_cache.take(c->blob.size(), device);
+    const size_t cap = BlobCache::capacity_for(c->blob.size());
+    unsigned char *d = g_blob_cache.take(cap, device);
     if (d) {
         // the buffer belonged to a destroyed cloud: whatever may still read it (a run enqueued on a non-blocking stream)
         // must be over before it is overwritten -- what cudaFree used to guarantee
         CU(cudaDeviceSynchronize(), "cudaDeviceSynchronize(reuse of a cloud buffer)");
     } else {
-        CU(cudaMalloc(&d, c->blob.size()), "cudaMalloc(cloud tables)");
+        CU(cudaMalloc(&d, cap), "cudaMalloc(cloud tables)");
     }
-    c->d_bytes = c->blob.size();                              // a reused buffer may be larger: only this much is vouched for
+    c->d_bytes = cap;                                         // capacity of the buffer (the image fills blob.size() of it)
     cudaError_t e = cudaMemcpy(d, c->blob.data(), c->blob.size(), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(cloud tables)"); }
     c->d_blob = d;
@@ -722,7 +740,7 @@ pdv_status pdv_cloud_create(const pdv_cloud_params *params, pdv_cloud **out) {
 
 void pdv_cloud_destroy(pdv_cloud *c) {
     if (!c) return;
-    if (c->d_blob && !g_blob_cache.give(c->d_blob, c->d_bytes, c->device)) cudaFree(c->d_blob);
+    if (c->d_blob) g_blob_cache.give(c->d_blob, c->d_bytes, c->device);
     delete c;
 }
 
