@@ -461,7 +461,10 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
             const double f = estimated_flights(h.tau_ext, om, o);
             sum += f; sum2 += f * f;
         }
-        kv.alt = sum > 0.0 && sum2 / sum >= 45.0;
+#ifndef PDV_ALT_MIN_FLIGHTS
+#define PDV_ALT_MIN_FLIGHTS 45.0          /* experiment builds may override */
+#endif
+        kv.alt = sum > 0.0 && sum2 / sum >= PDV_ALT_MIN_FLIGHTS;
     }
     if (kv.poly) {       // several classes: alt = every class guide of the launch is clean
         kv.alt = true;
