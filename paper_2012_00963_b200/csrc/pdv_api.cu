@@ -507,7 +507,10 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     // one class: 1024 resident threads per SM either way.  Several units: two blocks of 512 when their shared memory fits twice
     // (finer grain where blocks move from unit to unit: config 4 123.9 ms against 135.3 with one block of 1024); ONE unit: one
     // block of 1024 (half as many stagings, flushes and warp pools: config 2 3.73 ms against 3.81)
-    if (block == 0) block = (n_units > 1 && 2 * (size_t)(smem + 1024 + 18432) <= di.smem_optin + 1024) ? 512 : 1024;   // 18 KB: the kernel's static shared memory (warp queues)
+    // long histories (the ALT instantiation of the production one-class kernel): PDV_LB_THREADS_LONG resident threads at 80 registers
+    const int lb = !kv.poly && kv.alt && !kv.analog && !kv.sso && !kv.trace && kv.dm == 0 ? PDV_LB_THREADS_LONG : PDV_LB_THREADS;
+    if (block == 0) block = (n_units > 1 && 2 * (size_t)(smem + 1024 + 18432) <= di.smem_optin + 1024) ? lb / 2 : lb;   // 18 KB: the kernel's static shared memory (warp queues)
+    block = std::min(block, lb);
     {
         struct Key { KernelVariant v; int block, smem, device; };
         static std::mutex mu;

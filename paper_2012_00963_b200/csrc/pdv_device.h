@@ -18,6 +18,12 @@
 #ifndef PDV_LB_THREADS_POLY
 #define PDV_LB_THREADS_POLY 1024
 #endif
+// The long-history instantiations of the one-class kernel (ALT, four draws per pass) are compiled for PDV_LB_THREADS_LONG resident
+// threads (80 registers: no spill; at 64 registers they spilled 16 ... 40 bytes) and launched as blocks of half that size.  Config 4:
+// 512 x 2 at 64 registers 118.3 ms; 384 x 2 at 80 registers 111.2; 256 x 3 111.4; 320 x 2 at 102 registers 109.9; 256 x 4 at 64: 120.2.
+#ifndef PDV_LB_THREADS_LONG
+#define PDV_LB_THREADS_LONG 768
+#endif
 #ifndef PDV_LB_BLOCKS
 #define PDV_LB_BLOCKS 1
 #endif

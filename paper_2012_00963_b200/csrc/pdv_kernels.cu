@@ -297,7 +297,7 @@ __device__ __noinline__ void drain_queue(uint32_t n_bins, float v_lo, float inv_
 }
 
 template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool ALT = false>
-__global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
+__global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THREADS_LONG : PDV_LB_THREADS, PDV_LB_BLOCKS) transport_kernel(const __grid_constant__ RunParams P) {
     // ALT: the second production instantiation of the implicit-capture depth-table kernels (KernelVariant::alt).
     // One class -- LONG histories: a lane flies 4 random draws (Philox blocks = 2 flights each) between two end-of-history
     // passes of its warp instead of 1; the host picks it for launches whose histories are long (config 4).  A compile-time
