@@ -299,9 +299,13 @@ pdv_status pdv_issue_peaks(double millis, double *ffma_thread_inst_per_s, double
 
 /* Launch statistics of the last pdv_mc_run / pdv_mc_trace on this thread: kernels launched and the duration of
  * the transport kernel in ms measured with CUDA events on cuda_stream.  After an output_on_device = 1 run this
- * call waits (cudaEventSynchronize) for that run's transport kernel to finish.  Any pointer may be NULL. */
+ * call waits (cudaEventSynchronize) for that run's transport kernel to finish.  Any pointer may be NULL.
+ * variant: which instantiation of the transport kernel ran -- bit 0 several size classes, bit 1 analog absorption,
+ * bit 2 single-scatter-only, bit 3 trace, bit 4 Russian roulette, bit 5 the second production instantiation (one
+ * class: long histories, several draws per pass; several classes: clean class guides), bits 8.. the depth model
+ * (0 depth table, 1 closed form, 2 general, 3 gas units).  The result of a run never depends on it. */
 pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block,
-                                int32_t *smem_bytes);
+                                int32_t *smem_bytes, int32_t *variant);
 
 /* Thread-local message of the last failing call on this thread; "" if none.  Valid until the next call. */
 const char *pdv_last_error(void);

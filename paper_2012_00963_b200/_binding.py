@@ -104,7 +104,7 @@ def lib() -> C.CDLL:
         L.pdv_phase_sampling_check.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int32, vp, vp, C.POINTER(PhaseCheck), vp]
         L.pdv_issue_peaks.argtypes = [C.c_double, dp, dp, dp, C.POINTER(C.c_int32), vp]
         L.pdv_last_launch_info.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32),
-                                           C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+                                           C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.pdv_last_error.restype = C.c_char_p
         L.pdv_version.restype = C.c_char_p
         for name in EXPORTS:
@@ -376,7 +376,8 @@ def pdv_issue_peaks(millis: float = 50.0, stream: int | None = None) -> dict:
 
 
 def pdv_last_launch_info() -> dict:
-    k, g, b, s = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0)
+    k, g, b, s, v = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0)
     ms = C.c_float(0)
-    lib().pdv_last_launch_info(C.byref(k), C.byref(ms), C.byref(g), C.byref(b), C.byref(s))
-    return dict(n_kernels=k.value, transport_ms=ms.value, grid=g.value, block=b.value, smem_bytes=s.value)
+    lib().pdv_last_launch_info(C.byref(k), C.byref(ms), C.byref(g), C.byref(b), C.byref(s), C.byref(v))
+    return dict(n_kernels=k.value, transport_ms=ms.value, grid=g.value, block=b.value, smem_bytes=s.value, variant=v.value,
+                alt=bool(v.value & 32))

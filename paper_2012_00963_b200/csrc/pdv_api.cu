@@ -29,7 +29,7 @@ struct pdv_cloud {
 namespace {
 
 thread_local std::string g_err;
-thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0; bool pending = false; } g_last;
+thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0, variant = 0; bool pending = false; } g_last;
 
 // Timing events of the last run of this host thread (pdv_last_launch_info).
 struct LastEvents {
@@ -659,6 +659,12 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *
 
     g_last.n_kernels = 0; g_last.ms = 0.f; g_last.pending = false;
     g_last.grid = plan.shape.grid; g_last.block = plan.shape.block; g_last.smem = plan.shape.smem;
+    {
+        const KernelVariant &v = plan.variant;
+        const bool alt = v.alt && !v.analog && !v.sso && !v.trace && v.dm == 0;          // the ALT instantiation exists and was launched
+        g_last.variant = (v.poly ? 1 : 0) | (v.analog ? 2 : 0) | (v.sso ? 4 : 0) | (v.trace ? 8 : 0) | (v.roulette ? 16 : 0) | (alt ? 32 : 0) |
+                         ((v.sso || v.trace ? 2 : v.dm) << 8);
+    }
     CUX(cudaEventRecord(g_ev.e0, st), "cudaEventRecord");
     if (n_photons > 0) {
         CUX(launch_transport(rp, plan.variant, plan.shape, st), "transport kernel launch");
@@ -1004,7 +1010,7 @@ pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mh
     return PDV_OK;
 }
 
-pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes) {
+pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes, int32_t *variant) {
     if (g_last.pending && g_ev.e0 && g_ev.e1) {      // output_on_device run: wait for its transport kernel only
         float ms = 0.f;
         if (cudaEventSynchronize(g_ev.e1) == cudaSuccess && cudaEventElapsedTime(&ms, g_ev.e0, g_ev.e1) == cudaSuccess)
@@ -1018,6 +1024,7 @@ pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t
     if (grid) *grid = g_last.grid;
     if (block) *block = g_last.block;
     if (smem_bytes) *smem_bytes = g_last.smem;
+    if (variant) *variant = g_last.variant;
     return PDV_OK;
 }
 

@@ -414,6 +414,44 @@ def test_sharded_runs_reduce_to_the_single_run_bit_for_bit(P, idx, n_snap, n_clo
         assert np.array_equal(st[k], whole.stats.reshape(-1)[k]), k
 
 
+def test_second_production_instantiation_gives_the_same_tallies(P):
+    """The ALT instantiations must not change a single bit.  Several classes: a cloud whose class guide is
+    clean runs ALT alone, and the plain instantiation when a cloud with a flagged guide cell (config 5's tiny classes) rides in
+    the same launch.  One class: a thin cloud runs one draw per pass alone, and four (long histories) next to a thick cloud.
+    unit_streams gives the unit the same sub-stream in both launches."""
+    for probe, other in ((W.config(2)["clouds"][0], W.config(4)["clouds"][0]),                 # 16 classes: clean / flagged guide
+                         (W.config(1)["clouds"][0], W._cloud(20.0, 6.0, 2000.0, diameter_um=1.0))):     # one class: tau 1.9 / 108
+        run = dict(W.config(1)["run"], n_bins=512, v_hi=9000.0)
+        n = 300_007
+        a, b = P.pdv_cloud_create(probe), P.pdv_cloud_create(other)
+        poly = len(probe.get("diameters", [])) > 1 or "lognormal" in probe
+        alone = P.pdv_mc_run([a], [2.0e-6], n, 77, dict(run, unit_streams=[5]))
+        alt_alone = P.pdv_last_launch_info()["alt"]
+        both = P.pdv_mc_run([b, a], [2.0e-6], n, 77, dict(run, unit_streams=[9, 5]))
+        alt_both = P.pdv_last_launch_info()["alt"]
+        assert alt_alone != alt_both, (poly, alt_alone, alt_both)      # the two launches did run different instantiations
+        assert alt_alone == poly
+        assert np.array_equal(alone.hist[0, 0], both.hist[1, 0]) and np.array_equal(alone.hist2[0, 0], both.hist2[1, 0])
+        for k in alone.stats.dtype.names:
+            assert alone.stats[0, 0][k] == both.stats[1, 0][k], k
+        assert float(alone.stats[0, 0]["detected"]) > 0
+
+
+def test_detection_queue_under_full_load(P):
+    """Every history is a detection (aperture 2 pi, empty cloud: each photon reflects once and leaves): every lane of a warp pushes
+    on the detection queue in the same pass, the queue is tallied every pass, and the counts must still be exact."""
+    params = W._cloud(0.0, 4.0, 2000.0, diameter_um=5.0)
+    run = dict(W.config(0)["run"], aperture_sr=2.0 * math.pi, n_bins=64)
+    n = 1_000_003
+    r = P.pdv_mc_run([P.pdv_cloud_create(params)], [2.0e-6], n, 5, run)
+    s = r.stats[0, 0]
+    assert int(s["histories"]) == n and int(s["surface_reflections"]) == n and int(s["particle_events"]) == 0
+    assert r.conservation_residual()[0, 0] == 0.0
+    # weight R per history, all inside [0, v_fs): Q31 sums are exact
+    assert float(s["detected"]) + float(s["underflow"]) + float(s["overflow"]) == pytest.approx(0.6 * n, rel=1e-6)
+    assert r.hist[0, 0].sum() == pytest.approx(float(s["detected"]), rel=1e-12)
+
+
 def test_photon_count_limit_of_the_fixed_point_tallies(P):
     cfg = W.config(1)
     c = P.pdv_cloud_create(cfg["clouds"][0])
