@@ -124,12 +124,15 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     DevCloudHeader hd;
     std::memset(&hd, 0, sizeof(hd));
     size_t off = sizeof(DevCloudHeader);
-    hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * 2 * (size_t)nc * K);
+    // a one-class cloud carries its phase table and albedo twice: in a polydisperse launch without the class clamp (transport_kernel's
+    // ALT) a class word of 0xffffffff picks "class 1" of such a cloud -- it must be the same class
+    const int nc_tab = nc == 1 ? 2 : nc;
+    hd.off_phase = (uint32_t)off;  off = align16(off + sizeof(float) * 2 * (size_t)nc_tab * K);
     off += 80;                                                // the block writes its Philox round keys in front of the rows (pdv_device.h)
     hd.off_rows = (uint32_t)off;   off = align16(off + sizeof(float) * 4 * (size_t)nd);
     hd.off_thr = (uint32_t)off;    off = align16(off + sizeof(uint32_t) * 2 * PDV_MAX_CLASSES);     // thr[32] | thr24[32] (pdv_device.h)
-    hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * n_pad);
-    hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * n_pad);
+    hd.off_albedo = (uint32_t)off; off = align16(off + sizeof(float) * std::max(n_pad, 2));
+    hd.off_albthr = (uint32_t)off; off = align16(off + sizeof(uint32_t) * std::max(n_pad, 2));
     hd.off_guide = (uint32_t)off;  off = align16(off + sizeof(uint16_t) * n_guide);
     // class thresholds first: the class guide is sized from them (layout: pdv_device.h)
     std::vector<uint32_t> thr_v(n_pad, 0xFFFFFFFFu);
@@ -191,7 +194,8 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     std::memcpy(blob.data(), &hd, sizeof(hd));
     float *ph = reinterpret_cast<float *>(blob.data() + hd.off_phase);
     std::vector<float> Mf(K + 1);
-    for (int c = 0; c < nc; ++c) {
+    for (int ct = 0; ct < nc_tab; ++ct) {
+        const int c = ct < nc ? ct : 0;
         float prev = -1.f;
         for (int k = 0; k <= K; ++k) {
             float v = (float)h.phase[(size_t)c * (K + 1) + k];
@@ -200,8 +204,8 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
             prev = v;
         }
         for (int k = 0; k < K; ++k) {                         // (M[k], (M[k+1] - M[k]) 2^-shiftK): layout in pdv_device.h
-            ph[2 * ((size_t)c * K + k) + 0] = Mf[k];
-            ph[2 * ((size_t)c * K + k) + 1] = (float)std::ldexp((double)Mf[k + 1] - (double)Mf[k], -(int)shiftK);
+            ph[2 * ((size_t)ct * K + k) + 0] = Mf[k];
+            ph[2 * ((size_t)ct * K + k) + 1] = (float)std::ldexp((double)Mf[k + 1] - (double)Mf[k], -(int)shiftK);
         }
     }
     float *rows = reinterpret_cast<float *>(blob.data() + hd.off_rows);
@@ -228,6 +232,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
         alb[c] = (float)std::min(std::max(om, 0.0), 1.0);
         albt[c] = to_thr32(om);
     }
+    if (nc == 1) { alb[1] = alb[0]; albt[1] = albt[0]; }
     std::memcpy(blob.data() + hd.off_guide, guide.data(), sizeof(uint16_t) * n_guide);
     if (gu) {
         uint32_t *gt = reinterpret_cast<uint32_t *>(blob.data() + hd.off_gthr);
@@ -248,6 +253,9 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
     for (uint32_t g = 0; nc > 1 && g < n_cg; ++g) {
         int below, inside;
         cell_counts(cg_shift, g, below, inside);
+        // a cell above every threshold points at the LAST threshold (below it, so the compare is true and the class is nc - 1)
+        // instead of at the padding behind it: the padding (0xffffffff) is then never compared, and the class needs no clamp
+        if (below == nc - 1) below = nc - 2;
         cg[g] = (unsigned char)(below | (inside > 1 ? 0x80 : 0));
         if (inside > 1) ++hd.cguide_flagged;
     }

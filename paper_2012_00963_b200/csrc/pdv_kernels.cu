@@ -508,9 +508,14 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
                 // c = #{j : thr[j] <= cw} through the class guide (pdv_device.h); thr is padded with 0xffffffff
                 const uint32_t e = lds_u8(cv.cg_s + (cw >> cv.cg_shift));
                 c = WALK ? e & 0x7Fu : e;
-                c += cv.thr[thr_tab + c] <= cw ? 1u : 0u;
+                {   // c += thr[c] <= cw, as one compare and one predicated add (the compiler's version: add, compare, move)
+                    const uint32_t t = cv.thr[thr_tab + c];
+                    asm("{\n\t.reg .pred p;\n\tsetp.le.u32 p, %1, %2;\n\t@p add.u32 %0, %0, 1;\n\t}" : "+r"(c) : "r"(t), "r"(cw));
+                }
                 if (WALK && (e & 0x80u)) c = class_walk(cv.thr + thr_tab, c, cv.n_classes - 1u, cw);      // rare cells with several thresholds
-                c = min(c, cv.n_classes - 1u);
+                // the guide never points at the padding behind the last threshold (pdv_api.cu::build_blob), so without the walk
+                // c <= n_classes - 1 by construction
+                if (WALK) c = min(c, cv.n_classes - 1u);
                 if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
             }
             if (ANALOG) {                                     // Eq. 11 literally: absorbed with probability 1 - albedo

@@ -437,6 +437,27 @@ def test_second_production_instantiation_gives_the_same_tallies(P):
         assert float(alone.stats[0, 0]["detected"]) > 0
 
 
+def test_one_class_cloud_inside_a_polydisperse_launch(P):
+    """A one-class cloud that rides in a polydisperse launch runs through the class pick (guide of zeros, padded thresholds,
+    its table and albedo stored twice): its spectrum must agree with the one-class kernel's (another random word map, so
+    statistically) and its weights must be conserved exactly."""
+    mono, poly = W.config(1)["clouds"][0], W.config(2)["clouds"][0]
+    run = W.config(1)["run"]
+    n = 2_000_000
+    a, b = P.pdv_cloud_create(mono), P.pdv_cloud_create(poly)
+    alone = P.pdv_mc_run([a], [3.0e-6], n, 31, run)
+    assert not (P.pdv_last_launch_info()["variant"] & 1)
+    mixed = P.pdv_mc_run([b, a], [3.0e-6], n, 32, run)
+    assert P.pdv_last_launch_info()["variant"] & 1 and P.pdv_last_launch_info()["alt"]
+    assert mixed.conservation_residual()[1, 0] == 0.0
+    res = compare(alone.hist[0, 0], alone.hist2[0, 0], n, mixed.hist[1, 0], mixed.hist2[1, 0], n)
+    assert res["ndf"] >= 50 and res["worst"] < 5.0, res["z"]
+    for k in ("detected", "escaped", "absorbed_particles", "absorbed_surface"):
+        x, y = float(alone.stats[0, 0][k]) / n, float(mixed.stats[1, 0][k]) / n
+        assert abs(x - y) < 5 * math.sqrt((x + y) / n), (k, x, y)
+    assert int(mixed.stats[1, 0]["particle_events"]) == pytest.approx(int(alone.stats[0, 0]["particle_events"]), rel=5e-3)
+
+
 def test_detection_queue_under_full_load(P):
     """Every history is a detection (aperture 2 pi, empty cloud: each photon reflects once and leaves): every lane of a warp pushes
     on the detection queue in the same pass, the queue is tallied every pass, and the counts must still be exact."""
