@@ -162,7 +162,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
         }
         if (clean) break;
     }
-    const uint32_t n_cg = nc > 1 ? 1u << (32 - cg_shift) : 16u;
+    const uint32_t n_cg = 1u << (32 - cg_shift);             // one class: 256 zeros (a polydisperse launch reads the guide of every cloud)
     hd.off_cguide = (uint32_t)off; off = align16(off + n_cg);
     hd.cguide_shift = cg_shift;
     if (gu) {

@@ -5,16 +5,19 @@
 //     same pass ("photon regeneration"), taking the next id of its warp's pool; a warp refills its pool from the unit's
 //     global cursor (guided pool sizes: large at the start, 32 at the end), so all 32 lanes of a warp fly a photon in every
 //     iteration until the unit is drained;
-//   * every history draws from its own Philox4x32-10 counter stream, counter = (id_lo, id_hi, unit, 2*flight+sub),
+//   * every history draws from its own Philox4x32-10 counter stream, counter = (id_lo, id_hi, unit, 2*block+sub),
 //     key = seed: results do not depend on which lane, warp or block runs a history (D1/D2);
-//   * the cloud tables (inverse-CDF phase tables, depth rows + guide, class thresholds) live in shared memory;
-//   * one loop iteration = one flight: free flight in vertical optical depth T (exact sampling of Eq. 7/10), then
-//     either the photon leaves through the top (tally, Eq. 19) or it interacts.  Particle scattering (Eq. 11,
-//     13-17) and free-surface reflection run through ONE branch-free instruction stream with
-//     selects: a reflection is "a scatter with albedo R, velocity v_fs and an absolute new direction";
+//   * the cloud tables (inverse-CDF phase tables, depth rows + guide, class thresholds + guide) live in shared memory;
+//   * one loop iteration (a "pass") = one group of random words -- one Philox block = two flights of a one-class cloud, two
+//     blocks = three flights of a polydisperse one -- and ONE reconverged end-of-history region for the lanes whose history
+//     ended in any of them.  A flight: free flight in vertical optical depth T (exact sampling of Eq. 7/10; T in units of
+//     ln 2), then either the photon leaves through the top or it interacts.  Particle scattering (Eq. 11, 13-17) and
+//     free-surface reflection run through ONE branch-free instruction stream with selects: a reflection is
+//     "a scatter with albedo R, velocity v_fs and an absolute new direction";
 //   * only mu = u_z is tracked (z row of Eq. 16 / Eq. 17; exact in slab geometry, reading R7);
-//   * Doppler update Eq. 4 with half velocities from the depth rows; weights and tallies are Q31 integers;
-//     the block's private shared-memory histogram is flushed once per block and unit.
+//   * Doppler update Eq. 4 with half velocities from the depth rows; weights and tallies are Q31 integers; a history that
+//     leaves inside the aperture is pushed on its warp's detection queue and tallied (Eq. 19) by the whole warp, 32 at a
+//     time; the block's private shared-memory histogram is flushed once per block and unit.
 #include "pdv_device.h"
 
 #ifdef PDV_DEBUG_BOUNDS
@@ -240,7 +243,6 @@ __device__ __forceinline__ RouletteOut roulette(float w, float abss, uint32_t yr
     const float wn = fminf(w * s_roul_inv_p, 1.f);
     const uint32_t q0 = __float2uint_rn(w * kWOneF), q1 = __float2uint_rn(wn * kWOneF);
     const uint32_t gain = q1 > q0 ? q1 - q0 : 0u;
-    smem_add64(&s_stats[ST_GAINED], gain);
     o.add_lost = gain;
     // surface losses so far go to the tally now: afterwards `abss` again stays below 1 - w
     o.add_abss = min(__float2uint_rn(abss * kWOneF), kWOne - q0);
@@ -516,6 +518,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
                 // the guide never points at the padding behind the last threshold (pdv_api.cu::build_blob), so without the walk
                 // c <= n_classes - 1 by construction
                 if (WALK) c = min(c, cv.n_classes - 1u);
+                PDV_BOUND(3, c, max(cv.n_classes, 2u));
                 if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
             }
             if (ANALOG) {                                     // Eq. 11 literally: absorbed with probability 1 - albedo
@@ -657,6 +660,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
             acc_esc += __shfl_xor_sync(FULL_MASK, acc_esc, o);
             acc_absp += __shfl_xor_sync(FULL_MASK, acc_absp, o);
             acc_abss += __shfl_xor_sync(FULL_MASK, acc_abss, o);
+            if (ROUL) acc_gain += __shfl_xor_sync(FULL_MASK, acc_gain, o);
             cnt_hist += __shfl_xor_sync(FULL_MASK, cnt_hist, o);
             cnt_ev += __shfl_xor_sync(FULL_MASK, cnt_ev, o);
             cnt_refl += __shfl_xor_sync(FULL_MASK, cnt_refl, o);
@@ -666,6 +670,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
             atomicAdd(&s_stats[ST_ESCAPED], acc_esc);
             atomicAdd(&s_stats[ST_ABS_PART], acc_absp);
             atomicAdd(&s_stats[ST_ABS_SURF], acc_abss);
+            if (ROUL) atomicAdd(&s_stats[ST_GAINED], acc_gain);      // the games only add to the thread's sum (no atomics in a game)
             atomicAdd(&s_stats[ST_HISTORIES], (unsigned long long)cnt_hist);
             atomicAdd(&s_stats[ST_EVENTS], (unsigned long long)cnt_ev);
             atomicAdd(&s_stats[ST_REFLECT], (unsigned long long)cnt_refl);
