@@ -121,6 +121,24 @@ pdv_status pdv_cloud_get_info(const pdv_cloud *cloud, pdv_cloud_info *out);
 pdv_status pdv_cloud_get_tables(const pdv_cloud *cloud, double *k_ext, double *k_sca, double *g, double *p_class,
                                 double *phase, double *T_edge);
 
+/* Diagnostic: the DEVICE IMAGE of a cloud in vacuum -- the fp32 / integer tables each block stages in shared memory
+ * (layout and meaning of every section: csrc/pdv_device.h) -- with the offsets and parameters needed to read it.  For
+ * tests of the host logic that builds it (guides, thresholds, units); needs no GPU.  `image` may be NULL (layout only);
+ * otherwise it receives min(capacity, image_bytes) bytes.  Optical depths in the image are in units of ln 2. */
+typedef struct {
+    size_t struct_size;
+    uint32_t image_bytes, n_classes, n_phase_bins, log2_phase_bins, n_depth_bins;
+    uint32_t off_phase;          /* float2 [max(n_classes, 2)][n_phase_bins]: (M[k], (M[k+1] - M[k]) 2^-(32 - log2 K)) */
+    uint32_t off_rows;           /* float4 [n_depth_bins]; the 80 bytes in front of it are the block's round-key slot */
+    uint32_t off_thr, off_thr24; /* uint32 [PDV_MAX_CLASSES] each */
+    uint32_t off_albedo;         /* float [>= max(n_classes, 2)] */
+    uint32_t off_guide, n_guide, guide_base, guide_shift, depth_bisect;   /* uint16 [n_guide] */
+    uint32_t off_cguide, cguide_cells, cguide_shift, cguide_flagged;      /* uint8 [cguide_cells] */
+    uint32_t frac_mask;
+    float tau_ext_ln2, half_v_fs, surface_reflectivity;
+} pdv_image_layout;
+pdv_status pdv_cloud_get_image(const pdv_cloud *cloud, pdv_image_layout *layout, unsigned char *image, size_t capacity);
+
 /* Host (double) depth tables of the (cloud, snapshot time t) unit of a cloud in a gas environment (gas_density > 0), as
  * pdv_mc_run builds them (R36, R37): n = n_depth_bins bins uniform in the height zeta above the free surface.
  *   zeta_edge [n+1]  heights of the bin edges, from the cloud top zeta_top(t) = max_c L_c ln(1 + u_max t / L_c) down to 0

@@ -18,7 +18,7 @@ PDV_MAX_CLASSES = 32
 PDV_MAX_BINS = 8192
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
-           "pdv_cloud_get_tables", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
+           "pdv_cloud_get_tables", "pdv_cloud_get_image", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
            "pdv_last_launch_info", "pdv_last_error", "pdv_version")
 
 
@@ -63,6 +63,13 @@ TRACE_DTYPE = np.dtype([("vt", "f4"), ("weight", "f4"), ("mu_exit", "f4"), ("fat
                         ("n_reflect", "i4")])
 PEAK_DTYPE = np.dtype([("x_peak", "f8"), ("i_peak", "f8"), ("curvature", "f8"), ("k_peak", "i4"), ("status", "i4"),
                        ("beta_eq35", "f8"), ("tau0_eq35", "f8")])
+
+
+class ImageLayout(C.Structure):
+    _fields_ = [("struct_size", C.c_size_t)] + [(n, C.c_uint32) for n in (
+        "image_bytes", "n_classes", "n_phase_bins", "log2_phase_bins", "n_depth_bins", "off_phase", "off_rows", "off_thr", "off_thr24",
+        "off_albedo", "off_guide", "n_guide", "guide_base", "guide_shift", "depth_bisect", "off_cguide", "cguide_cells", "cguide_shift",
+        "cguide_flagged", "frac_mask")] + [(n, C.c_float) for n in ("tau_ext_ln2", "half_v_fs", "surface_reflectivity")]
 
 
 class PhaseCheck(C.Structure):
@@ -170,6 +177,23 @@ class Cloud:
         _check(lib().pdv_cloud_get_tables(self.handle, *[out[k].ctypes.data for k in
                                                          ("k_ext", "k_sca", "g", "p_class", "phase", "T_edge")]))
         return out
+
+    def image(self) -> dict:
+        """The device image of the cloud with its layout (pdv_cloud_get_image): `layout` dict + the sections as numpy views."""
+        lay = ImageLayout()
+        lay.struct_size = C.sizeof(ImageLayout)
+        _check(lib().pdv_cloud_get_image(self.handle, C.byref(lay), None, 0))
+        buf = np.zeros(lay.image_bytes, dtype=np.uint8)
+        _check(lib().pdv_cloud_get_image(self.handle, C.byref(lay), buf.ctypes.data, buf.size))
+        L = {k: getattr(lay, k) for k, _ in ImageLayout._fields_ if k != "struct_size"}
+        nct = max(L["n_classes"], 2)
+        sec = lambda off, dt, n: np.frombuffer(buf, dtype=dt, count=n, offset=off)
+        return dict(layout=L, bytes=buf,
+                    phase=sec(L["off_phase"], np.float32, 2 * nct * L["n_phase_bins"]).reshape(nct, L["n_phase_bins"], 2),
+                    rows=sec(L["off_rows"], np.float32, 4 * L["n_depth_bins"]).reshape(L["n_depth_bins"], 4),
+                    thr=sec(L["off_thr"], np.uint32, PDV_MAX_CLASSES), thr24=sec(L["off_thr24"], np.uint32, PDV_MAX_CLASSES),
+                    albedo=sec(L["off_albedo"], np.float32, nct), guide=sec(L["off_guide"], np.uint16, L["n_guide"]),
+                    cguide=sec(L["off_cguide"], np.uint8, L["cguide_cells"]))
 
     def gas_tables(self, t: float) -> dict:
         """Host depth tables of the (cloud, snapshot time t) unit of a cloud in a gas environment (pdv_cloud_gas_tables)."""

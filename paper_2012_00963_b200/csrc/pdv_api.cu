@@ -798,6 +798,24 @@ pdv_status pdv_cloud_get_tables(const pdv_cloud *c, double *k_ext, double *k_sca
     return PDV_OK;
 }
 
+pdv_status pdv_cloud_get_image(const pdv_cloud *c, pdv_image_layout *lay, unsigned char *image, size_t capacity) {
+    g_err.clear();
+    if (!c || !lay) return fail(PDV_E_INVALID, "cloud / layout is NULL");
+    if (lay->struct_size != sizeof(pdv_image_layout)) return fail(PDV_E_INVALID, "layout->struct_size mismatch");
+    if (c->host.gas()) return fail(PDV_E_INVALID, "a cloud in a gas environment has one image per snapshot, built by pdv_mc_run");
+    DevCloudHeader hd;
+    std::memcpy(&hd, c->blob.data(), sizeof(hd));
+    lay->image_bytes = hd.blob_bytes; lay->n_classes = hd.n_classes; lay->n_phase_bins = hd.K; lay->log2_phase_bins = hd.log2K;
+    lay->n_depth_bins = hd.n_depth; lay->off_phase = hd.off_phase; lay->off_rows = hd.off_rows; lay->off_thr = hd.off_thr;
+    lay->off_thr24 = hd.off_thr + 4u * PDV_MAX_CLASSES; lay->off_albedo = hd.off_albedo; lay->off_guide = hd.off_guide;
+    lay->n_guide = hd.n_guide; lay->guide_base = hd.guide_base; lay->guide_shift = hd.guide_shift; lay->depth_bisect = hd.depth_bisect;
+    lay->off_cguide = hd.off_cguide; lay->cguide_cells = 1u << (32u - hd.cguide_shift); lay->cguide_shift = hd.cguide_shift;
+    lay->cguide_flagged = hd.cguide_flagged; lay->frac_mask = hd.frac_mask;
+    lay->tau_ext_ln2 = hd.tau_ext; lay->half_v_fs = hd.vh_fs; lay->surface_reflectivity = hd.R_f;
+    if (image) std::memcpy(image, c->blob.data(), std::min(capacity, c->blob.size()));
+    return PDV_OK;
+}
+
 pdv_status pdv_cloud_gas_tables(const pdv_cloud *c, double t, double *zeta_edge, double *T_edge, double *class_cum, double *drag_length) {
     g_err.clear();
     if (!c) return fail(PDV_E_INVALID, "cloud is NULL");
