@@ -34,9 +34,10 @@
  * reflections, over many events) by the mean-path invariance of a non-absorbing medium under diffuse
  * illumination (P16: <events> = 4 tau_ext, <reflections> = 1, Lambertian exit; launch_model 1).  The
  * Doppler bookkeeping is pinned per event (P2, P3) and over whole multiple-scattering histories in
- * a rigid cloud, where it telescopes to the exit angle (P17).  The SHAPE of the multiple-scattering
- * spectrum of a cloud with a velocity profile has no closed form and no figure data is available:
- * "parity unpinned" for that output beyond those pins.
+ * a rigid cloud, where it telescopes to the exit angle (P17); with a velocity PROFILE the spectrum of
+ * the histories of exactly two particle events is pinned to a 4-D quadrature (P20).  The SHAPE of the
+ * multiple-scattering spectrum of a cloud with a velocity profile at orders >= 3 has no closed form and
+ * no figure data is available: "parity unpinned" for that output beyond those pins.
  */
 #include <math.h>
 #include <pthread.h>

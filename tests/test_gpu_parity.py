@@ -613,6 +613,37 @@ def test_rigid_cloud_doppler_telescopes_on_the_device(P, poly):
     assert np.max(np.abs(resid)) < 0.05
 
 
+def test_double_scattering_closed_form_on_the_device(P):
+    """Pin P20 on the device, no reference run in the loop: the histories of exactly two particle events of an isotropic cloud
+    with a velocity profile over an absorbing surface, traced on the GPU, against the 4-D Gauss-Legendre quadrature of
+    tests/test_oracle_mc.py (count, first three moments of v~, coarse histogram)."""
+    from test_oracle_mc import _double_scatter_quadrature
+    params = dict(W.config(1)["clouds"][0], phase_model=1, surface_reflectivity=0.0)
+    oc = ocloud.build_cloud(params, phase_override=ocloud.isotropic_quantile_table(1024)[None, :])       # tables of the closed form
+    om, omega_sr, n = float(oc.omega0[0]), 2.0, 4_000_000
+    mu_a = 1.0 - omega_sr / (2.0 * math.pi)
+    run = dict(W.config(1)["run"], aperture_sr=omega_sr)
+    _, rec = P.pdv_mc_trace(P.pdv_cloud_create(params), 0, n, 2012, run)
+    sel = (rec["fate"] == 0) & (rec["n_scatter"] == 2) & (rec["n_reflect"] == 0)
+    assert np.allclose(rec["weight"][sel], om ** 2, rtol=1e-6)
+    vt, wt = _double_scatter_quadrature(oc, om, mu_a)
+    W0 = float(wt.sum())
+    p_sel = W0 / om ** 2
+    assert sel.sum() == pytest.approx(n * p_sel, abs=5 * math.sqrt(n * p_sel))
+    v_g = rec["vt"][sel].astype(np.float64)
+    for k in (1, 2, 3):
+        m_q = float(np.sum(wt * vt ** k)) / W0
+        sig = float(np.std(v_g ** k)) / math.sqrt(sel.sum())
+        assert float(np.mean(v_g ** k)) == pytest.approx(m_q, abs=5 * sig + 2e-4 * m_q), k
+    edges = np.linspace(0.0, 6000.0, 25)
+    h_q, _ = np.histogram(vt, bins=edges, weights=wt)
+    h_g, _ = np.histogram(v_g, bins=edges)
+    big = h_q * n > 2000 * om ** 2
+    assert big.sum() >= 8
+    expect = n * h_q[big] / om ** 2
+    assert np.all(np.abs(h_g[big] - expect) <= 5 * np.sqrt(expect) + 0.01 * expect)
+
+
 def test_rare_paths_stress_many_short_runs(P):
     """Short runs that spend most of their time in the rare paths (roulette kill / survive, analog absorption,
     single-scatter truncation, drained-queue lanes) in varying order: every run must complete, conserve weight

@@ -326,3 +326,82 @@ def test_rigid_cloud_doppler_telescopes_to_the_exit_angle_P17(kw):
     # history by history: v~ = (1 + mu_exit) v / 2 for every photon that left through the top, detected or not
     out = r.trace["fate"] <= 1
     assert np.max(np.abs(r.trace["vt"][out] - 0.5 * (1.0 + r.trace["mu_exit"][out]) * 2000.0)) < 0.002 * 40
+
+
+# ------------------------------------------------------------------------------------------ P20
+def _double_scatter_quadrature(c, omega0, mu_a, n1=240, nm=120, ns=96, n2=12):
+    """Detected weight per launched photon of the histories that scatter EXACTLY twice (no reflection) in a cloud with an
+    isotropic phase function, as nodes (v~, weight) of a Gauss-Legendre rule over (T1, mu1, s, mu2):
+       e^{-T1} dT1 . dmu1/2 . e^{-s} ds . dmu2/2 1[mu2 >= mu_a] e^{-T2/mu2} . omega0^2,   T2 = T1 - mu1 s inside (0, tau),
+       v~ = [(mu1 + 1) v(T1) + (mu2 - mu1) v(T2)] / 2        (Eq. 4 per event, launch direction mu0 = -1),
+    v(T) the canonical depth table (T linear in v inside a bin, R24)."""
+    tau = c.tau_ext
+    nd = c.T_edge.size - 1
+    v_edge = c.v_max - np.arange(nd + 1) * (c.v_max - c.v_fs) / nd
+    v_of = lambda T: np.interp(T, c.T_edge, v_edge)
+    x1, w1 = np.polynomial.legendre.leggauss(n1)
+    T1 = 0.5 * tau * (x1 + 1.0); wT1 = 0.5 * tau * w1 * np.exp(-T1)
+    xm, wm = np.polynomial.legendre.leggauss(nm)
+    xs, ws = np.polynomial.legendre.leggauss(ns)
+    xs, ws = 0.5 * (xs + 1.0), 0.5 * ws                                   # on [0, 1]
+    x2, w2 = np.polynomial.legendre.leggauss(n2)
+    mu2 = mu_a + 0.5 * (1.0 - mu_a) * (x2 + 1.0); wmu2 = 0.5 * (1.0 - mu_a) * w2 * 0.5
+    vt_all, wt_all = [], []
+    for sign in (+1.0, -1.0):                                            # second flight up (T2 < T1) / down (T2 > T1)
+        mu1 = sign * 0.5 * (xm + 1.0); wmu1 = 0.5 * wm * 0.5             # |mu1| on (0, 1), density 1/2
+        room = (T1 if sign > 0 else tau - T1)[:, None] / np.abs(mu1)[None, :]       # optical path to the boundary
+        smax = np.minimum(room, 60.0)
+        s = smax[:, :, None] * xs[None, None, :]
+        wseg = smax[:, :, None] * ws[None, None, :] * np.exp(-s)
+        T2 = T1[:, None, None] - mu1[None, :, None] * s
+        base = wT1[:, None, None] * wmu1[None, :, None] * wseg * omega0 ** 2
+        va = 0.5 * (mu1 + 1.0)[None, :, None] * v_of(T1)[:, None, None]
+        v2 = v_of(T2)
+        for m2, wq in zip(mu2, wmu2):
+            vt_all.append((va + 0.5 * (m2 - mu1)[None, :, None] * v2).ravel())
+            wt_all.append((base * wq * np.exp(-T2 / m2)).ravel())
+    return np.concatenate(vt_all), np.concatenate(wt_all)
+
+
+def test_double_scattering_spectrum_with_a_velocity_profile_P20(cfg2_oracle_cloud):
+    """The part of the multiple-scattering spectrum that has a closed form although the particles move with a velocity
+    PROFILE: histories of exactly two particle events (isotropic phase function, absorbing surface).  Transport (two free
+    flights and the exit flight in a depth-dependent extinction), the per-event Doppler sum (Eq. 4) with the
+    velocity taken at each event's own depth, implicit capture and the aperture all enter; the expectation is a 4-D
+    Gauss-Legendre quadrature with no random number in it.  Compared: total weight, first three moments of v~, and a coarse
+    histogram."""
+    K = cfg2_oracle_cloud.phase.shape[1] - 1
+    c = dataclasses.replace(cfg2_oracle_cloud, surface_reflectivity=0.0, phase=cloud.isotropic_quantile_table(K)[None, :])
+    om = float(c.omega0[0])
+    n = 4_000_000
+    omega_sr = 2.0                                                        # a wide aperture: 4 % of the histories qualify
+    mu_a = 1.0 - omega_sr / (2.0 * math.pi)
+    r = mc.run(c, _run_opts(n, aperture_sr=omega_sr), trace=True)
+    t = r.trace
+    sel = (t["fate"] == 0) & (t["n_scatter"] == 2) & (t["n_reflect"] == 0)
+    assert sel.sum() > 100_000
+    assert np.allclose(t["w"][sel], om ** 2, rtol=1e-12)                  # implicit capture: two albedos
+    vt, wt = _double_scatter_quadrature(c, om, mu_a)
+    vt_b, wt_b = _double_scatter_quadrature(c, om, mu_a, n1=160, nm=80, ns=64, n2=8)    # the rule has converged
+    for k in range(4):
+        assert float(np.sum(wt_b * vt_b ** k)) == pytest.approx(float(np.sum(wt * vt ** k)), rel=2e-4)
+    w_mc, v_mc = t["w"][sel], t["vt"][sel]
+    W0 = float(wt.sum())
+    # number of selected histories ~ Binomial(n, W0 / om^2)
+    p_sel = W0 / om ** 2
+    assert sel.sum() == pytest.approx(n * p_sel, abs=5 * math.sqrt(n * p_sel))
+    for k in (1, 2, 3):                                                   # moments of v~ over the selected histories
+        m_q = float(np.sum(wt * vt ** k)) / W0
+        m_mc = float(np.mean(v_mc ** k))
+        sig = float(np.std(v_mc ** k)) / math.sqrt(sel.sum())
+        assert m_mc == pytest.approx(m_q, abs=5 * sig + 2e-4 * m_q), k
+    edges = np.linspace(0.0, 6000.0, 25)                                  # 250 m/s bins: the rule's nodes are dense inside each
+    h_q, _ = np.histogram(vt, bins=edges, weights=wt)
+    h_mc, _ = np.histogram(v_mc, bins=edges, weights=w_mc)
+    sig = np.sqrt(np.histogram(v_mc, bins=edges, weights=w_mc ** 2)[0])
+    big = h_q * n > 2000 * om ** 2
+    assert big.sum() >= 8
+    assert np.all(np.abs(h_mc[big] - n * h_q[big]) <= 5 * sig[big] + 0.01 * n * h_q[big])
+    # a Doppler sum that took both velocities at one depth, or dropped the second event, is far outside the band
+    bad = float(np.sum(wt * 0.5 * (1.0 + np.full_like(vt, mu_a)) * 2000.0)) / W0
+    assert abs(bad - float(np.mean(v_mc))) > 50 * float(np.std(v_mc)) / math.sqrt(sel.sum())
