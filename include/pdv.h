@@ -165,7 +165,8 @@ typedef struct {
     int32_t output_on_device;    /* 0: hist/hist2/stats are host pointers, the call returns when they are filled;
                                     1: they are DEVICE pointers, the call only enqueues work on cuda_stream */
     int32_t blocks_per_sm;       /* launch shape override for tests; 0: library default */
-    int32_t threads_per_block;   /* 0: library default; multiple of 32, <= 1024 */
+    int32_t threads_per_block;   /* 0: library default; multiple of 32, <= 1024; lowered to what the kernel instantiation of the
+                                    launch was compiled for (768 for long one-class histories).  Never changes a result */
     int32_t launch_model;        /* 0: the paper's collimated probe beam, u = (0,0,-1) at the cloud top (R1);
                                     1: diffuse (Lambertian) illumination of the cloud top, mu = -sqrt(xi) with xi from word 0 of
                                        the history's Philox block with counter word 3 = 0xffffffff.  Not in the paper: it makes
