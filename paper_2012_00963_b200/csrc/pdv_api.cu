@@ -470,7 +470,9 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
             sum += f; sum2 += f * f;
         }
 #ifndef PDV_ALT_MIN_FLIGHTS
-#define PDV_ALT_MIN_FLIGHTS 45.0          /* experiment builds may override */
+#define PDV_ALT_MIN_FLIGHTS 22.0          /* experiment builds may override.  One 5 um cloud, 2e7 histories, plain / long-history kernel,
+                                             ns per 1e3 flights at 9.8 / 14 / 18.5 / 23 / 32 / 46 / 93 flights per history:
+                                             3.71 / 3.49 / 3.40 / 3.35 / 3.31 / 3.24 / 3.24  against  4.06 / 3.63 / 3.42 / 3.30 / 3.17 / 3.06 / 3.03 */
 #endif
         kv.alt = sum > 0.0 && sum2 / sum >= PDV_ALT_MIN_FLIGHTS;
     }

@@ -138,7 +138,7 @@ struct LaunchShape { int grid, block, smem; };
 
 // Host wrappers implemented in pdv_kernels.cu.
 // alt: run the second production instantiation (transport_kernel's ALT).  One-class launches: the histories are long
-// (cost-weighted mean of the estimated flights per history >= 45), a lane then flies several random draws between two
+// (cost-weighted mean of the estimated flights per history >= 22), a lane then flies several random draws between two
 // end-of-history passes -- that pass runs at one or two lanes when histories are long, and running it less often costs fewer
 // issue slots than the lanes that wait for it (measured: profiles/README.md).  Polydisperse launches: no class-guide cell of
 // any cloud holds two thresholds (DevCloudHeader::cguide_flagged == 0 everywhere).
