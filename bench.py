@@ -118,11 +118,22 @@ class ClockSampler:
 
 
 def _workload(index: int) -> dict:
-    """BASELINE.json configs 0..4, or 5: the paper's Figs. 13-15 parameter sweep (row f1)."""
+    """BASELINE.json configs 0..4, 5: the paper's Figs. 13-15 parameter sweep (row f1), 6: ejecta in a gas environment (row f4)."""
+    if index == 6:
+        return W.gas_spectrogram()
     return W.paper_sweep("fig13_15", n_photons=10 ** 7) if index == 5 else W.config(index)
 
 
 # ------------------------------------------------------------------------------------------------------ CPU oracle
+def _oracle_gas(cfg: dict, oc):
+    """Tables of unit 0 of a gas workload (row f4) for the oracle, or None in vacuum."""
+    par = cfg["clouds"][0]
+    if not par.get("gas_density", 0.0) > 0.0:
+        return None
+    from oracle import gas as ogas
+    return ogas.build_tables(oc, par, cfg["t_snap"][0], par.get("n_depth_bins", 1024))
+
+
 def oracle_timed(cfg: dict, seconds: float, seed: int):
     """Times the oracle, as it stands, on all host cores for about `seconds` of work on unit 0 of `cfg`."""
     from oracle import cloud as ocloud
@@ -132,12 +143,13 @@ def oracle_timed(cfg: dict, seconds: float, seed: int):
     cores = os.cpu_count() or 1
     run = dict(cfg["run"], seed=seed)
     n0 = 200_000
+    gas = _oracle_gas(cfg, oc)
     t = time.perf_counter()
-    omc.run(oc, run, n_photons=n0, n_threads=cores)
+    omc.run(oc, run, n_photons=n0, n_threads=cores, gas=gas)
     dt = max(time.perf_counter() - t, 1e-3)
     n = int(min(max(n0, seconds * n0 / dt), cfg["run"]["n_photons"]))
     t = time.perf_counter()
-    r = omc.run(oc, run, n_photons=n, n_threads=cores, first_id=n0)
+    r = omc.run(oc, run, n_photons=n, n_threads=cores, first_id=n0, gas=gas)
     dt = time.perf_counter() - t
     return dict(n=n, seconds=dt, events=int(r.stats["particle_events"]), cores=cores)
 
@@ -155,11 +167,12 @@ def run_reference(args):
     cores = os.cpu_count() or 1
     n = int(min(args.ref_photons, cfg["run"]["n_photons"]))
     ev = 0
+    gas = _oracle_gas(cfg, oc)
     for i in range(args.warmup):
-        omc.run(oc, dict(cfg["run"], seed=1000 + i), n_photons=n, n_threads=cores)
+        omc.run(oc, dict(cfg["run"], seed=1000 + i), n_photons=n, n_threads=cores, gas=gas)
     t = time.perf_counter()
     for i in range(args.steps):
-        ev += int(omc.run(oc, dict(cfg["run"], seed=2000 + i), n_photons=n, n_threads=cores).stats["particle_events"])
+        ev += int(omc.run(oc, dict(cfg["run"], seed=2000 + i), n_photons=n, n_threads=cores, gas=gas).stats["particle_events"])
     dt = time.perf_counter() - t
     val = ev / dt
     sample = f"unit 0 of {cfg['name']}: {n} histories per step (of {cfg['run']['n_photons']}), {args.steps} steps"
@@ -332,7 +345,11 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
         a = dict(ALG_INST_PER_FLIGHT)
         if args.depth_model == 1:                      # closed-form v(T): log + 2 FMA (4 with the clamp) instead of the 8 of the table probe
             a["scatter"] -= 4
-        if any(len(c.get("diameters", [])) > 1 or "lognormal" in c for c in cfg["clouds"]):
+        if any(c.get("gas_density", 0.0) > 0.0 for c in cfg["clouds"]):
+            # gas unit (row f4): class by bisection of the depth bin's 16 thresholds (4 steps x load, compare, add) + per-class albedo
+            # and table base (2) + velocity from the closed form of the drag law (multiply, ex2, subtract, multiply, add, select: 6)
+            a["scatter"] += 20
+        elif any(len(c.get("diameters", [])) > 1 or "lognormal" in c for c in cfg["clouds"]):
             a["scatter"] += 6                        # polydisperse: class pick (guide byte, threshold, compare, clamp) + per-class albedo and table base
         alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
         tr_s = max(tr_ms, 1e-9) * 1e-3
@@ -378,7 +395,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1,
                     help="BASELINE.json configs index (default 1 = headline); 5 = the paper's Figs. 13-15 sweep (SURVEY.md 8(f) row "
-                         "f1: 14 clouds x 1e7 photons in one launch, then pdv_spectrum_peaks on the device)")
+                         "f1: 14 clouds x 1e7 photons in one launch, then pdv_spectrum_peaks on the device); 6 = row f4: a 16-class cloud "
+                         "in a gas environment, 20 snapshots x 1e7 photons")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: how the job is shared (see the module docstring)")
     ap.add_argument("--photons", type=int, default=0, help="override histories per unit (debugging; invalidates the number)")
     ap.add_argument("--depth-model", type=int, default=0, choices=[0, 1],
@@ -417,7 +435,7 @@ def main():
     others = []
     do_others = args.other_configs == 1 or (args.other_configs < 0 and world == 1 and args.config == 1 and not args.depth_model)
     if do_others:
-        for idx in (0, 2, 3, 4, 5):
+        for idx in (0, 2, 3, 4, 5, 6):
             if idx == args.config:
                 continue
             o = time_workload(P, torch, dist, _workload(idx), args, steps=2, warmup=3, e2e_steps=2, rank=rank, world=world, local=local,

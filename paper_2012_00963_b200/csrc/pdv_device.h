@@ -88,15 +88,17 @@ struct DevCloudHeader {
     uint32_t cguide_shift;     // 24 ... 20
     // Gas environment (R35-R37; one image per (cloud, snapshot) unit): the depth rows hold the HEIGHT zeta above the
     // free surface instead of v/2 (y = zeta_{j+1}, z / w = dzeta/dT inside bins j / j+1), bins uniform in zeta;
-    // gas thresholds u32 [n_depth][n_pad]: row j = cumulative class pick probabilities inside bin j as 32-bit thresholds
+    // gas thresholds u32 [n_depth][n_pad + 1] (an ODD row length: the lanes of a warp read the same column of different rows, which
+    // with rows of 2^k words fell on two banks: 13 wavefronts per load): row j = cumulative class pick probabilities inside bin j as 32-bit thresholds
     // (c = #{k : thr[j][k] <= cw}, padded with 0xffffffff to n_pad = 2^gas_steps entries, found by gas_steps bisection steps);
-    // gas class constants float2 [n_pad]: (L_c / (2 t), -1 / L_c), or (1 / (2 t), 0) for a class without drag, so that half the
-    // class-c particle velocity at zeta is  v_fs/2 + x (1 - e^{y zeta})   resp.   v_fs/2 + x zeta.
+    // gas class constants float2 [n_pad]: (L_c / (2 t), -1 / L_c), or (0, 0) for a class without drag, so that half the
+    // class-c particle velocity at zeta is  v_fs/2 + x (1 - e^{y zeta}),  = v_fs/2 + gas_inv_2t zeta (1 + y zeta / 2 + ...) for small y zeta.
     uint32_t gas;              // 1: this image is a gas unit
     uint32_t off_gthr, off_gcls, gas_steps;
     float omr_q31;             // (1 - R_f) 2^31: weight that reached the surface -> Q31 weight left in it
     uint32_t cguide_flagged;   // number of class-guide cells that hold several thresholds (0: an entry is the class count itself)
-    uint32_t pad[3];
+    float gas_inv_2t;          // gas unit: 1 / (2 t) of its snapshot
+    uint32_t pad[2];
 };
 static_assert(sizeof(DevCloudHeader) % 16 == 0, "header must keep 16-byte alignment");
 

@@ -58,6 +58,10 @@ struct SharedKeys {              // the five key vectors at a shared-memory addr
         return k;
     }
 };
+struct ParamKeys {               // the round keys as they sit in the kernel parameters (constant bank): key0[r], key1[r]
+    const uint32_t *k0, *k1;
+    __device__ __forceinline__ uint4 operator[](int i) const { return make_uint4(k0[2 * i], k1[2 * i], k0[2 * i + 1], k1[2 * i + 1]); }
+};
 template <class Keys>
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const Keys keys,
                                               uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3) {
@@ -88,7 +92,17 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 // slower on the polydisperse kernels).
 // cv.rows_s is that address as an integer the compiler cannot see through (else it may move it to a uniform register and pay a
 // move per load: config 4 +2.5 %).
-#define PHILOX_MAIN(c0, c1, c2, c3, o0, o1, o2, o3) philox4x32_10(c0, c1, c2, c3, SharedKeys{cv.rows_s - 80u}, o0, o1, o2, o3)
+// The shared-memory data pipe is the second bottleneck of every instantiation (73 ... 80 % of its wavefront peak: the random
+// 64- and 128-bit table loads take 5.7 and 9.2 wavefronts instead of 2 and 4), and the five broadcast LDS.128 of a block are 10
+// of the 45 (one class) / 79 (several classes) wavefronts of a pass.  KEYS_PARAM instantiations read the keys from the kernel
+// parameters instead (constant bank -> uniform registers, five LDCU.128 per block, no shared-memory wavefront): measured
+// -1.1 % (config 2), -3.7 % (Figs. 13-15 sweep); +1.4 % on the long-history one-class kernel and +1.1 % on the roulette kernel,
+// which keep the shared copy.
+#define PHILOX_MAIN(c0, c1, c2, c3, o0, o1, o2, o3)                                                                              \
+    do {                                                                                                                         \
+        if (KEYS_PARAM) philox4x32_10(c0, c1, c2, c3, ParamKeys{P.key0, P.key1}, o0, o1, o2, o3);                                \
+        else philox4x32_10(c0, c1, c2, c3, SharedKeys{cv.rows_s - 80u}, o0, o1, o2, o3);                                         \
+    } while (0)
 
 // threadIdx.x read where it is used: the address of a warp's shared state is then computed inside the rare path that needs it
 // instead of being hoisted into every pass (or kept in a register the polydisperse kernels do not have)
@@ -138,6 +152,11 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
     asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
     return v;
 }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t saddr) {
+    uint32_t v;
+    asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr));
+    return v;
+}
 __device__ __forceinline__ uint32_t lds_u8(uint32_t saddr) {
     uint32_t v;
     asm("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(saddr));
@@ -150,7 +169,8 @@ __device__ __forceinline__ uint32_t lds_u16(uint32_t saddr) {
 }
 
 struct CloudView {               // per-unit scalars and shared-memory table pointers
-    const uint32_t *gthr;        // gas units: per-bin class thresholds [n_depth][1 << gas_steps]
+    uint32_t gthr_s;             // gas units: shared-memory address of the per-bin class thresholds [n_depth][1 << gas_steps]
+    float gas_inv_2t;            // gas units: 1 / (2 t)
     const float2 *gcls;          // gas units: per-class (L / 2t, -1 / L)
     uint32_t gas_steps;
     float vh_fs;
@@ -203,13 +223,15 @@ __device__ __forceinline__ float gas_height(const CloudView &cv, float Tc, uint3
     return fmaf(Tc - r.x, lower ? r.w : r.z, r.y);
 }
 // half the velocity RELATIVE to the free surface of the class particle found at height zeta:  (L/2t)(1 - e^{-zeta/L}), the closed
-// form of the drag law du/dt = -u^2/L; g = (L/2t, -1/L), or (1/2t, 0) for a class without drag.  1 - e^x by its series for
-// |x| < 1/16 (fp32 cancellation), by ex2 otherwise.
-__device__ __forceinline__ float gas_half_velocity(float2 g, float zeta) {
+// form of the drag law du/dt = -u^2/L; g = (L/2t, -1/L), or (0, 0) for a class without drag.
+// With x = -zeta / L:  (L/2t)(1 - e^x) = (zeta/2t)(1 + x/2 + x^2/6 + x^3/24 + ...): the series for |x| < 1/16 (fp32 cancellation
+// in 1 - e^x, and the only form that survives L -> infinity, where x = 0 and the velocity is zeta / 2t), ex2 otherwise.
+__device__ __forceinline__ float gas_half_velocity(float2 g, float zeta, float inv_2t) {
     const float x = g.y * zeta;
-    const float series = x * fmaf(x, fmaf(x, fmaf(x, 1.f / 24.f, 1.f / 6.f), 0.5f), 1.f);       // e^x - 1
-    const float em1 = fabsf(x) < 0.0625f ? series : exp2f(x * 1.4426950408889634f) - 1.f;
-    return g.y == 0.f ? g.x * zeta : -g.x * em1;
+    const float small = (zeta * inv_2t) * fmaf(x, fmaf(x, fmaf(x, 1.f / 24.f, 1.f / 6.f), 0.5f), 1.f);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 1.4426950408889634f));
+    return fabsf(x) < 0.0625f ? small : g.x * (1.f - e);
 }
 
 // ---- rare paths kept out of line: the flight loop stays small, and the compiler cannot fold their conditions into the
@@ -310,6 +332,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
     // gave config 5 275.9 / 272.4 / 274.0 ms, Figs. 13-15 sweep 74.2 / 78.2 / 77.8 ms.)
     constexpr uint32_t draws = ALT && !POLY ? PDV_DRAWS_LONG_MONO : 1;
     constexpr bool WALK = !(ALT && POLY);                     // class-guide cells may hold several thresholds
+    constexpr bool KEYS_PARAM = !ANALOG && !SSO && !TRACE && !ROUL && DM == 0 && POLY == ALT;      // see PHILOX_MAIN
     constexpr bool NREFL = SSO || ROUL || TRACE;              // variants that read the history's own reflection count
     __shared__ int s_go;
     constexpr bool QUEUE = !TRACE;                            // aperture hits go through the warp's detection queue
@@ -359,7 +382,7 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
             cv.n_classes = h->n_classes; cv.K = h->K; cv.shiftK = 32u - h->log2K; cv.frac_mask = h->frac_mask;
             cv.n_depth = h->n_depth; cv.n_guide = h->n_guide; cv.guide_base = h->guide_base; cv.guide_shift = h->guide_shift;
             cv.depth_bisect = h->depth_bisect; cv.cg_shift = h->cguide_shift;
-            cv.gthr = reinterpret_cast<const uint32_t *>(s_blob + h->off_gthr);
+            cv.gthr_s = (uint32_t)__cvta_generic_to_shared(s_blob + h->off_gthr); cv.gas_inv_2t = h->gas_inv_2t;
             cv.gcls = reinterpret_cast<const float2 *>(s_blob + h->off_gcls);
             cv.gas_steps = h->gas_steps; cv.vh_fs = h->vh_fs;
             cv.tau_ext = h->tau_ext; cv.R_f = h->R_f; cv.one_minus_R = 1.f - h->R_f; cv.omr_q31 = h->omr_q31;
@@ -497,13 +520,18 @@ __global__ void __launch_bounds__(POLY ? PDV_LB_THREADS_POLY : ALT ? PDV_LB_THRE
                 uint32_t bin;
                 const float zeta = gas_height(cv, T, bin);
                 if (POLY) {
-                    if (sub != 2u) cw = (cw & 0xFFFFFF00u) | 0x80u;
-                    const uint32_t *t = cv.gthr + (bin << cv.gas_steps);
-                    for (uint32_t st = 1u << cv.gas_steps >> 1; st > 0u; st >>= 1) c += t[c + st - 1u] <= cw ? st : 0u;
-                    c = min(c, cv.n_classes - 1u);
+                    if (sub != 2u) cw = __byte_perm(cw, 0x80u, 0x3214);        // low byte counts as 0x80 (D2)
+                    // c = #{k : thr[bin][k] <= cw}: bisection of the bin's padded row, unrolled, on the byte address (one load with
+                    // an immediate offset, one compare, one predicated add per step)
+                    const uint32_t row = cv.gthr_s + bin * (4u + (4u << cv.gas_steps));       // rows of 2^steps + 1 words (pdv_device.h)
+                    uint32_t a = row;
+#pragma unroll
+                    for (int k = 4; k >= 0; --k)
+                        if ((uint32_t)k < cv.gas_steps && lds_u32(a + 4u * ((1u << k) - 1u)) <= cw) a += 4u << k;
+                    c = min((a - row) >> 2, cv.n_classes - 1u);
                     if (ANALOG) albt = cv.albthr[c]; else alb = cv.albedo[c];
                 }
-                vh = cv.vh_fs + gas_half_velocity(cv.gcls[c], zeta);
+                vh = cv.vh_fs + gas_half_velocity(cv.gcls[c], zeta, cv.gas_inv_2t);
             } else if (DM == 1 || (DM == 2 && closed)) vh = fmaf(an1, fast_lg2(fmaf(an3, T, an2)), an0);
             else vh = depth_half_velocity<DM == 2>(cv, T);
             if (POLY && DM != 3) {

@@ -117,3 +117,14 @@ def paper_sweep(name: str, n_photons=1e7, seed=11, n_bins=1024, v_fs=2000.0) -> 
     return dict(name=f"paper_{name}", points=copy.deepcopy(pts),
                 clouds=[_cloud(p["m0"], p["beta"], v_fs, lognormal=(p["d_m"], p["sigma"], 16)) for p in pts],
                 t_snap=[2.0e-6], run=_run(n_photons, seed, n_bins, 3.0 * v_fs))
+
+
+# SURVEY.md 8(f) row f4 (the paper's stated future work; readings R35-R38 are NOT the paper's): config 3's
+# 16-class cloud in a gas that moves with the free surface.  The depth tables depend on the snapshot time, so every snapshot is
+# a unit with its own device image; 20 snapshots x 1e7 photons.  Gas density 5 kg/m^3, drag coefficient 0.5, 256 depth bins
+# (the values of tests/test_gpu_gas.py).
+def gas_spectrogram(n_photons=1e7, n_snap=20, seed=13) -> dict:
+    ts = [0.5e-6 + i * (10.0e-6 - 0.5e-6) / max(n_snap - 1, 1) for i in range(n_snap)]
+    cl = dict(_cloud(5.0, 4.0, 2000.0, lognormal=(3.0, 0.5, 16)), gas_density=5.0, drag_coefficient=0.5, n_depth_bins=256)
+    return dict(name="f4_gas_spectrogram", clouds=[cl], t_snap=ts, run=_run(n_photons, seed, 512, 6000.0))
+
