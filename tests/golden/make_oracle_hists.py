@@ -39,26 +39,38 @@ JOBS = {
     "cfg4_cloud36": (3, 36, 100_000_000),
     "cfg4_cloud44": (3, 44, 100_000_000),
     "cfg5": (4, 0, 400_000_000),
+    # row f4 (pdv_workloads.gas_spectrogram, bench.py --config 6): with a gas the spectrum depends on the snapshot time (DESIGN.md
+    # R38), so a spectrum is stored per snapshot: the first and the last of the 20.  ("gas", snapshot index, histories)
+    "f4gas_snap00": ("gas", 0, 100_000_000),
+    "f4gas_snap19": ("gas", 19, 100_000_000),
 }
 
 
 def make(name: str) -> str:
     idx, ci, n = JOBS[name]
-    cfg = W.config(idx)
-    oc = ocloud.build_cloud(cfg["clouds"][ci])
+    gas = None
+    if idx == "gas":
+        from oracle import gas as ogas
+        cfg, snap, ci = W.gas_spectrogram(), ci, 0
+        par = cfg["clouds"][0]
+        oc = ocloud.build_cloud(par)
+        gas = ogas.build_tables(oc, par, cfg["t_snap"][snap], par["n_depth_bins"])
+    else:
+        cfg = W.config(idx)
+        oc = ocloud.build_cloud(cfg["clouds"][ci])
     run = dict(cfg["run"], seed=SEED)
     hist = hist2 = None
     stats: dict = {}
     t0 = time.time()
     for first in range(0, n, CHUNK):
-        r = omc.run(oc, run, n_photons=min(CHUNK, n - first), first_id=first)
+        r = omc.run(oc, run, n_photons=min(CHUNK, n - first), first_id=first, gas=gas)
         hist = r.hist if hist is None else hist + r.hist
         hist2 = r.hist2 if hist2 is None else hist2 + r.hist2
         for k, v in r.stats.items():
             stats[k] = max(stats.get(k, 0), v) if k == "max_events_in_history" else stats.get(k, 0) + v
     out = {
         "what": "oracle/ (fp64 CPU Monte-Carlo) tallies; written by tests/golden/make_oracle_hists.py; no value comes from the CUDA path",
-        "workload": cfg["name"], "config_index": idx, "cloud_index": ci, "n_photons": n, "seed": SEED, "rng_mode": 0,
+        "workload": cfg["name"], "config_index": idx, "cloud_index": ci, "t_snap": (gas["t"] if gas else None), "n_photons": n, "seed": SEED, "rng_mode": 0,
         "run": {k: run[k] for k in ("n_bins", "v_lo", "v_hi", "aperture_sr", "mode", "max_events", "roulette_survival")},
         "tau_ext": oc.tau_ext, "seconds": round(time.time() - t0, 1), "threads": os.cpu_count(),
         "stats": {k: (int(v) if isinstance(v, int) else float(v)) for k, v in stats.items()},

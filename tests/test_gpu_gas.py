@@ -119,3 +119,29 @@ def test_gas_requests_the_kernel_does_not_implement_are_refused(P):
         P.pdv_cloud_create(dict(cfg["clouds"][0], gas_density=8.0, drag_coefficient=0.0))
     with pytest.raises(P.PdvError):
         P.pdv_cloud_create(dict(cfg["clouds"][0], gas_density=8.0, drag_coefficient=0.5, depth_model=1))
+
+
+def test_full_size_gas_spectrogram_against_stored_oracle_runs(P):
+    """Row f4 at the size and in the launch bench.py --config 6 times (20 snapshots x 1e7 photons of the 16-class cloud in a gas, one
+    launch, every snapshot a unit with its own image): the first and the last spectrum against the stored 1e8-history oracle runs of
+    those two units (tests/golden/oracle_hist_f4gas_snap*.json, written by make_oracle_hists.py from oracle/ alone)."""
+    from histcmp import load_golden
+    cfg = W.gas_spectrogram()
+    run, n = cfg["run"], cfg["run"]["n_photons"]
+    r = P.pdv_mc_run([P.pdv_cloud_create(cfg["clouds"][0])], cfg["t_snap"], n, run["seed"], run)
+    assert (P.pdv_last_launch_info()["variant"] >> 8) == 3 and P.pdv_last_launch_info()["variant"] & 1
+    assert np.all(r.conservation_residual() == 0.0)
+    for j, name in ((0, "f4gas_snap00"), (len(cfg["t_snap"]) - 1, "f4gas_snap19")):
+        o = load_golden(name)
+        res = _parity(r.hist[0, j], r.hist2[0, j], n, o, min_ndf=100)
+        s = r.stats[0, j]
+        for key in ("detected", "escaped", "absorbed_particles", "absorbed_surface"):
+            a, b = float(s[key]) / n, o.stats[key] / o.n_photons
+            assert abs(a - b) < 5 * math.sqrt(max(a, 1e-12) / n + max(b, 1e-12) / o.n_photons), (key, a, b)
+        assert s["particle_events"] / n == pytest.approx(o.stats["particle_events"] / o.n_photons, rel=2e-3)
+        assert abs((float(s["detected"]) + float(s["underflow"]) + float(s["overflow"]) + float(s["escaped"])) / n
+                   - (o.stats["detected"] + o.stats["underflow"] + o.stats["overflow"] + o.stats["escaped"]) / o.n_photons) \
+            < 1e-3 * (o.stats["detected"] + o.stats["escaped"]) / o.n_photons + 5 * math.sqrt(0.5 / n)
+    # the two spectra are far apart (R38): the stored runs themselves differ by many sigma
+    a, b = load_golden("f4gas_snap00"), load_golden("f4gas_snap19")
+    assert compare(a.hist, a.hist2, a.n_photons, b.hist, b.hist2, b.n_photons)["worst"] > 50
