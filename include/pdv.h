@@ -220,6 +220,45 @@ pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const do
                       uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
                       double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream);
 
+/* pdv_mc_run for callers that must not allocate device memory.
+ *
+ * Who that is: pdv_mc_run takes its workspace from the device's stream-ordered memory pool on every call.  That is the wrong
+ * thing to do inside a host program that has already handed the whole HBM to an arena of its own (a hydrocode that calls this
+ * library as an in-situ PDV diagnostic every few time steps, a framework with a caching allocator that was told to take all
+ * free memory): there the pool has nothing left to give and the call fails with PDV_E_NOMEM at an unpredictable step, or it
+ * succeeds by growing the pool and the host program's next allocation fails instead.  It is also wrong for a caller on a
+ * real-time path (a shot-by-shot analysis loop next to a running experiment) who wants the footprint of the library fixed when
+ * it is loaded, not decided per call by a pool whose first allocation costs milliseconds.
+ *
+ * What this call does instead: its workspace (photon-id cursors, Q31 tallies, per-unit statistics, unit table, block starts)
+ * is a fixed array of PDV_STATIC_SCRATCH_BYTES that is part of the library's device image -- every GPU that loads the
+ * library holds those 2 MiB from load to exit, whether this call is ever used or not.  The call itself runs no cudaMalloc,
+ * cudaMallocAsync, cudaFree, cudaMallocHost or cudaEventCreate and uses no pinned staging buffer; the only memory it takes is a
+ * few KB of host heap for the unit table it uploads.  The transport and finalize kernels are the ones pdv_mc_run launches, so
+ * hist / hist2 / stats are bit-identical to pdv_mc_run's for the same arguments.
+ *
+ * Arguments as pdv_mc_run, except:
+ *   - hist, hist2 (may be NULL), stats (may be NULL) are DEVICE pointers owned by the caller, and opts->output_on_device must
+ *     be 1: the call only enqueues work on cuda_stream and returns;
+ *   - every cloud must already be resident on the current device (pdv_cloud_create with that device current uploads it -- and
+ *     allocates, so create the clouds during set-up); a host-only cloud or one on another device is PDV_E_INVALID;
+ *   - clouds in a gas environment are PDV_E_UNSUPPORTED (their per-snapshot images are built and uploaded per call);
+ *   - the workspace must fit:  n_units (8 + 16 n_bins + 8*16 + 24) + 4 * (blocks of the launch, <= 2 per SM) bytes, each
+ *     section rounded up to 16, must not exceed PDV_STATIC_SCRATCH_BYTES (one unit of 8192 bins, 120 units of 1024 bins, or the
+ *     paper's 200 x 512 spectrogram fit); a larger request is PDV_E_UNSUPPORTED and pdv_last_error() states both sizes.
+ *     Split it over several calls (whole units, or id ranges whose results add) or use pdv_mc_run.
+ * Set-up: the first call on each device looks the array's device address up (cudaGetSymbolAddress, with that device current)
+ * and keeps it; make that first call during set-up, before any stream capture is begun on the thread.
+ * Sharing: there is ONE array per device and every call uses it from offset 0.  It keeps whatever the previous call left; each
+ * call clears the part that must start at zero (cursors and tallies) on cuda_stream before its kernel.  Calls on one stream
+ * run in order and are safe.  Two calls whose work can overlap on the GPU -- different streams, or different host threads
+ * without a common stream -- race on the array and give garbage: serialise them (one stream, or an event between them).
+ * pdv_last_launch_info does not see these calls (it would need timing events). */
+#define PDV_STATIC_SCRATCH_BYTES (2u << 20)
+pdv_status pdv_mc_run_static(const pdv_cloud *const *clouds, int32_t n_clouds, const double *t_snap, int32_t n_snap,
+                             uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
+                             double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream);
+
 /* Per-history record of the diagnostic entry point below. */
 typedef struct {
     float vt;                    /* Doppler velocity v~ at termination, m/s */

@@ -16,9 +16,10 @@ LIB_PATH = os.path.join(_HERE, "libpdv_b200.so")
 PDV_OK, PDV_E_INVALID, PDV_E_NOMEM, PDV_E_CUDA, PDV_E_UNSUPPORTED = range(5)
 PDV_MAX_CLASSES = 32
 PDV_MAX_BINS = 8192
+PDV_STATIC_SCRATCH_BYTES = 2 << 20
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
-           "pdv_cloud_get_tables", "pdv_cloud_get_image", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
+           "pdv_cloud_get_tables", "pdv_cloud_get_image", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_run_static", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
            "pdv_last_launch_info", "pdv_last_error", "pdv_version")
 
 
@@ -103,6 +104,7 @@ def lib() -> C.CDLL:
         L.pdv_cloud_gas_tables.argtypes = [vp, C.c_double, vp, vp, vp, vp]
         L.pdv_mc_run.argtypes = [C.POINTER(vp), C.c_int32, dp, C.c_int32, C.c_uint64, C.c_uint64, C.POINTER(RunOpts),
                                  vp, vp, vp, vp]
+        L.pdv_mc_run_static.argtypes = L.pdv_mc_run.argtypes
         L.pdv_mc_trace.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint64, C.POINTER(RunOpts), vp, vp, vp, vp, vp]
         L.pdv_spectrogram.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_double, C.c_double, C.c_int32,
                                       C.c_float, vp, C.c_int32, vp]
@@ -312,6 +314,34 @@ def pdv_mc_run_device(clouds, t_snap, n_photons: int, seed: int, run: dict, hist
     _check(lib().pdv_mc_run(arr, nc, t.ctypes.data_as(C.POINTER(C.c_double)), ns, int(n_photons), int(seed), C.byref(o),
                             hist.data_ptr(), hist2.data_ptr() if hist2 is not None else None,
                             stats.data_ptr() if stats is not None else None, C.c_void_p(stream)))
+
+
+def pdv_mc_run_static(clouds, t_snap, n_photons: int, seed: int, run: dict, hist, hist2=None, stats=None,
+                      stream: int | None = None):
+    """pdv_mc_run_device through the entry point that allocates no device memory (pdv_mc_run_static in include/pdv.h).
+
+    For a caller whose process cannot spare the library a device allocation per call -- all HBM already sits in the
+    caller's own arena, or the footprint must be fixed when the library is loaded.  The workspace is a fixed 2 MiB array
+    inside the library (PDV_STATIC_SCRATCH_BYTES), shared by every call on the device: calls on one stream are safe, calls
+    that can overlap on the GPU race.  The clouds must have been created (and so uploaded) beforehand; the tensors are the
+    caller's, as for pdv_mc_run_device.  Results are bit-identical to pdv_mc_run_device's.  Raises PdvError
+    (PDV_E_UNSUPPORTED) when n_units x n_bins does not fit the array, or for gas clouds."""
+    import torch
+    clouds = list(clouds)
+    t = np.ascontiguousarray(t_snap, dtype=np.float64)
+    nc, ns, nb = len(clouds), t.size, int(run["n_bins"])
+    for x in (hist, hist2):
+        if x is not None and not (x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and x.numel() == nc * ns * nb):
+            raise ValueError("hist/hist2 must be contiguous CUDA float64 tensors of n_clouds*n_snap*n_bins elements")
+    if stats is not None and not (stats.is_cuda and stats.dtype == torch.uint8 and stats.numel() == nc * ns * STATS_DTYPE.itemsize):
+        raise ValueError("stats must be a CUDA uint8 tensor of n_units*STATS_DTYPE.itemsize bytes")
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    arr = (C.c_void_p * nc)(*[c.handle for c in clouds])
+    o = _opts(run, output_on_device=True)
+    _check(lib().pdv_mc_run_static(arr, nc, t.ctypes.data_as(C.POINTER(C.c_double)), ns, int(n_photons), int(seed), C.byref(o),
+                                   hist.data_ptr(), hist2.data_ptr() if hist2 is not None else None,
+                                   stats.data_ptr() if stats is not None else None, C.c_void_p(stream)))
 
 
 def pdv_mc_trace(cloud: Cloud, unit: int, n_photons: int, seed: int, run: dict, stream: int | None = None):

@@ -727,6 +727,136 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *
     return PDV_OK;
 }
 
+// ---- pdv_mc_run_static: the workspace of a run as a fixed array inside the library (include/pdv.h) -----------------------------
+// For host programs that cannot let this library allocate device memory (all HBM already belongs to their own arena, or their
+// footprint must be fixed at load time).  The array is part of this module's device image: every GPU that loads the library
+// holds PDV_STATIC_SCRATCH_BYTES of it until the process exits.
+//
+// `g_static_scratch` below is, in HOST code, only a handle for the runtime's symbol table -- not a device address.  Handing it
+// to a kernel would make the kernel fault (or, on a system where the GPU can reach host memory, scribble over host data).  The
+// device address is looked up once per device with cudaGetSymbolAddress while that device is current, and that pointer is
+// what the kernels get.
+}  // namespace
+static __device__ __align__(256) unsigned char g_static_scratch[PDV_STATIC_SCRATCH_BYTES];
+namespace {
+
+pdv_status static_scratch_address(int device, unsigned char **out) {
+    static std::mutex mu;
+    static unsigned char *addr[64] = {nullptr};
+    if (device < 0 || device >= 64) return fail(PDV_E_UNSUPPORTED, "pdv_mc_run_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lk(mu);
+    if (!addr[device]) {                                      // set-up, once per device; `device` is the current device here
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_scratch), "cudaGetSymbolAddress(static scratch)");
+        if (!p) return fail(PDV_E_CUDA, "cudaGetSymbolAddress(static scratch) returned a null address");
+        addr[device] = static_cast<unsigned char *>(p);
+    }
+    *out = addr[device];
+    return PDV_OK;
+}
+
+// Same work as run_impl for a vacuum launch with device outputs, with every device allocation taken out: the clouds must be
+// resident already, the workspace is the static array, no timing events, no pinned staging.
+pdv_status run_static_impl(const pdv_cloud *const *clouds, int n_clouds, int n_snap, const uint32_t *unit_streams,
+                           uint64_t n_photons, uint64_t seed, const pdv_run_opts *o, double *hist, double *hist2,
+                           pdv_run_stats *stats, void *cuda_stream) {
+    const int n_units = n_clouds * n_snap;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    int device = 0;
+    CU(cudaGetDevice(&device), "cudaGetDevice");
+    size_t max_blob = 0;
+    for (int i = 0; i < n_clouds; ++i) {
+        if (clouds[i]->host.gas())
+            return fail(PDV_E_UNSUPPORTED, "pdv_mc_run_static: a cloud in a gas environment needs per-snapshot images that are uploaded per call; use pdv_mc_run");
+        std::lock_guard<std::mutex> lk(clouds[i]->mu);
+        if (!clouds[i]->d_blob || clouds[i]->device != device)
+            return fail(PDV_E_INVALID, "pdv_mc_run_static: every cloud must already be resident on the current device "
+                                       "(create it with pdv_cloud_create while this device is current; this call uploads nothing)");
+        max_blob = std::max(max_blob, clouds[i]->blob.size());
+    }
+    RunPlan plan;
+    pdv_status s = make_plan(clouds, n_clouds, n_units, n_photons, seed, o, false, device, plan, max_blob);
+    if (s != PDV_OK) return s;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nb = (size_t)o->n_bins;
+    const int grid = plan.shape.grid;
+    // layout inside the array: [cursors | Q31 hist | Q31 hist2 | stats] (cleared by every call) [unit table | block starts]
+    size_t off = 0;
+    const size_t o_next = off;  off = align16(off + 8 * (size_t)n_units);
+    const size_t o_hist = off;  off = align16(off + 8 * nb * n_units);
+    const size_t o_hist2 = off; off = align16(off + 8 * nb * n_units);
+    const size_t o_stats = off; off = align16(off + 8 * (size_t)ST_COUNT * n_units);
+    const size_t zero_bytes = off;
+    const size_t o_units = off; off = align16(off + sizeof(UnitDesc) * (size_t)n_units);
+    const size_t o_start = off; off = align16(off + sizeof(uint32_t) * (size_t)grid);
+    const size_t table_bytes = off - o_units;
+    if (off > (size_t)PDV_STATIC_SCRATCH_BYTES) {
+        char msg[256];
+        std::snprintf(msg, sizeof(msg), "pdv_mc_run_static: %d units x %d bins need %zu bytes of workspace, the static array holds %u "
+                      "(split the run into fewer units per call, or use pdv_mc_run)", n_units, o->n_bins, off, (unsigned)PDV_STATIC_SCRATCH_BYTES);
+        return fail(PDV_E_UNSUPPORTED, msg);
+    }
+    unsigned char *ws = nullptr;
+    if ((s = static_scratch_address(device, &ws)) != PDV_OK) return s;
+
+    // unit table: visiting order by descending estimated cost, block starts along the cost line, guided chunk sizes -- as
+    // run_impl builds it.  It only schedules: no result depends on it.
+    std::vector<unsigned char> table(table_bytes, 0);
+    UnitDesc *units = reinterpret_cast<UnitDesc *>(table.data());
+    uint32_t *block_start = reinterpret_cast<uint32_t *>(table.data() + (o_start - o_units));
+    {
+        std::vector<double> cost(n_units);
+        for (int i = 0; i < n_clouds; ++i) {
+            const HostCloud &h = clouds[i]->host;
+            double om = 0.0;
+            for (int c = 0; c < h.n_classes; ++c) om += h.p_class[c] * h.k_sca[c] / h.k_ext[c];
+            const double f = estimated_flights(h.tau_ext, om, o);
+            for (int j = 0; j < n_snap; ++j) cost[(size_t)i * n_snap + j] = f;
+        }
+        std::vector<uint32_t> ord(n_units);
+        for (int k = 0; k < n_units; ++k) ord[k] = (uint32_t)k;
+        std::stable_sort(ord.begin(), ord.end(), [&](uint32_t x, uint32_t y) { return cost[x] > cost[y]; });
+        double total = 0.0;
+        for (int k = 0; k < n_units; ++k) total += cost[k];
+        for (int i = 0; i < n_clouds; ++i)
+            for (int j = 0; j < n_snap; ++j) {
+                const size_t k = (size_t)i * n_snap + j;
+                UnitDesc &u = units[k];
+                u.cloud_blob = clouds[i]->d_blob;
+                u.stream = unit_streams ? unit_streams[k] : (uint32_t)k;
+                const double threads = std::max(1.0, cost[k] / total * grid) * plan.shape.block;
+                u.chunk = (uint32_t)std::min(std::max(std::floor((double)n_photons / (threads * 4.0)), 1.0), 128.0);
+                u.chunk_per_remaining = (float)(1.0 / (2.0 * threads));
+            }
+        for (int k = 0; k < n_units; ++k) units[k].visit = ord[k];
+        double cum = 0.0;
+        int k = 0;
+        for (int b = 0; b < grid; ++b) {
+            const double x = (b + 0.5) / grid * total;
+            while (k + 1 < n_units && cum + cost[ord[k]] <= x) { cum += cost[ord[k]]; ++k; }
+            block_start[b] = (uint32_t)k;
+        }
+    }
+    // the array still holds the previous call's cursors and tallies: clear them in stream order, then upload the table
+    CU(cudaMemsetAsync(ws, 0, zero_bytes, st), "cudaMemsetAsync(static workspace)");
+    CU(cudaMemcpyAsync(ws + o_units, table.data(), table_bytes, cudaMemcpyHostToDevice, st), "copy unit table");
+    RunParams &rp = plan.rp;
+    rp.units = reinterpret_cast<const UnitDesc *>(ws + o_units);
+    rp.block_start = reinterpret_cast<const uint32_t *>(ws + o_start);
+    rp.next_id = reinterpret_cast<unsigned long long *>(ws + o_next);
+    rp.hist = reinterpret_cast<unsigned long long *>(ws + o_hist);
+    rp.hist2 = reinterpret_cast<unsigned long long *>(ws + o_hist2);
+    rp.stats = reinterpret_cast<unsigned long long *>(ws + o_stats);
+    rp.trace = nullptr;
+    if (n_photons > 0) CU(launch_transport(rp, plan.variant, plan.shape, st), "transport kernel launch");
+    CU(launch_finalize(rp.hist, rp.hist2, rp.stats, (uint32_t)n_units, (uint32_t)nb, hist, hist2, stats, st), "finalize kernel launch");
+    return PDV_OK;
+}
+
 }  // namespace
 
 // =================================================================================================================
@@ -862,6 +992,24 @@ pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const do
     if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
     if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
     return run_impl(clouds, n_clouds, t_snap, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
+}
+
+pdv_status pdv_mc_run_static(const pdv_cloud *const *clouds, int32_t n_clouds, const double *t_snap, int32_t n_snap,
+                             uint64_t n_photons, uint64_t seed, const pdv_run_opts *opts,
+                             double *hist, double *hist2, pdv_run_stats *stats, void *cuda_stream) {
+    g_err.clear();
+    if (!clouds || n_clouds < 1) return fail(PDV_E_INVALID, "need at least one cloud");
+    if (!t_snap || n_snap < 1) return fail(PDV_E_INVALID, "need at least one snapshot time");
+    if (!hist) return fail(PDV_E_INVALID, "hist is NULL");
+    pdv_status s = check_opts(opts);
+    if (s != PDV_OK) return s;
+    if (!opts->output_on_device) return fail(PDV_E_INVALID, "pdv_mc_run_static writes device buffers only: set output_on_device = 1");
+    for (int i = 0; i < n_clouds; ++i) if (!clouds[i]) return fail(PDV_E_INVALID, "clouds[i] is NULL");
+    for (int j = 0; j < n_snap; ++j) if (!(t_snap[j] > 0.0) || !std::isfinite(t_snap[j])) return fail(PDV_E_INVALID, "snapshot times must be > 0");
+    if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
+    if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
+    if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
+    return run_static_impl(clouds, n_clouds, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, cuda_stream);
 }
 
 pdv_status pdv_mc_trace(const pdv_cloud *cloud, uint32_t unit, uint64_t n_photons, uint64_t seed,

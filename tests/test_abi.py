@@ -137,6 +137,27 @@ def test_run_argument_validation_and_no_cpu_fallback():
     assert len(P.pdv_spectrum_peaks(np.ones((0, 64)), 10, 0.0, 6000.0, 2000.0)) == 0                 # n_units = 0 is valid
 
 
+def test_static_scratch_entry_validates_before_any_cuda_call():
+    """pdv_mc_run_static (the entry point that allocates no device memory): host outputs are refused, and without a device it
+    reports PDV_E_CUDA like pdv_mc_run.  Through raw ctypes: the Python wrapper wants CUDA tensors."""
+    import torch
+    from paper_2012_00963_b200 import _binding as B
+    cfg = W.config(0)
+    c = P.pdv_cloud_create(cfg["clouds"][0])
+    L = P.lib()
+    arr = (C.c_void_p * 1)(c.handle)
+    t = np.asarray(cfg["t_snap"], dtype=np.float64)
+    dummy = np.zeros(cfg["run"]["n_bins"])                      # never written: every call below fails first
+    call = lambda o, n_snap=1: L.pdv_mc_run_static(arr, 1, t.ctypes.data_as(C.POINTER(C.c_double)), n_snap, 100, 1, C.byref(o),
+                                                   dummy.ctypes.data, None, None, None)
+    assert call(B._opts(cfg["run"], output_on_device=False)) == 1 and "output_on_device" in L.pdv_last_error().decode()
+    assert call(B._opts(dict(cfg["run"], n_bins=0), output_on_device=True)) == 1
+    assert call(B._opts(cfg["run"], output_on_device=True), n_snap=0) == 1
+    if not torch.cuda.is_available():
+        assert call(B._opts(cfg["run"], output_on_device=True)) == 3 and "no CPU fallback" in L.pdv_last_error().decode()
+    assert not dummy.any()
+
+
 def test_product_does_not_import_oracle():
     """The product path must not route through the oracle (or any CPU fallback)."""
     pkg = os.path.join(ROOT, "paper_2012_00963_b200")
