@@ -11,12 +11,22 @@ BASELINE.json configs[I] (default I = 1: 2 mg/cm^2 tin cloud, 1e8 photons, 512 b
 
   value      scattering events/s (particle interactions, BASELINE.json "metric"), whole job, cloud tables resident in HBM and
              outputs left in HBM, timed with CUDA events on the launching stream (max over ranks)
-  e2e        the same metric through the host-buffer C-ABI calls a user makes: pdv_cloud_create (host Mie tables + H2D) +
-             pdv_mc_run into host arrays (D2H inside) + pdv_spectrogram on host arrays, wall clock
-  roofline   transport kernel against the instruction-issue peak (bound "alu": no HBM traffic, no contraction)
+  e2e        the same metric through the host-buffer C-ABI calls a user makes: pdv_cloud_create (host tables + H2D; the
+             per-class Mie tables come from the library's process-wide memo, which is WARM after the first step) +
+             pdv_mc_run into host arrays (D2H inside) + pdv_spectrogram on host arrays, wall clock, with the time of each
+             phase (e2e.phases).  e2e.cold is the same with the memo defeated (the wavelength moved by 1e-12 per step, so every
+             Mie table is computed again): what a user pays for a cloud of sizes the process has not seen yet
+  roofline   transport kernel against the instruction-issue peak (bound "alu": no HBM traffic, no contraction).  frac =
+             EXECUTED thread-instructions of one launch (ncu capture under profiles/, keyed by the sha256 of the kernel
+             sources) / the launch duration measured here / the issue peak; null when no capture matches the sources.
+             frac_model is the hand count of algorithmic instructions per flight (it charges a whole Philox block to every
+             flight while the kernel draws one per two or three flights: it exceeds the executed count, context only)
   cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores, bounded sample of the same workload
   configs    (N = 1, default run) the other BASELINE.json configs and the row-f1 sweep at full size, 2 timed steps each, each
-             with ms_per_step, events/s, roofline and clocks -- so that every config is measured by whoever runs this file
+             with ms_per_step, events/s, roofline, cpu_baseline and clocks -- every config is measured by whoever runs this file
+
+    python bench.py --ingest-ncu <csv> --config I [--command "<the ncu command>"] >> profiles/r3_transport_counters.txt
+turns the ncu export of ONE transport-kernel launch into the record `roofline` is computed from (no GPU needed).
 
 --impl reference times the oracle itself (there is no reference code).
 N > 1 (paper_2012_00963_b200/_shard.py::plan): --scaling weak (default): rank r runs the same number of histories per unit on
@@ -40,6 +50,7 @@ import numpy as np  # noqa: E402
 
 import pdv_workloads as W  # noqa: E402
 
+_E2E_COLD_CALLS = [0]            # cold end-to-end legs so far in this process (each uses wavelengths no earlier one used)
 METRIC = "scattering events/s"
 UNIT = "events/s"
 
@@ -48,7 +59,25 @@ UNIT = "events/s"
 # table "algorithmic instructions per flight").  A particle event, a surface reflection and the final exit flight are
 # one flight each.
 ALG_INST_PER_FLIGHT = {"scatter": 96, "reflect": 70, "exit": 64}
-COUNTERS_FILE = os.path.join(ROOT, "profiles", "r2_transport_counters.txt")
+COUNTERS_FILES = [os.path.join(ROOT, "profiles", f) for f in ("r3_transport_counters.txt", "r2_transport_counters.txt")]
+
+# ncu metric -> key of a counters record.  The first five are required; the rest describe where the issue slots go
+# (north_star: pipe utilisation, warp execution efficiency, shared-memory / atomic throughput) and may be absent from old records.
+NCU_METRICS = {
+    "smsp__thread_inst_executed.sum": "thread_inst_executed", "smsp__inst_executed.sum": "inst_executed",
+    "dram__bytes_read.sum": "dram_bytes_read", "dram__bytes_write.sum": "dram_bytes_write", "gpu__time_duration.sum": "gpu_time_ms",
+    "smsp__issue_active.avg.pct_of_peak_sustained_active": "issue_active_pct",
+    "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active": "pipe_alu_pct",
+    "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": "pipe_fmaheavy_pct",
+    "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active": "pipe_xu_pct",
+    "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed": "smem_wavefronts_pct",
+    "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum": "smem_wavefronts",
+    "sm__warps_active.avg.pct_of_peak_sustained_active": "warps_active_pct",
+    "smsp__inst_executed_op_shared_atom.sum": "shared_atom_inst",
+}
+NCU_REQUIRED = ("thread_inst_executed", "inst_executed", "dram_bytes_read", "dram_bytes_write", "gpu_time_ms")
+NCU_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1e-6, "us": 1e-3, "usecond": 1e-3, "ms": 1.0, "msecond": 1.0,
+             "nsecond": 1e-6, "second": 1e3, "s": 1e3}
 
 
 def _env_int(name, default):
@@ -154,6 +183,13 @@ def oracle_timed(cfg: dict, seconds: float, seed: int):
     return dict(n=n, seconds=dt, events=int(r.stats["particle_events"]), cores=cores)
 
 
+def _cpu_baseline(cfg: dict, seconds: float, seed: int) -> dict:
+    o = oracle_timed(cfg, seconds, seed)
+    return {"value": o["events"] / o["seconds"], "unit": UNIT, "cores": o["cores"], "kind": "oracle",
+            "histories_per_s": o["n"] / o["seconds"],
+            "sample": f"unit 0 of {cfg['name']}: {o['n']} histories in {o['seconds']:.1f} s"}
+
+
 def run_reference(args):
     """`--impl reference`: the oracle timed on the host cores, each step a bounded sample of the workload."""
     rank = _env_int("RANK", 0)
@@ -187,24 +223,72 @@ def run_reference(args):
     }))
 
 
+# ------------------------------------------------------------------------------------------- ncu capture -> record
+def parse_ncu_csv(path: str) -> dict:
+    """Metrics of ONE kernel launch from ncu's long csv (`--csv --log-file`: one row per metric) or the wide one
+    (`ncu -i x.ncu-rep --page raw --csv`: header, units row, one row per launch)."""
+    import csv
+    num = lambda text: float(text.replace(",", ""))
+    rows = [r for r in csv.reader(open(path, newline="")) if r]
+    start = next(i for i, r in enumerate(rows) if "Kernel Name" in r or "ID" in r)
+    hdr, rows = rows[start], rows[start + 1:]
+    out: dict = {}
+    if "Metric Name" in hdr:
+        i_n, i_u, i_v, i_k = hdr.index("Metric Name"), hdr.index("Metric Unit"), hdr.index("Metric Value"), hdr.index("Kernel Name")
+        for r in rows:
+            if len(r) > i_v and r[i_n] in NCU_METRICS:
+                out[NCU_METRICS[r[i_n]]] = num(r[i_v]) * NCU_SCALE.get(r[i_u], 1.0)
+                out["kernel"] = r[i_k]
+    else:
+        units, vals = rows[0], rows[1]
+        for name, key in NCU_METRICS.items():
+            if name in hdr:
+                j = hdr.index(name)
+                out[key] = num(vals[j]) * NCU_SCALE.get(units[j], 1.0)
+        out["kernel"] = vals[hdr.index("Kernel Name")]
+        ratio = "smsp__thread_inst_executed_per_inst_executed.ratio"       # what `--set full` holds instead of the sum
+        if "thread_inst_executed" not in out and ratio in hdr and "inst_executed" in out:
+            out["thread_inst_executed"] = out["inst_executed"] * num(vals[hdr.index(ratio)])
+    missing = [k for k in NCU_REQUIRED if k not in out]
+    if missing:
+        raise SystemExit(f"{path}: metrics missing: {missing}")
+    return out
+
+
+def ingest_ncu(args):
+    """`--ingest-ncu csv --config I`: prints the one-line record of that capture, keyed by the sha256 of the kernel sources."""
+    from paper_2012_00963_b200.build import kernel_source_hash
+    cfg = _workload(args.config)
+    n = int(args.photons or cfg["run"]["n_photons"]) * len(cfg["clouds"]) * len(cfg["t_snap"])
+    rec = {"workload": cfg["name"], "histories_per_launch": n, "kernel_source_sha256": kernel_source_hash()}
+    rec.update(parse_ncu_csv(args.ingest_ncu))
+    for k in ("thread_inst_executed", "inst_executed", "dram_bytes_read", "dram_bytes_write", "smem_wavefronts", "shared_atom_inst"):
+        if k in rec:
+            rec[k] = int(round(rec[k]))
+    rec["lanes_per_inst"] = rec["thread_inst_executed"] / max(rec["inst_executed"], 1)
+    rec["command"] = args.command
+    print(json.dumps(rec))
+
+
 # ------------------------------------------------------------------------------------------------------- GPU arm
 def _captured_counters(workload: str, histories_per_launch: int):
-    """Counters of one transport-kernel launch of this workload from the committed ncu capture (written by
-    `python -m paper_2012_00963_b200.ncu_counters`), or None when there is none for the kernel sources as they are now."""
+    """Counters of one transport-kernel launch of this workload from a committed ncu capture (a record written by
+    `bench.py --ingest-ncu`), or None when there is none for the kernel sources as they are now."""
     from paper_2012_00963_b200.build import kernel_source_hash
-    if not os.path.exists(COUNTERS_FILE):
-        return None
     want = kernel_source_hash()
     found = None
-    with open(COUNTERS_FILE) as f:
-        for line in f:
-            line = line.strip()
-            if not line.startswith("{"):
-                continue
-            rec = json.loads(line)
-            if rec.get("workload") == workload and rec.get("histories_per_launch") == histories_per_launch \
-                    and rec.get("kernel_source_sha256") == want:
-                found = rec
+    for path in COUNTERS_FILES:
+        if found is not None or not os.path.exists(path):
+            continue
+        with open(path) as f:
+            for line in f:
+                line = line.strip()
+                if not line.startswith("{"):
+                    continue
+                rec = json.loads(line)
+                if rec.get("workload") == workload and rec.get("histories_per_launch") == histories_per_launch \
+                        and rec.get("kernel_source_sha256") == want:
+                    found = rec
     return found
 
 
@@ -291,44 +375,64 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
     step_ms, tr_ms = (float(x) for x in t_all.cpu())
     events, reflections, histories = (float(x) for x in cnt.cpu())
 
-    # ---- end to end through the host-buffer API (every step: host Mie tables + H2D, run, D2H, spectrogram) -------------
-    e2e_events = 0
+    # ---- end to end through the host-buffer API (every step: host tables + H2D, run, D2H, spectrogram) ----------------
+    # warm: the per-class Mie tables come from the library's memo after the first step; cold: the wavelength moves by
+    # 1e-12 per step, so every size parameter is new and every Mie table is computed again
+    phase_names = ("cloud_create_ms", "run_ms", "spectrogram_ms")
+    v_fs_host = [c["v_fs"] for c in cfg["clouds"] for _ in t_all_snaps]
 
-    def e2e_step(i):
-        cl = [P.pdv_cloud_create(c) for c in params]
-        r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run) if n_units else None
-        ev = int(r.stats["particle_events"].sum()) if r is not None else 0
+    def e2e_step(i, phases, cold=0):
+        t0 = time.perf_counter()
+        pp = [dict(c, wavelength=c["wavelength"] * (1.0 + 1e-12 * cold)) for c in params] if cold else params
+        cl = [P.pdv_cloud_create(c) for c in pp]
+        t1 = time.perf_counter()
+        if n_units:
+            r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run)
+            ev, rh, rh2, rs = int(r.stats["particle_events"].sum()), r.hist.reshape(-1, nb), r.hist2.reshape(-1, nb), r.stats.reshape(-1)
+        else:                                                # strong scaling with fewer units than ranks: this rank only reduces
+            ev, rh, rh2, rs = 0, np.zeros((0, nb)), np.zeros((0, nb)), np.zeros(0, dtype=P.STATS_DTYPE)
+        t2 = time.perf_counter()
         if world > 1:
-            import torch as _t
-            h, _, _ = _shard.reduce_job(_t.from_numpy(r.hist.reshape(-1, nb)).to(dev), _t.from_numpy(r.hist2.reshape(-1, nb)).to(dev),
-                                        r.stats.reshape(-1), plan["unit_ids"], n_units_job)
+            h, _, _ = _shard.reduce_job(torch.from_numpy(rh).to(dev), torch.from_numpy(rh2).to(dev), rs, plan["unit_ids"], n_units_job)
             h = h.cpu().numpy()
         else:
-            h = r.hist.reshape(n_units, nb)
+            h = rh
         sp = P.pdv_spectrogram(h, photons_job, run["v_lo"], run["v_hi"], scale=2)
         if sweep:
-            sp = P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"],
-                                      [c["v_fs"] for c in cfg["clouds"] for _ in t_all_snaps], half=6, n_pass=2, fit_half=16, x_min=1.03)
+            sp = P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"], v_fs_host, half=6, n_pass=2, fit_half=16, x_min=1.03)
         for c in cl:
             c.destroy()
+        t3 = time.perf_counter()
+        for k, dt in zip(phase_names, (t1 - t0, t2 - t1, t3 - t2)):
+            phases[k] = phases.get(k, 0.0) + 1e3 * dt
         return ev, sp
 
-    for i in range(2 if e2e_steps else 0):
-        e2e_step(-1 - i)
-    barrier()
-    e2e_s = 0.0
-    if e2e_steps:
+    def e2e_leg(n_steps, cold):
+        """-> (events, seconds, phases summed over the steps) of n_steps timed end-to-end steps, max / sum over ranks."""
+        phases = {}
+        ev = 0
+        barrier()
         with clk:
             t0 = time.perf_counter()
-            for i in range(e2e_steps):
-                e2e_events += e2e_step(i)[0]
+            for i in range(n_steps):
+                ev += e2e_step(i + (1000 if cold else 0), phases, cold=(1 + i + 7 * _E2E_COLD_CALLS[0]) if cold else 0)[0]
             torch.cuda.synchronize()
-            e2e_s = time.perf_counter() - t0
-    e2e_t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    e2e_c = torch.tensor([float(e2e_events)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(e2e_c, op=dist.ReduceOp.SUM)
+            sec = time.perf_counter() - t0
+        if cold:
+            _E2E_COLD_CALLS[0] += 1
+        tt = torch.tensor([sec] + [phases.get(k, 0.0) for k in phase_names], dtype=torch.float64, device=dev)
+        cc = torch.tensor([float(ev)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dist.all_reduce(cc, op=dist.ReduceOp.SUM)
+        tt = [float(x) for x in tt.cpu()]
+        return float(cc), tt[0], {k: v / max(n_steps, 1) for k, v in zip(phase_names, tt[1:])}
+
+    for i in range(2 if e2e_steps else 0):
+        e2e_step(-1 - i, {})
+    e2e_c, e2e_t, e2e_phases = e2e_leg(e2e_steps, cold=False) if e2e_steps else (0.0, 0.0, {})
+    cold_steps = min(e2e_steps, 3)
+    cold_c, cold_t, cold_phases = e2e_leg(cold_steps, cold=True) if cold_steps else (0.0, 0.0, {})
     blob_bytes = max(info["smem_bytes"] - 16 * nb, 0)                           # largest cloud image staged per block
     h2d = nc * blob_bytes + 24 * n_units + 4 * info["grid"] + 8 * n_units_job * nb   # tables + unit table + block starts + hist (spectrogram)
     d2h = 2 * 8 * n_units * nb + n_units * P.STATS_DTYPE.itemsize + 4 * n_units_job * nb
@@ -355,19 +459,29 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
         tr_s = max(tr_ms, 1e-9) * 1e-3
         achieved = alg / tr_s
         cap = _captured_counters(cfg["name"], n * n_units) if world == 1 else None
-        roof = {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12, "unit": "Tthread-inst/s",
-                "frac": achieved / issue_peak,
+        launch_s = tr_s / steps                                                 # one transport-kernel launch, CUDA events, this run
+        executed = cap["thread_inst_executed"] / launch_s if cap else None      # executed thread-instructions / s
+        roof = {"bound": "alu",
+                "achieved": executed / 1e12 if cap else None, "peak": issue_peak / 1e12, "unit": "Tthread-inst/s",
+                "frac": executed / issue_peak if cap else None,
+                "frac_is": "executed thread-instructions of one launch (ncu capture keyed by the kernel-source sha256, profiles/) / the "
+                           "launch duration measured in this run (CUDA events) / peak" if cap else
+                           "null: no ncu capture under profiles/ matches the kernel sources as they are (bench.py --ingest-ncu writes one)",
                 "traffic": (cap["dram_bytes_read"] + cap["dram_bytes_write"]) if cap else None,
-                "traffic_is": "dram bytes of one launch (ncu capture of the same workload and kernel sources)" if cap else
-                              "no ncu capture of this workload for the kernel sources as they are",
+                "traffic_is": "dram bytes of one launch (same capture)" if cap else "no capture",
                 "executed_thread_inst_per_launch": cap["thread_inst_executed"] if cap else None,
-                "frac_executed": (cap["thread_inst_executed"] / (tr_s / steps) / issue_peak) if cap else None,
+                "frac_of_measured_ffma": executed / peaks["ffma_thread_inst_per_s"] if cap else None,
                 "peak_is": f"{n_sm} SMs x 4 sub-partitions x 32 lanes x {sm_max:.0f} MHz (DESIGN.md), not in MEASURED_PEAKS.json",
-                "kernel": "pdv::transport_kernel", "alg_inst_per_flight": a,
+                "kernel": "pdv::transport_kernel",
                 "measured_ffma_Tinst_s": peaks["ffma_thread_inst_per_s"] / 1e12,
                 "measured_mufu_Tinst_s": peaks["mufu_thread_inst_per_s"] / 1e12,
-                "frac_of_measured_ffma": achieved / peaks["ffma_thread_inst_per_s"],
-                "sm_clock_mhz_in_microbench": peaks["sm_clock_mhz"]}
+                "sm_clock_mhz_in_microbench": peaks["sm_clock_mhz"],
+                "frac_model": achieved / issue_peak, "achieved_model": achieved / 1e12, "alg_inst_per_flight": a,
+                "frac_model_is": "hand count of algorithmic instructions per flight x flights / time / peak: charges every flight a whole "
+                                 "Philox block, so it EXCEEDS the executed count; context only"}
+        for k in ("lanes_per_inst", "issue_active_pct", "pipe_alu_pct", "pipe_fmaheavy_pct", "pipe_xu_pct", "smem_wavefronts_pct",
+                  "warps_active_pct", "shared_atom_inst"):
+            roof[k] = cap.get(k) if cap else None
         out = {
             "value": events / (step_ms * 1e-3), "ms_per_step": step_ms / steps, "steps": steps, "warmup": warmup,
             "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units_job, "depth_model": args.depth_model,
@@ -380,9 +494,15 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
             "launch": {"grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
                        "transport_ms_per_step": tr_ms / steps},
             "clocks": clocks,
-            "e2e": {"value": (float(e2e_c) / float(e2e_t)) if e2e_steps else None, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": (1e3 * float(e2e_t) / e2e_steps) if e2e_steps else None,
-                    "includes": "pdv_cloud_create (host Mie + tables + H2D), pdv_mc_run (host outputs), pdv_spectrogram"},
+            "e2e": {"value": (e2e_c / e2e_t) if e2e_steps else None, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": (1e3 * e2e_t / e2e_steps) if e2e_steps else None,
+                    "includes": "pdv_cloud_create (host tables + H2D; per-class Mie tables from the library's memo: WARM after the "
+                                "first step), pdv_mc_run (host outputs), pdv_spectrogram" + (", pdv_spectrum_peaks" if sweep else ""),
+                    "phases": e2e_phases,
+                    "cold": {"value": (cold_c / cold_t) if cold_steps else None, "ms_per_step": (1e3 * cold_t / cold_steps) if cold_steps else None,
+                             "steps": cold_steps, "phases": cold_phases,
+                             "is": "the same step with the Mie memo defeated (wavelength x (1 + k 1e-12), a new k per step): "
+                                   "every per-class Mie table is computed again on the host"}},
             "roofline": roof,
         }
     return out
@@ -408,7 +528,15 @@ def main():
     ap.add_argument("--other-configs", type=int, default=-1,
                     help="1: append the 'configs' array (the other workloads at full size, 2 timed steps each); 0: skip; "
                          "default: 1 for the plain default run on one GPU (no --config), else 0")
+    ap.add_argument("--other-cpu-seconds", type=float, default=1.5, help="CPU work of the cpu_baseline of each entry of 'configs'")
+    ap.add_argument("--ingest-ncu", default="", metavar="CSV",
+                    help="no GPU work: turn the ncu csv of ONE transport-kernel launch of --config (and --photons) into the record that "
+                         "roofline.frac is computed from; append the printed line to profiles/r3_transport_counters.txt")
+    ap.add_argument("--command", default="", help="--ingest-ncu: the full ncu command that wrote the csv")
     args = ap.parse_args()
+    if args.ingest_ncu:
+        ingest_ncu(args)
+        return
     if args.impl == "reference":
         run_reference(args)
         return
@@ -438,17 +566,22 @@ def main():
         for idx in (0, 2, 3, 4, 5, 6):
             if idx == args.config:
                 continue
-            o = time_workload(P, torch, dist, _workload(idx), args, steps=2, warmup=3, e2e_steps=2, rank=rank, world=world, local=local,
+            wl = _workload(idx)
+            o = time_workload(P, torch, dist, wl, args, steps=2, warmup=3, e2e_steps=2, rank=rank, world=world, local=local,
                               clk=clk, want_peaks=peaks)
             if o is not None:
                 others.append({"workload": o["config"]["workload"], "config_index": idx, "value": o["value"], "unit": UNIT,
                                "ms_per_step": o["ms_per_step"], "steps": o["steps"], "warmup": o["warmup"],
                                "histories_per_s": o["histories_per_s"], "transport_ms_per_step": o["launch"]["transport_ms_per_step"],
                                "launch": o["launch"], "config": o["config"], "gpu_launches": o["gpu_launches"],
-                               "e2e": {"value": o["e2e"]["value"], "ms_per_step": o["e2e"]["ms_per_step"]},
+                               "e2e": {k: o["e2e"][k] for k in ("value", "ms_per_step", "phases", "cold")},
                                "roofline": {k: o["roofline"][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic",
-                                                                          "executed_thread_inst_per_launch", "frac_executed")},
+                                                                          "executed_thread_inst_per_launch", "frac_of_measured_ffma",
+                                                                          "frac_model", "lanes_per_inst", "issue_active_pct", "pipe_alu_pct",
+                                                                          "pipe_fmaheavy_pct", "pipe_xu_pct", "smem_wavefronts_pct")},
                                "clocks": o["clocks"]})
+                if args.other_cpu_seconds > 0:
+                    others[-1]["cpu_baseline"] = _cpu_baseline(wl, args.other_cpu_seconds, seed=97 + idx)
     if rank == 0:
         out = {"metric": METRIC, "value": main_out["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                "ms_per_step": main_out["ms_per_step"], "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
@@ -456,10 +589,7 @@ def main():
         out.update({k: main_out[k] for k in ("config", "histories_per_s", "events_incl_surface_per_s", "gpu_launches", "launch", "clocks",
                                              "e2e", "roofline")})
         if args.cpu_seconds > 0:
-            o = oracle_timed(cfg, args.cpu_seconds, seed=97)
-            out["cpu_baseline"] = {"value": o["events"] / o["seconds"], "unit": UNIT, "cores": o["cores"], "kind": "oracle",
-                                   "histories_per_s": o["n"] / o["seconds"],
-                                   "sample": f"unit 0 of {cfg['name']}: {o['n']} histories in {o['seconds']:.1f} s"}
+            out["cpu_baseline"] = _cpu_baseline(cfg, args.cpu_seconds, seed=97)
         if others:
             out["configs"] = others
     if world > 1:

@@ -208,8 +208,8 @@ typedef struct {                 /* weights in units of photons; identity (exact
  * hist/hist2/stats for any launch shape -- tallies are integer fixed point (Q31) and every history draws
  * from its own Philox4x32-10 counter stream keyed by (seed, photon id, unit).  Runs over id ranges [a,b)
  * and [b,c) sum to the run over [a,c).  n_photons = 0 is valid and yields zeros.
- * Limits: n_photons <= 2^33 per unit (a tally is a Q31 sum in 64 bits: it holds the weight of 2^33 photons; larger runs are
- * split by the caller into id ranges, whose results add), n_clouds * n_snap <= 2^20, photon ids below 2^63; otherwise
+ * Limits: n_photons < 2^33 per unit (a tally is a Q31 sum in 64 bits: the weight of 2^33 photons, 2^33 * 2^31 = 2^64, would wrap
+ * it to 0 -- e.g. "escaped" of an empty cloud; larger runs are split by the caller into id ranges, whose results add), n_clouds * n_snap <= 2^20, photon ids below 2^63; otherwise
  * PDV_E_INVALID.
  * Streams: every call takes its device scratch (id cursors, Q31 tallies, unit table, output staging) from the device's
  * stream-ordered memory pool on cuda_stream and releases it there behind its last kernel, so calls enqueued on DIFFERENT

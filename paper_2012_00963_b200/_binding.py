@@ -101,6 +101,7 @@ def lib() -> C.CDLL:
         L.pdv_cloud_destroy.restype = None
         L.pdv_cloud_get_info.argtypes = [vp, C.POINTER(CloudInfo)]
         L.pdv_cloud_get_tables.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.pdv_cloud_get_image.argtypes = [vp, C.POINTER(ImageLayout), vp, C.c_size_t]
         L.pdv_cloud_gas_tables.argtypes = [vp, C.c_double, vp, vp, vp, vp]
         L.pdv_mc_run.argtypes = [C.POINTER(vp), C.c_int32, dp, C.c_int32, C.c_uint64, C.c_uint64, C.POINTER(RunOpts),
                                  vp, vp, vp, vp]

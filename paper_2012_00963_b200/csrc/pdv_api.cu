@@ -989,7 +989,7 @@ pdv_status pdv_mc_run(const pdv_cloud *const *clouds, int32_t n_clouds, const do
     for (int i = 0; i < n_clouds; ++i) if (!clouds[i]) return fail(PDV_E_INVALID, "clouds[i] is NULL");
     for (int j = 0; j < n_snap; ++j) if (!(t_snap[j] > 0.0) || !std::isfinite(t_snap[j])) return fail(PDV_E_INVALID, "snapshot times must be > 0");
     if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
-    if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
+    if (n_photons >= (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit must be below 2^33: a Q31 tally in 64 bits wraps at the weight of 2^33 photons (split the run into id ranges)");
     if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
     return run_impl(clouds, n_clouds, t_snap, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, nullptr, cuda_stream);
 }
@@ -1007,7 +1007,7 @@ pdv_status pdv_mc_run_static(const pdv_cloud *const *clouds, int32_t n_clouds, c
     for (int i = 0; i < n_clouds; ++i) if (!clouds[i]) return fail(PDV_E_INVALID, "clouds[i] is NULL");
     for (int j = 0; j < n_snap; ++j) if (!(t_snap[j] > 0.0) || !std::isfinite(t_snap[j])) return fail(PDV_E_INVALID, "snapshot times must be > 0");
     if ((long long)n_clouds * n_snap > (1 << 20)) return fail(PDV_E_INVALID, "too many (cloud, snapshot) units");
-    if (n_photons > (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit is limited to 2^33: a Q31 tally in 64 bits holds 2^33 photons (split the run into id ranges)");
+    if (n_photons >= (1ull << 33)) return fail(PDV_E_INVALID, "n_photons per unit must be below 2^33: a Q31 tally in 64 bits wraps at the weight of 2^33 photons (split the run into id ranges)");
     if (opts->first_photon_id > (1ull << 62)) return fail(PDV_E_INVALID, "photon ids must stay below 2^63");
     return run_static_impl(clouds, n_clouds, n_snap, opts->unit_streams, n_photons, seed, opts, hist, hist2, stats, cuda_stream);
 }

@@ -110,6 +110,9 @@ def test_run_argument_validation_and_no_cpu_fallback():
     with pytest.raises(P.PdvError) as e:
         P.pdv_mc_run([c], [0.0], 100, 1, cfg["run"])
     assert e.value.status == 1
+    with pytest.raises(P.PdvError) as e:                       # exactly 2^33 photons would wrap a 64-bit Q31 tally
+        P.pdv_mc_run([c], cfg["t_snap"], 2 ** 33, 1, cfg["run"])
+    assert e.value.status == 1 and "2^33" in str(e.value)
     if not torch.cuda.is_available():
         with pytest.raises(P.PdvError) as e:
             P.pdv_mc_run([c], cfg["t_snap"], 100, 1, cfg["run"])

@@ -27,6 +27,10 @@ def test_bench_prints_one_json_line_with_the_contract_keys(flags):
     assert d["gpu_launches"] == (4 if flags else 3) * 2
     assert set(("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")) <= set(d["e2e"]) and d["e2e"]["value"] > 0
     assert set(("bound", "achieved", "peak", "unit", "frac", "traffic")) <= set(d["roofline"]) and d["roofline"]["bound"] == "alu"
+    assert set(("frac_model", "frac_is", "issue_active_pct", "lanes_per_inst", "smem_wavefronts_pct")) <= set(d["roofline"])
+    assert d["roofline"]["frac"] is None or 0.0 < d["roofline"]["frac"] < 1.0           # measured or null, never the model
+    assert set(("cloud_create_ms", "run_ms", "spectrogram_ms")) <= set(d["e2e"]["phases"]) and d["e2e"]["cold"]["value"] > 0
+    assert d["e2e"]["cold"]["phases"]["cloud_create_ms"] >= d["e2e"]["phases"]["cloud_create_ms"] * 0.5
     assert set(("value", "unit", "cores", "kind", "sample")) <= set(d["cpu_baseline"]) and d["cpu_baseline"]["kind"] == "oracle"
     assert set(("sm_mhz", "sm_max_mhz", "reasons")) <= set(d["clocks"])
 

@@ -476,8 +476,9 @@ def test_detection_queue_under_full_load(P):
 def test_photon_count_limit_of_the_fixed_point_tallies(P):
     cfg = W.config(1)
     c = P.pdv_cloud_create(cfg["clouds"][0])
-    with pytest.raises(P.PdvError):
-        P.pdv_mc_run([c], cfg["t_snap"], 2 ** 33 + 1, 1, cfg["run"])
+    with pytest.raises(P.PdvError) as e:                       # 2^33 photons of weight 1 in one tally = 2^64: wraps
+        P.pdv_mc_run([c], cfg["t_snap"], 2 ** 33, 1, cfg["run"])
+    assert e.value.status == 1 and "2^33" in str(e.value)
 
 
 def test_full_size_config2_in_bench_launch_configuration(P):
