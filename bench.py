@@ -31,7 +31,8 @@ turns the ncu export of ONE transport-kernel launch into the record `roofline` i
 --impl reference times the oracle itself (there is no reference code).
 N > 1 (paper_2012_00963_b200/_shard.py::plan): --scaling weak (default): rank r runs the same number of histories per unit on
 photon ids [r n, (r+1) n); --scaling strong: the job is fixed, one-unit configs split the id range, multi-unit configs give
-whole units to ranks.  Either way the only exchange is one reduction of the tallies per step.
+stretches of equal estimated cost to ranks (_shard.plan_balanced: units that straddle a rank boundary are split by photon id).
+Either way the only exchange is one reduction of the tallies per step, on device tensors.
 """
 from __future__ import annotations
 
@@ -303,20 +304,41 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
     n_job = int(args.photons or run["n_photons"])                      # histories per unit of the job (per rank when weak)
     nb, t_all_snaps = run["n_bins"], cfg["t_snap"]
     nc_job, ns_job = len(cfg["clouds"]), len(t_all_snaps)
-    plan = _shard.plan(nc_job, ns_job, n_job, rank, world, args.scaling)
-    n = plan["n_photons"]
-    run["first_photon_id"] = plan["first_photon_id"]
-    if world > 1 and args.scaling == "strong":
-        run["unit_streams"] = plan["unit_ids"]
-    params = [cfg["clouds"][i] for i in plan["clouds"]]
-    t_snap = [t_all_snaps[j] for j in plan["snaps"]]
-    clouds = [P.pdv_cloud_create(c) for c in params]
-    nc, ns = len(clouds), len(t_snap)
-    n_units, n_units_job = nc * ns, nc_job * ns_job
+    # What this rank runs: a list of SEGMENTS, each one pdv_mc_run call over a clouds x snapshots grid with its own id range.
+    # One GPU, weak scaling and one-unit jobs: one segment (_shard.plan).  Strong scaling of a multi-unit job: a contiguous stretch
+    # of the job's cost line (the library's own flights-per-history estimate), units that straddle a rank boundary split by photon
+    # id (_shard.plan_balanced): at most a partial unit at each end and the whole units in between.
+    n_units_job = nc_job * ns_job
+    if world > 1 and args.scaling == "strong" and n_units_job > 1:
+        probe = [P.pdv_cloud_create(c) for c in cfg["clouds"]]             # host optics only matter here (memoised per class)
+        costs = [c.estimated_flights(run) for c in probe for _ in t_all_snaps]
+        for c in probe:
+            c.destroy()
+        segs = _shard.plan_balanced(costs, nc_job, ns_job, n_job, rank, world)
+        for sg in segs:
+            sg["unit_streams"] = sg["unit_ids"]
+    else:
+        pl = _shard.plan(nc_job, ns_job, n_job, rank, world, args.scaling)
+        if world > 1 and args.scaling == "strong":
+            pl["unit_streams"] = pl["unit_ids"]
+        segs = [pl] if pl["clouds"] and pl["snaps"] else []
+    row = 0
+    for sg in segs:
+        sg["params"] = [cfg["clouds"][i] for i in sg["clouds"]]
+        sg["t"] = [t_all_snaps[j] for j in sg["snaps"]]
+        sg["run"] = dict(run, first_photon_id=sg["first_photon_id"], **({"unit_streams": sg["unit_streams"]} if "unit_streams" in sg else {}))
+        sg["rows"] = (row, row + len(sg["unit_ids"]))
+        row += len(sg["unit_ids"])
+        sg["handles"] = [P.pdv_cloud_create(c) for c in sg["params"]]
+    n_units = row
+    unit_ids = [u for sg in segs for u in sg["unit_ids"]]
+    hist_per_step = sum(sg["n_photons"] * len(sg["unit_ids"]) for sg in segs)      # histories this rank runs per step
+    n = segs[0]["n_photons"] if segs else 0
     photons_job = n_job * (world if args.scaling == "weak" else 1)     # histories per unit of the whole job
-    hist = torch.zeros((max(nc, 1), max(ns, 1), nb), dtype=torch.float64, device=dev)
+    SB = P.STATS_DTYPE.itemsize
+    hist = torch.zeros((max(n_units, 1), nb), dtype=torch.float64, device=dev)
     hist2 = torch.zeros_like(hist)
-    stats = torch.zeros(max(n_units, 1) * P.STATS_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    stats = torch.zeros(max(n_units, 1) * SB, dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
     stream = torch.cuda.current_stream()
     sweep = "points" in cfg                                   # sweep + interpretation workload: one v_fs per spectrum
@@ -331,18 +353,24 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
         return np.frombuffer(stats.cpu().numpy().tobytes(), dtype=P.STATS_DTYPE)[:n_units]
 
     def step(i):
-        if n_units:
-            P.pdv_mc_run_device(clouds, t_snap, n, run["seed"] + 7919 * i, run, hist, hist2, stats, stream=stream.cuda_stream)
-        if world > 1:                                        # the one exchange: tallies of the whole job on every rank
-            h, _, _ = _shard.reduce_job(hist.view(-1, nb)[:n_units], hist2.view(-1, nb)[:n_units], read_stats(), plan["unit_ids"], n_units_job)
+        ms = 0.0
+        for sg in segs:
+            a, b = sg["rows"]
+            P.pdv_mc_run_device(sg["handles"], sg["t"], sg["n_photons"], run["seed"] + 7919 * i, sg["run"], hist[a:b], hist2[a:b],
+                                stats[a * SB:b * SB], stream=stream.cuda_stream)
+            if timing[0]:
+                ms += P.pdv_last_launch_info()["transport_ms"]       # waits for this segment's kernel (one GPU: the only one)
+        if world > 1:                                        # the one exchange: tallies of the whole job on every rank, all on the device
+            h, _, _ = _shard.reduce_job(hist[:n_units], hist2[:n_units], stats[:n_units * SB], unit_ids, n_units_job)
         else:
-            h = hist.view(n_units, nb)
+            h = hist[:n_units]
         sp = P.pdv_spectrogram(h, photons_job, run["v_lo"], run["v_hi"], scale=2, stream=stream.cuda_stream)
         if sweep:                                            # row f1: peak position / value / curvature of every spectrum
-            return P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"], v_fs_job, half=6, n_pass=2, fit_half=16,
-                                        x_min=1.03, stream=stream.cuda_stream)
-        return sp
+            sp = P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"], v_fs_job, half=6, n_pass=2, fit_half=16,
+                                      x_min=1.03, stream=stream.cuda_stream)
+        return sp, ms
 
+    timing = [False]
     for i in range(warmup):
         flush.zero_()
         step(i)
@@ -353,14 +381,15 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
     tot = dict(particle_events=0, surface_reflections=0, histories=0)
     transport_ms = []
     clk.reset()
+    timing[0] = world == 1                                   # per-kernel times (roofline) on one GPU only: reading them waits for the kernel
     with clk:                                                # sampled during the device-timed steps and the end-to-end steps
         barrier()
         for i in range(steps):
             flush.zero_()                                    # L2 flush between timed iterations (outside the events)
             ev0[i].record(stream)
-            step(warmup + i)
+            _, ms = step(warmup + i)
             ev1[i].record(stream)
-            transport_ms.append(P.pdv_last_launch_info()["transport_ms"] if n_units else 0.0)      # waits for this step's kernel
+            transport_ms.append(ms)
             s = read_stats()
             for k in tot:
                 tot[k] += int(s[k].sum())
@@ -383,25 +412,27 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
 
     def e2e_step(i, phases, cold=0):
         t0 = time.perf_counter()
-        pp = [dict(c, wavelength=c["wavelength"] * (1.0 + 1e-12 * cold)) for c in params] if cold else params
-        cl = [P.pdv_cloud_create(c) for c in pp]
+        cl = [[P.pdv_cloud_create(dict(c, wavelength=c["wavelength"] * (1.0 + 1e-12 * cold)) if cold else c) for c in sg["params"]] for sg in segs]
         t1 = time.perf_counter()
-        if n_units:
-            r = P.pdv_mc_run(cl, t_snap, n, run["seed"] + 104729 * (i + 1), run)
-            ev, rh, rh2, rs = int(r.stats["particle_events"].sum()), r.hist.reshape(-1, nb), r.hist2.reshape(-1, nb), r.stats.reshape(-1)
-        else:                                                # strong scaling with fewer units than ranks: this rank only reduces
-            ev, rh, rh2, rs = 0, np.zeros((0, nb)), np.zeros((0, nb)), np.zeros(0, dtype=P.STATS_DTYPE)
+        # a rank without units (strong scaling with fewer units than ranks) only takes part in the reduction
+        ev, rh, rh2, rs = 0, [np.zeros((0, nb))], [np.zeros((0, nb))], [np.zeros(0, dtype=P.STATS_DTYPE)]
+        for sg, handles in zip(segs, cl):
+            r = P.pdv_mc_run(handles, sg["t"], sg["n_photons"], run["seed"] + 104729 * (i + 1), sg["run"])
+            ev += int(r.stats["particle_events"].sum())
+            rh.append(r.hist.reshape(-1, nb)); rh2.append(r.hist2.reshape(-1, nb)); rs.append(r.stats.reshape(-1))
+        rh, rh2, rs = np.concatenate(rh), np.concatenate(rh2), np.concatenate(rs)
         t2 = time.perf_counter()
         if world > 1:
-            h, _, _ = _shard.reduce_job(torch.from_numpy(rh).to(dev), torch.from_numpy(rh2).to(dev), rs, plan["unit_ids"], n_units_job)
+            h, _, _ = _shard.reduce_job(torch.from_numpy(rh).to(dev), torch.from_numpy(rh2).to(dev), rs, unit_ids, n_units_job)
             h = h.cpu().numpy()
         else:
             h = rh
         sp = P.pdv_spectrogram(h, photons_job, run["v_lo"], run["v_hi"], scale=2)
         if sweep:
             sp = P.pdv_spectrum_peaks(h, photons_job, run["v_lo"], run["v_hi"], v_fs_host, half=6, n_pass=2, fit_half=16, x_min=1.03)
-        for c in cl:
-            c.destroy()
+        for handles in cl:
+            for c in handles:
+                c.destroy()
         t3 = time.perf_counter()
         for k, dt in zip(phase_names, (t1 - t0, t2 - t1, t3 - t2)):
             phases[k] = phases.get(k, 0.0) + 1e3 * dt
@@ -434,10 +465,12 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
     cold_steps = min(e2e_steps, 3)
     cold_c, cold_t, cold_phases = e2e_leg(cold_steps, cold=True) if cold_steps else (0.0, 0.0, {})
     blob_bytes = max(info["smem_bytes"] - 16 * nb, 0)                           # largest cloud image staged per block
-    h2d = nc * blob_bytes + 24 * n_units + 4 * info["grid"] + 8 * n_units_job * nb   # tables + unit table + block starts + hist (spectrogram)
+    n_handles = sum(len(sg["handles"]) for sg in segs)
+    h2d = n_handles * blob_bytes + 24 * n_units + 4 * info["grid"] + 8 * n_units_job * nb   # tables + unit table + block starts + hist (spectrogram)
     d2h = 2 * 8 * n_units * nb + n_units * P.STATS_DTYPE.itemsize + 4 * n_units_job * nb
-    for c in clouds:
-        c.destroy()
+    for sg in segs:
+        for c in sg["handles"]:
+            c.destroy()
 
     out = None
     if rank == 0:
@@ -458,7 +491,7 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
         alg = (events * a["scatter"] + reflections * a["reflect"] + histories * a["exit"]) / world
         tr_s = max(tr_ms, 1e-9) * 1e-3
         achieved = alg / tr_s
-        cap = _captured_counters(cfg["name"], n * n_units) if world == 1 else None
+        cap = _captured_counters(cfg["name"], hist_per_step) if world == 1 else None
         launch_s = tr_s / steps                                                 # one transport-kernel launch, CUDA events, this run
         executed = cap["thread_inst_executed"] / launch_s if cap else None      # executed thread-instructions / s
         roof = {"bound": "alu",
@@ -484,13 +517,13 @@ def time_workload(P, torch, dist, cfg, args, *, steps, warmup, e2e_steps, rank, 
             roof[k] = cap.get(k) if cap else None
         out = {
             "value": events / (step_ms * 1e-3), "ms_per_step": step_ms / steps, "steps": steps, "warmup": warmup,
-            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": n * n_units, "units": n_units_job, "depth_model": args.depth_model,
-                       "n_bins": nb, "parallelism": f"{args.scaling}: " + ("photon-id ranges" if args.scaling == "weak" or n_units_job == 1 else "whole units") + f" x{world}",
+            "config": {"workload": cfg["name"], "histories_per_step_per_gpu": hist_per_step, "units": n_units_job, "depth_model": args.depth_model,
+                       "n_bins": nb, "parallelism": f"{args.scaling}: " + ("photon-id ranges" if args.scaling == "weak" or n_units_job == 1 else "equal estimated cost (units split by photon id at rank boundaries)") + f" x{world}",
                        "l2": "flushed between steps (256 MiB write)",
                        "events_per_history": events / max(histories, 1), "reflections_per_history": reflections / max(histories, 1)},
             "histories_per_s": histories / (step_ms * 1e-3),
             "events_incl_surface_per_s": (events + reflections) / (step_ms * 1e-3),
-            "gpu_launches": (4 if sweep else 3) * steps,    # transport + finalize + spectrogram (+ peak) kernels per step
+            "gpu_launches": (2 * max(len(segs), 1) + (2 if sweep else 1)) * steps,    # (transport + finalize) per segment + spectrogram (+ peak) kernels per step
             "launch": {"grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
                        "transport_ms_per_step": tr_ms / steps},
             "clocks": clocks,

@@ -115,6 +115,13 @@ typedef struct {
 
 pdv_status pdv_cloud_get_info(const pdv_cloud *cloud, pdv_cloud_info *out);
 
+/* The library's own estimate of the flights (particle events + surface reflections + the exit flight) of ONE history of this
+ * cloud under the run options `opts` (a pdv_run_opts; only mode, max_events, roulette_survival and single_scatter_only are read;
+ * NULL: defaults) -- the number pdv_mc_run lays its blocks out with (2.3 + 4.8 tau_ext, capped by the roulette, the analog
+ * absorption and the single-scatter cut).  Only ratios matter.  A caller that splits a job over several GPUs cuts it into
+ * stretches of equal estimated cost with it (paper_2012_00963_b200/_shard.py::plan_balanced).  No device needed. */
+pdv_status pdv_estimated_flights(const pdv_cloud *cloud, const void *opts, double *out);
+
 /* Copies the host (double) tables of the cloud into caller buffers; any pointer may be NULL to skip it.
  * k_ext,k_sca,g,p_class: [n_classes].  phase: [n_classes][n_phase_bins+1], M_c[k] = F_c^-1(k/K) in cos(theta).
  * T_edge: [n_depth_bins+1], T at velocity v_max - j (v_max - v_fs)/n_depth_bins. */
@@ -348,6 +355,14 @@ typedef struct {
 pdv_status pdv_phase_sampling_check(const pdv_cloud *cloud, int32_t class_index, uint64_t n_samples, uint64_t seed,
                                     int32_t n_bins, uint64_t *hist_table, uint64_t *hist_exact, pdv_phase_check *info,
                                     void *cuda_stream);
+
+/* Diagnostic (pin P13 of the test suite): raw blocks of the kernels' own Philox4x32-10.  Block i = the generator applied to the
+ * counter counters[4i .. 4i+3] with the key (low word of seed, high word of seed) -- the key pdv_mc_run derives from `seed` --
+ * computed three times, once through each way the transport kernel reads its ten round keys: static shared memory, a shared
+ * address held in a register, and the kernel parameters (constant bank).  All three must equal the published Random123 vectors.
+ * counters: HOST [4 n] words; out_static / out_shared / out_param: HOST [4 n] words each; 0 <= n <= 2^20. */
+pdv_status pdv_philox_blocks(const uint32_t *counters, int32_t n, uint64_t seed, uint32_t *out_static, uint32_t *out_shared,
+                             uint32_t *out_param);
 
 /* Measures the issue-rate denominators on the current device: a dependent-free FFMA stream and a MUFU
  * stream, each run for ~`millis` ms on every SM.  Outputs (any may be NULL): thread-instructions/s of each,

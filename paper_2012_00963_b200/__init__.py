@@ -6,5 +6,5 @@ entry points; all computation happens in hand-written CUDA kernels for sm_100a. 
 from ._binding import (  # noqa: F401
     EXPORTS, LIB_PATH, PDV_MAX_BINS, PDV_MAX_CLASSES, PDV_STATIC_SCRATCH_BYTES, PEAK_DTYPE, STATS_DTYPE, TRACE_DTYPE, Cloud, PdvError, RunResult, lib,
     pdv_cloud_create, pdv_issue_peaks, pdv_last_launch_info, pdv_lognormal_classes, pdv_mc_run, pdv_mc_run_device, pdv_mc_run_static,
-    pdv_mc_trace, pdv_phase_sampling_check, pdv_spectrogram, pdv_spectrum_peaks, pdv_version,
+    pdv_mc_trace, pdv_phase_sampling_check, pdv_philox_blocks, pdv_spectrogram, pdv_spectrum_peaks, pdv_version,
 )

@@ -19,7 +19,7 @@ PDV_MAX_BINS = 8192
 PDV_STATIC_SCRATCH_BYTES = 2 << 20
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
-           "pdv_cloud_get_tables", "pdv_cloud_get_image", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_run_static", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_issue_peaks",
+           "pdv_estimated_flights", "pdv_cloud_get_tables", "pdv_cloud_get_image", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_run_static", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_philox_blocks", "pdv_issue_peaks",
            "pdv_last_launch_info", "pdv_last_error", "pdv_version")
 
 
@@ -100,6 +100,7 @@ def lib() -> C.CDLL:
         L.pdv_cloud_destroy.argtypes = [vp]
         L.pdv_cloud_destroy.restype = None
         L.pdv_cloud_get_info.argtypes = [vp, C.POINTER(CloudInfo)]
+        L.pdv_estimated_flights.argtypes = [vp, C.POINTER(RunOpts), dp]
         L.pdv_cloud_get_tables.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.pdv_cloud_get_image.argtypes = [vp, C.POINTER(ImageLayout), vp, C.c_size_t]
         L.pdv_cloud_gas_tables.argtypes = [vp, C.c_double, vp, vp, vp, vp]
@@ -112,6 +113,7 @@ def lib() -> C.CDLL:
         L.pdv_spectrum_peaks.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_double, C.c_double, vp,
                                          C.POINTER(PeakOpts), vp, C.c_int32, vp]
         L.pdv_phase_sampling_check.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int32, vp, vp, C.POINTER(PhaseCheck), vp]
+        L.pdv_philox_blocks.argtypes = [vp, C.c_int32, C.c_uint64, vp, vp, vp]
         L.pdv_issue_peaks.argtypes = [C.c_double, dp, dp, dp, C.POINTER(C.c_int32), vp]
         L.pdv_last_launch_info.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32),
                                            C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -171,6 +173,15 @@ class Cloud:
         ci.struct_size = C.sizeof(CloudInfo)
         _check(lib().pdv_cloud_get_info(self.handle, C.byref(ci)))
         return {k: getattr(ci, k) for k, _ in CloudInfo._fields_ if k != "struct_size"}
+
+    def estimated_flights(self, run: dict | None = None) -> float:
+        """The library's estimate of the flights per history of this cloud under the run options (pdv_estimated_flights): the
+        cost a multi-GPU caller balances its split with."""
+        out = C.c_double(0.0)
+        o = _opts(dict(n_bins=1, v_lo=0.0, v_hi=1.0, aperture_sr=1.0, **{k: run[k] for k in ("mode", "max_events", "roulette_survival",
+                                                                                             "single_scatter_only") if run and k in run}))
+        _check(lib().pdv_estimated_flights(self.handle, C.byref(o), C.byref(out)))
+        return out.value
 
     def tables(self) -> dict:
         i = self.info()
@@ -421,6 +432,15 @@ def pdv_phase_sampling_check(cloud: Cloud, class_index: int, n_samples: int, see
     n = max(int(n_samples), 1)
     return dict(hist_table=ht, hist_exact=he, mean_cos_table=info.sum_cos_table / n, mean_cos_exact=info.sum_cos_exact / n,
                 i_max=info.i_max, n_trials=int(info.n_trials), n_bound_violations=int(info.n_bound_violations))
+
+
+def pdv_philox_blocks(counters, seed: int):
+    """Raw Philox4x32-10 blocks of the device generator (pdv_philox_blocks): counters uint32 [n, 4], key = the two words of `seed`.
+    -> (static, shared, param): uint32 [n, 4] each, one per key path of the transport kernel."""
+    c = np.ascontiguousarray(counters, dtype=np.uint32).reshape(-1, 4)
+    outs = [np.zeros_like(c) for _ in range(3)]
+    _check(lib().pdv_philox_blocks(c.ctypes.data, c.shape[0], int(seed), *[o.ctypes.data for o in outs]))
+    return tuple(outs)
 
 
 def pdv_issue_peaks(millis: float = 50.0, stream: int | None = None) -> dict:

@@ -523,6 +523,16 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
     const int lb = !kv.poly && kv.alt && !kv.analog && !kv.sso && !kv.trace && kv.dm == 0 ? PDV_LB_THREADS_LONG : PDV_LB_THREADS;
     if (block == 0) block = (n_units > 1 && 2 * (size_t)(smem + 1024 + 18432) <= di.smem_optin + 1024) ? lb / 2 : lb;   // 18 KB: the kernel's static shared memory (warp queues)
     block = std::min(block, lb);
+    // dynamic + STATIC shared memory (warp queues, keys, statistics: ~17 KB) must fit the opt-in limit of a block: without this
+    // check a launch within 17 KB of the limit failed later, inside cudaFuncSetAttribute, with a misleading CUDA error
+    size_t static_smem = 0;
+    CU(transport_static_smem(kv, &static_smem), "cudaFuncGetAttributes(transport kernel)");
+    if ((size_t)smem + static_smem > di.smem_optin) {
+        char msg[200];
+        std::snprintf(msg, sizeof(msg), "cloud tables + histogram (%d bytes) + the kernel's static shared memory (%zu) exceed the %zu bytes "
+                      "of one block", smem, static_smem, di.smem_optin);
+        return fail(PDV_E_UNSUPPORTED, msg);
+    }
     {
         struct Key { KernelVariant v; int block, smem, device; };
         static std::mutex mu;
@@ -537,6 +547,7 @@ pdv_status make_plan(const pdv_cloud *const *clouds, int n_clouds, int n_units, 
         }
     }
     if (per_sm < 1) return fail(PDV_E_UNSUPPORTED, "transport kernel does not fit on an SM with these tables");
+    (void)static_smem;
     if (o->blocks_per_sm > 0) per_sm = std::min(per_sm, o->blocks_per_sm);
     long long grid = (long long)di.n_sm * per_sm;
     const unsigned long long total = n_photons * (unsigned long long)n_units;
@@ -930,6 +941,24 @@ pdv_status pdv_cloud_get_info(const pdv_cloud *c, pdv_cloud_info *out) {
     return PDV_OK;
 }
 
+pdv_status pdv_estimated_flights(const pdv_cloud *c, const void *opts, double *out) {
+    g_err.clear();
+    if (!c || !out) return fail(PDV_E_INVALID, "cloud / out is NULL");
+    pdv_run_opts o;
+    std::memset(&o, 0, sizeof(o));
+    if (opts) {
+        const pdv_run_opts *in = static_cast<const pdv_run_opts *>(opts);
+        if (in->struct_size != sizeof(pdv_run_opts)) return fail(PDV_E_INVALID, "opts->struct_size mismatch");
+        o = *in;
+        if (o.max_events > 0 && !(o.roulette_survival > 0.0 && o.roulette_survival <= 1.0)) return fail(PDV_E_INVALID, "roulette_survival not in (0,1]");
+    }
+    const HostCloud &h = c->host;
+    double om = 0.0;
+    for (int i = 0; i < h.n_classes; ++i) om += h.p_class[i] * h.k_sca[i] / h.k_ext[i];
+    *out = estimated_flights(h.tau_ext, om, &o);
+    return PDV_OK;
+}
+
 pdv_status pdv_cloud_get_tables(const pdv_cloud *c, double *k_ext, double *k_sca, double *g, double *p_class,
                                 double *phase, double *T_edge) {
     g_err.clear();
@@ -1181,6 +1210,34 @@ pdv_status pdv_phase_sampling_check(const pdv_cloud *cloud, int32_t class_index,
         info->sum_cos_table = sums[0]; info->sum_cos_exact = sums[1]; info->i_max = (double)(float)i_max;
         info->n_trials = cnts[0]; info->n_bound_violations = cnts[1];
     }
+    return PDV_OK;
+}
+
+pdv_status pdv_philox_blocks(const uint32_t *counters, int32_t n, uint64_t seed, uint32_t *out_static, uint32_t *out_shared,
+                             uint32_t *out_param) {
+    g_err.clear();
+    if (n < 0 || n > (1 << 20) || (n > 0 && (!counters || !out_static || !out_shared || !out_param)))
+        return fail(PDV_E_INVALID, "pdv_philox_blocks: need 0 <= n <= 2^20 and non-NULL buffers");
+    if (n == 0) return PDV_OK;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(PDV_E_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    uint32_t key0[10], key1[10];                              // the round keys as make_plan derives them from the seed
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { key0[r] = k0; key1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+    const size_t bytes = 16 * (size_t)n;
+    unsigned char *d = nullptr;
+    CU(cudaMalloc(&d, 4 * bytes), "cudaMalloc(philox check)");
+    cudaError_t e = cudaMemcpy(d, counters, bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_philox_check(key0, key1, reinterpret_cast<const uint4 *>(d), n, reinterpret_cast<uint4 *>(d + bytes),
+                                                  reinterpret_cast<uint4 *>(d + 2 * bytes), reinterpret_cast<uint4 *>(d + 3 * bytes), nullptr);
+    if (e == cudaSuccess) e = cudaMemcpy(out_static, d + bytes, bytes, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(out_shared, d + 2 * bytes, bytes, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(out_param, d + 3 * bytes, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "philox check kernel");
     return PDV_OK;
 }
 

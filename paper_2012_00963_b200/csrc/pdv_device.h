@@ -147,6 +147,11 @@ struct LaunchShape { int grid, block, smem; };
 struct KernelVariant { bool poly, analog, sso, trace, roulette; int dm; bool alt; };   // dm: see transport_kernel
 cudaError_t launch_transport(const RunParams &rp, KernelVariant v, LaunchShape shape, cudaStream_t st);
 cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, int *out);
+cudaError_t transport_static_smem(KernelVariant v, size_t *out);      // static shared memory of the instantiation (warp queues, keys, stats)
+// Test-only (pin P13): raw Philox4x32-10 blocks of n counters through the three key paths of the kernels; key0/key1: HOST [10]
+// round keys, ctr and the outputs: DEVICE [n].
+cudaError_t launch_philox_check(const uint32_t *key0, const uint32_t *key1, const uint4 *ctr, int n, uint4 *out_static,
+                                uint4 *out_shared, uint4 *out_param, cudaStream_t st);
 cudaError_t launch_finalize(const unsigned long long *hist, const unsigned long long *hist2, const unsigned long long *stats,
                             uint32_t n_units, uint32_t n_bins, double *out_hist, double *out_hist2, pdv_run_stats *out_stats,
                             cudaStream_t st);

@@ -760,7 +760,24 @@ static cudaError_t occ_t(int block, int smem, int *out) {
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT>, block, smem);
 }
 
+template <bool POLY, bool ANALOG, bool SSO, bool TRACE, bool ROUL, int DM, bool ALT = false>
+static cudaError_t sattr_t(size_t *out) {
+    cudaFuncAttributes a;
+    cudaError_t e = cudaFuncGetAttributes(&a, transport_kernel<POLY, ANALOG, SSO, TRACE, ROUL, DM, ALT>);
+    if (e == cudaSuccess) *out = a.sharedSizeBytes;
+    return e;
+}
+
 // DM = 0 / 1 exist for the production variants only; single-scatter-only and trace runs always take the general kernel.
+template <bool A, bool B, bool C, bool D, bool E>
+static cudaError_t sattr_dm(int dm, size_t *out) {
+    if constexpr (C || D) {
+        return sattr_t<A, B, C, D, E, 2>(out);
+    } else {
+        return dm == 0 ? sattr_t<A, B, C, D, E, 0>(out) : dm == 1 ? sattr_t<A, B, C, D, E, 1>(out)
+             : dm == 3 ? sattr_t<A, B, C, D, E, 3>(out) : sattr_t<A, B, C, D, E, 2>(out);
+    }
+}
 template <bool A, bool B, bool C, bool D, bool E>
 static cudaError_t launch_dm(int dm, const RunParams &rp, LaunchShape s, cudaStream_t st) {
     if constexpr (C || D) {
@@ -825,6 +842,61 @@ cudaError_t transport_max_blocks_per_sm(KernelVariant v, int block, int smem, in
 #else
     return PDV_DISPATCH(occ_dm, block, smem, out);
 #endif
+}
+
+cudaError_t transport_static_smem(KernelVariant v, size_t *out) {
+#ifdef PDV_FEW
+    if (!alt_variant(v)) {
+        if (v.analog || v.sso || v.trace || v.dm != 0) return cudaErrorNotSupported;
+        if (!v.poly) return v.roulette ? cudaErrorNotSupported : sattr_t<false, false, false, false, false, 0>(out);
+        return v.roulette ? sattr_t<true, false, false, false, true, 0>(out) : sattr_t<true, false, false, false, false, 0>(out);
+    }
+#endif
+    if (alt_variant(v)) {
+        if (v.poly) return v.roulette ? sattr_t<true, false, false, false, true, 0, true>(out) : sattr_t<true, false, false, false, false, 0, true>(out);
+        return v.roulette ? sattr_t<false, false, false, false, true, 0, true>(out) : sattr_t<false, false, false, false, false, 0, true>(out);
+    }
+#ifdef PDV_FEW
+    return cudaErrorNotSupported;
+#else
+    return PDV_DISPATCH(sattr_dm, out);
+#endif
+}
+
+// ---- pin P13: the device Philox4x32-10 through each of its three key paths, raw blocks -----------------------
+// Test-only kernel: block i of the output is philox4x32_10(ctr[i], keys) computed (a) with the round keys in static shared
+// memory (s_keys: launch draw, rare paths), (b) through SharedKeys, a shared address in a register (the flight loop of most
+// instantiations), (c) through ParamKeys, the constant bank (KEYS_PARAM instantiations).  The host compares the three with the
+// published Random123 vectors.
+struct PhiloxKeyParams { uint32_t key0[10], key1[10]; };
+__global__ void philox_check_kernel(PhiloxKeyParams P, const uint4 *ctr, int n, uint4 *out_static, uint4 *out_shared, uint4 *out_param) {
+    __shared__ __align__(16) uint4 keys_copy[5];
+    const int tid = threadIdx.x;
+    if (tid < 5) {
+        s_keys[tid] = make_uint4(P.key0[2 * tid], P.key1[2 * tid], P.key0[2 * tid + 1], P.key1[2 * tid + 1]);      // as transport_kernel stages them
+        keys_copy[tid] = s_keys[tid];
+    }
+    __syncthreads();
+    const uint32_t saddr = (uint32_t)__cvta_generic_to_shared(keys_copy);
+    for (int i = blockIdx.x * blockDim.x + tid; i < n; i += gridDim.x * blockDim.x) {
+        const uint4 c = ctr[i];
+        uint4 o;
+        philox4x32_10(c.x, c.y, c.z, c.w, s_keys, o.x, o.y, o.z, o.w);
+        out_static[i] = o;
+        philox4x32_10(c.x, c.y, c.z, c.w, SharedKeys{saddr}, o.x, o.y, o.z, o.w);
+        out_shared[i] = o;
+        philox4x32_10(c.x, c.y, c.z, c.w, ParamKeys{P.key0, P.key1}, o.x, o.y, o.z, o.w);
+        out_param[i] = o;
+    }
+}
+
+cudaError_t launch_philox_check(const uint32_t *key0, const uint32_t *key1, const uint4 *ctr, int n, uint4 *out_static,
+                                uint4 *out_shared, uint4 *out_param, cudaStream_t st) {
+    if (n <= 0) return cudaSuccess;
+    PhiloxKeyParams P;
+    for (int r = 0; r < 10; ++r) { P.key0[r] = key0[r]; P.key1[r] = key1[r]; }
+    philox_check_kernel<<<(n + 127) / 128, 128, 0, st>>>(P, ctr, n, out_static, out_shared, out_param);
+    return cudaGetLastError();
 }
 
 // ---- finalize: Q31 integers -> doubles (H12 input; stats) ------------------------------------------------------

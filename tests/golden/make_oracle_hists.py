@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Writes the stored oracle histograms tests/golden/oracle_hist_*.json -- calls ONLY oracle/ (and pdv_workloads for the inputs).
 
-    python tests/golden/make_oracle_hists.py [name ...]        # default: all; takes ~20 min on 8 cores
+    python tests/golden/make_oracle_hists.py [name ...]        # default: all; takes ~35 min on 8 cores
 
 The full-size GPU parity tests (tests/test_gpu_parity.py::test_full_size_*) compare 1e8 ... 1e9-history GPU runs with the oracle.
 An oracle run the test can afford live (a few 1e6 histories) leaves the comparison without power where it matters (the tolerance
@@ -39,15 +39,21 @@ JOBS = {
     "cfg4_cloud36": (3, 36, 100_000_000),
     "cfg4_cloud44": (3, 44, 100_000_000),
     "cfg5": (4, 0, 400_000_000),
+    # the other 44 clouds of config 4 at 2e7 histories each (twice the GPU's 1e7), in chunks of 1e6: filled in below
     # row f4 (pdv_workloads.gas_spectrogram, bench.py --config 6): with a gas the spectrum depends on the snapshot time (DESIGN.md
     # R38), so a spectrum is stored per snapshot: the first and the last of the 20.  ("gas", snapshot index, histories)
     "f4gas_snap00": ("gas", 0, 100_000_000),
     "f4gas_snap19": ("gas", 19, 100_000_000),
 }
+for _i in range(48):
+    if f"cfg4_cloud{_i:02d}" not in JOBS:
+        JOBS[f"cfg4_cloud{_i:02d}"] = (3, _i, 20_000_000)
+SMALL_CHUNK = 1_000_000     # chunk of the 2e7-history jobs: 20 chunks for the batch-means variances
 
 
 def make(name: str) -> str:
     idx, ci, n = JOBS[name]
+    chunk = CHUNK if n >= 100_000_000 else SMALL_CHUNK
     gas = None
     if idx == "gas":
         from oracle import gas as ogas
@@ -62,10 +68,12 @@ def make(name: str) -> str:
     hist = hist2 = None
     stats: dict = {}
     t0 = time.time()
-    for first in range(0, n, CHUNK):
-        r = omc.run(oc, run, n_photons=min(CHUNK, n - first), first_id=first, gas=gas)
+    chunk_stats = []        # statistics of every chunk: batch-means variances of the weights that are far from 0/1 per history
+    for first in range(0, n, chunk):
+        r = omc.run(oc, run, n_photons=min(chunk, n - first), first_id=first, gas=gas)
         hist = r.hist if hist is None else hist + r.hist
         hist2 = r.hist2 if hist2 is None else hist2 + r.hist2
+        chunk_stats.append({k: (int(v) if isinstance(v, int) else float(v)) for k, v in r.stats.items()})
         for k, v in r.stats.items():
             stats[k] = max(stats.get(k, 0), v) if k == "max_events_in_history" else stats.get(k, 0) + v
     out = {
@@ -74,6 +82,7 @@ def make(name: str) -> str:
         "run": {k: run[k] for k in ("n_bins", "v_lo", "v_hi", "aperture_sr", "mode", "max_events", "roulette_survival")},
         "tau_ext": oc.tau_ext, "seconds": round(time.time() - t0, 1), "threads": os.cpu_count(),
         "stats": {k: (int(v) if isinstance(v, int) else float(v)) for k, v in stats.items()},
+        "chunk": chunk, "chunk_stats": chunk_stats,
         "hist": [float(x) for x in hist], "hist2": [float(x) for x in hist2],
     }
     path = os.path.join(HERE, f"oracle_hist_{name}.json")

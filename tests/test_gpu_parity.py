@@ -15,7 +15,7 @@ import pdv_workloads as W
 from oracle import cloud as ocloud
 from oracle import mc as omc
 
-from histcmp import compare, load_golden
+from histcmp import compare, load_golden, per_history_variance
 
 pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("_library_is_built")]
 
@@ -50,7 +50,13 @@ def _assert_stats_parity(gs, n_g, o, same_game=True):
     DESIGN.md reading R20), so the number of events per history is not comparable, only the expectations are."""
     for key in ("detected", "escaped", "absorbed_particles", "absorbed_surface", "truncated"):
         a, b = float(gs[key]) / n_g, o.stats[key] / o.n_photons
-        sig = math.sqrt(max(a, 1e-12) / n_g + max(b, 1e-12) / o.n_photons)
+        sig = math.sqrt(max(a, 1e-12) / n_g + max(b, 1e-12) / o.n_photons)      # Bernoulli bound: w <= 1 gives var <= mean
+        # A history's share of `absorbed_particles` or `escaped` is far from 0/1, so that bound is 2-3 times too wide for them.
+        # Stored oracle runs carry per-chunk statistics: the batch-means variance of one history's contribution (both sides
+        # sample the same distribution, so it serves the GPU's term too), times 1.5 for the uncertainty of that estimate.
+        var_h = per_history_variance(o, key) if hasattr(o, "chunk_stats") else None
+        if var_h is not None:
+            sig = min(sig, 1.5 * math.sqrt(var_h / n_g + var_h / o.n_photons) + 1e-15)
         assert abs(a - b) < 5 * sig, (key, a, b, sig)
     if same_game:
         a = float(gs["particle_events"]) / n_g
@@ -536,13 +542,15 @@ def test_full_size_configs_3_4_5(P):
     # 1e7 * 2^31 exceeds 2^53: the double sum of exact Q31 terms may round in the last bit
     assert np.all(r.stats["histories"] == n) and np.all(np.abs(r.conservation_residual()) < 1e-7)
     assert np.allclose(r.hist.sum(axis=2), r.stats["detected"], rtol=1e-12)
-    # sampled clouds, thin ... thick (tau 1.2, 0.9, 9.3, 18.6), each against 1e8 oracle histories
-    for i in (3, 22, 36, 44):
+    # ALL 48 clouds against stored oracle runs: four of them (thin ... thick: tau 1.2, 0.9, 9.3, 18.6) at 1e8 oracle histories,
+    # the other 44 at 2e7 (20 chunks of 1e6: batch-means variances for the statistics)
+    for i in range(48):
         oo = load_golden(f"cfg4_cloud{i:02d}")
-        assert oo.n_photons >= 10 * n and oo.tau_ext == pytest.approx(clouds[i].info()["tau_ext"], rel=1e-9)
-        _assert_hist_parity(r.hist[i, 0], r.hist2[i, 0], n, oo, min_ndf=50)
+        big = i in (3, 22, 36, 44)
+        assert oo.n_photons >= (10 if big else 2) * n and oo.tau_ext == pytest.approx(clouds[i].info()["tau_ext"], rel=1e-9)
+        _assert_hist_parity(r.hist[i, 0], r.hist2[i, 0], n, oo, min_ndf=50 if big else 20)
         _assert_stats_parity(r.stats[i, 0], n, oo)
-        assert r.stats[i, 0]["particle_events"] / n == pytest.approx(oo.stats["particle_events"] / oo.n_photons, rel=3e-3)
+        assert r.stats[i, 0]["particle_events"] / n == pytest.approx(oo.stats["particle_events"] / oo.n_photons, rel=3e-3), i
     # ---- config 5
     cfg = W.config(4)
     c = P.pdv_cloud_create(cfg["clouds"][0])
