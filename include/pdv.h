@@ -96,7 +96,11 @@ pdv_status pdv_lognormal_classes(double d_median, double sigma_ln, int32_t n, do
  * PAPER.md:128-135); the class hit probabilities P_c ~ w_c d_c^2 K_ext,c (Eq. 8); the mass-extinction
  * coefficient kappa = 3 sum w d^2 K_ext / (2 rho0 sum w d^3) and tau_ext = kappa m0 (Eq. 10);
  * the depth table T_j (Eq. 20) -- and, when a CUDA device is present, copies the fp32 tables to it.
- * *out receives the new cloud; release it with pdv_cloud_destroy. */
+ * *out receives the new cloud; release it with pdv_cloud_destroy.
+ * Streams: the upload goes through a pinned staging buffer and a stream of the library's own and waits for that copy only; a
+ * device buffer recycled from a destroyed cloud is reused once the runs that read the old cloud have finished (an event behind
+ * its last launch), not after a device-wide synchronisation.  So creating or destroying clouds while a long pdv_mc_run with
+ * device outputs is in flight on another stream neither waits for that run nor disturbs it. */
 pdv_status pdv_cloud_create(const pdv_cloud_params *params, pdv_cloud **out);
 
 /* NULL is a no-op.  The cloud must not be in use by a running pdv_mc_run. */
@@ -379,6 +383,12 @@ pdv_status pdv_issue_peaks(double millis, double *ffma_thread_inst_per_s, double
  * (0 depth table, 1 closed form, 2 general, 3 gas units).  The result of a run never depends on it. */
 pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block,
                                 int32_t *smem_bytes, int32_t *variant);
+
+/* The same for the last run this thread enqueued on `cuda_stream` (the library remembers the 16 most recently used streams of
+ * each host thread): after two asynchronous runs on two streams each one's kernel time can still be read.  Zeros if the thread
+ * has not run anything on that stream. */
+pdv_status pdv_launch_info_on_stream(void *cuda_stream, int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block,
+                                     int32_t *smem_bytes, int32_t *variant);
 
 /* Thread-local message of the last failing call on this thread; "" if none.  Valid until the next call. */
 const char *pdv_last_error(void);

@@ -20,7 +20,7 @@ PDV_STATIC_SCRATCH_BYTES = 2 << 20
 
 EXPORTS = ("pdv_lognormal_classes", "pdv_cloud_create", "pdv_cloud_destroy", "pdv_cloud_get_info",
            "pdv_estimated_flights", "pdv_cloud_get_tables", "pdv_cloud_get_image", "pdv_cloud_gas_tables", "pdv_mc_run", "pdv_mc_run_static", "pdv_mc_trace", "pdv_spectrogram", "pdv_spectrum_peaks", "pdv_phase_sampling_check", "pdv_philox_blocks", "pdv_issue_peaks",
-           "pdv_last_launch_info", "pdv_last_error", "pdv_version")
+           "pdv_last_launch_info", "pdv_launch_info_on_stream", "pdv_last_error", "pdv_version")
 
 
 class PdvError(RuntimeError):
@@ -117,6 +117,7 @@ def lib() -> C.CDLL:
         L.pdv_issue_peaks.argtypes = [C.c_double, dp, dp, dp, C.POINTER(C.c_int32), vp]
         L.pdv_last_launch_info.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32),
                                            C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.pdv_launch_info_on_stream.argtypes = [vp] + L.pdv_last_launch_info.argtypes
         L.pdv_last_error.restype = C.c_char_p
         L.pdv_version.restype = C.c_char_p
         for name in EXPORTS:
@@ -450,9 +451,14 @@ def pdv_issue_peaks(millis: float = 50.0, stream: int | None = None) -> dict:
     return dict(ffma_thread_inst_per_s=f.value, mufu_thread_inst_per_s=m.value, sm_clock_mhz=z.value, n_sm=n.value)
 
 
-def pdv_last_launch_info() -> dict:
+def pdv_last_launch_info(stream: int | None = None) -> dict:
+    """Launch statistics of this thread's last run; stream (a cudaStream_t as int, 0 = the default stream): of its last run on
+    that stream (pdv_launch_info_on_stream)."""
     k, g, b, s, v = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0)
     ms = C.c_float(0)
-    lib().pdv_last_launch_info(C.byref(k), C.byref(ms), C.byref(g), C.byref(b), C.byref(s), C.byref(v))
+    if stream is None:
+        lib().pdv_last_launch_info(C.byref(k), C.byref(ms), C.byref(g), C.byref(b), C.byref(s), C.byref(v))
+    else:
+        lib().pdv_launch_info_on_stream(C.c_void_p(stream), C.byref(k), C.byref(ms), C.byref(g), C.byref(b), C.byref(s), C.byref(v))
     return dict(n_kernels=k.value, transport_ms=ms.value, grid=g.value, block=b.value, smem_bytes=s.value, variant=v.value,
                 alt=bool(v.value & 32))

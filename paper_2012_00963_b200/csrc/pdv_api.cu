@@ -26,20 +26,50 @@ struct pdv_cloud {
     mutable unsigned char *d_blob = nullptr;
     mutable size_t d_bytes = 0;
     mutable int device = -1;
+    // Recorded (by run_impl) behind every launch that reads d_blob.  It travels with the buffer into the cache when the cloud is
+    // destroyed: the next cloud that takes the buffer waits for THIS event only -- i.e. for the runs that could still read the
+    // old image -- instead of synchronising the whole device.  Created with the buffer, without timing.
+    mutable cudaEvent_t last_read = nullptr;
+    mutable bool read_pending = false;
+    // Gas environment: the per-snapshot device images of this cloud for the snapshot times of its last run (host copies).  A
+    // spectrogram that is run again for the same times (more histories, another seed: what bench.py's steps do) skips the host
+    // build of its images (0.4 ms each); another list of times rebuilds them.  Guarded by mu.
+    mutable std::vector<double> gas_t;
+    mutable std::vector<std::vector<unsigned char>> gas_imgs;
 };
 
 namespace {
 
 thread_local std::string g_err;
-thread_local struct { int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0, variant = 0; bool pending = false; } g_last;
 
-// Timing events of the last run of this host thread (pdv_last_launch_info).
-struct LastEvents {
+// Launch statistics and timing events of the last run of this host thread ON EACH STREAM it used (pdv_last_launch_info /
+// pdv_launch_info_on_stream): two asynchronous runs on two streams keep their own events, so the first one's kernel time is not
+// overwritten by the second.  A small table (the 16 most recently used streams of the thread); events are created once per slot.
+struct LastLaunch {
+    int n_kernels = 0; float ms = 0.f; int grid = 0, block = 0, smem = 0, variant = 0; bool pending = false;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     int device = -1;
-    // process teardown: the CUDA context may already be gone; leak rather than fault
+    cudaStream_t stream = nullptr;
+    unsigned long long used = 0;                              // recency stamp; 0: slot never used
+    // process teardown: the CUDA context may already be gone; the events are leaked rather than destroyed
 };
-thread_local LastEvents g_ev;
+thread_local LastLaunch g_launches[16];
+thread_local unsigned long long g_launch_clock = 0;
+thread_local LastLaunch *g_last_ptr = nullptr;                // the slot of the most recent run of this thread
+#define g_last (*g_last_ptr)
+#define g_ev (*g_last_ptr)
+
+LastLaunch *launch_slot(cudaStream_t st, bool create) {
+    LastLaunch *oldest = &g_launches[0];
+    for (LastLaunch &l : g_launches) {
+        if (l.used && l.stream == st) return &l;
+        if (l.used < oldest->used) oldest = &l;
+    }
+    if (!create) return nullptr;
+    oldest->stream = st;
+    oldest->n_kernels = 0; oldest->ms = 0.f; oldest->pending = false; oldest->grid = oldest->block = oldest->smem = oldest->variant = 0;
+    return oldest;                                            // its events, if any, are reused
+}
 
 // Pinned host staging buffer of this host thread for the read-back of a host-output run (one D2H copy at PCIe speed instead
 // of several pageable ones); grown on demand, never shrunk.
@@ -271,7 +301,7 @@ void build_blob(const HostCloud &h, std::vector<unsigned char> &blob, const GasU
 // clouds never reaches cudaMalloc / cudaFree after its first turn, whatever ran before it (round 2: the 14-cloud sweep at the
 // end of bench.py's default run took 426 ms per end-to-end step instead of 66, the cache being full of smaller buffers).
 struct BlobCache {
-    struct Entry { unsigned char *p; size_t bytes; int device; };
+    struct Entry { unsigned char *p; size_t bytes; int device; cudaEvent_t last_read; bool read_pending; };
     std::mutex mu;
     std::deque<Entry> free_list;                               // oldest first
     size_t total = 0;
@@ -280,51 +310,89 @@ struct BlobCache {
         while (cap < bytes) cap <<= 1;
         return cap;
     }
-    unsigned char *take(size_t cap, int device) {             // a cached buffer of exactly this capacity
+    bool take(size_t cap, int device, Entry &out) {           // a cached buffer of exactly this capacity; prefers one nobody reads any more
         std::lock_guard<std::mutex> lk(mu);
+        long pick = -1;
         for (size_t i = free_list.size(); i-- > 0;)
             if (free_list[i].device == device && free_list[i].bytes == cap) {
-                unsigned char *p = free_list[i].p;
-                total -= cap;
-                free_list.erase(free_list.begin() + (long)i);
-                return p;
+                if (pick < 0) pick = (long)i;
+                if (!free_list[i].read_pending || cudaEventQuery(free_list[i].last_read) == cudaSuccess) { pick = (long)i; break; }
             }
-        return nullptr;
+        if (pick < 0) { cudaGetLastError(); return false; }
+        cudaGetLastError();                                   // cudaErrorNotReady of a query is not an error
+        out = free_list[(size_t)pick];
+        total -= cap;
+        free_list.erase(free_list.begin() + pick);
+        return true;
     }
-    void give(unsigned char *p, size_t cap, int device) {
-        std::vector<unsigned char *> evict;
+    void give(const Entry &e) {
+        std::vector<Entry> evict;
         {
             std::lock_guard<std::mutex> lk(mu);
-            free_list.push_back({p, cap, device});
-            total += cap;
+            free_list.push_back(e);
+            total += e.bytes;
             while (free_list.size() > 256 || total > ((size_t)256 << 20)) {
-                evict.push_back(free_list.front().p);
+                evict.push_back(free_list.front());
                 total -= free_list.front().bytes;
                 free_list.pop_front();
             }
         }
-        for (unsigned char *q : evict) cudaFree(q);
+        for (const Entry &q : evict) { cudaFree(q.p); if (q.last_read) cudaEventDestroy(q.last_read); }      // cudaFree waits for the device
     }
 };
 BlobCache g_blob_cache;
+
+// Upload path of the cloud images: a pinned staging buffer per host thread and ONE library-owned non-blocking stream per device.
+// pdv_cloud_create copies the image into the staging buffer, enqueues one cudaMemcpyAsync on that stream and waits for that
+// stream only -- a kernel running on any other stream (a long pdv_mc_run with device outputs) neither delays the creation nor
+// is delayed by it.  (Round 2: a blocking cudaMemcpy from pageable memory plus a cudaDeviceSynchronize on every reuse of a cached
+// buffer: creating one cloud waited for every stream's work.)
+thread_local PinnedStage g_upload_stage;
+pdv_status upload_stream(int device, cudaStream_t *out) {
+    static std::mutex mu;
+    static cudaStream_t streams[64] = {nullptr};
+    std::lock_guard<std::mutex> lk(mu);
+    cudaStream_t &s = streams[device & 63];
+    if (!s) CU(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking), "cudaStreamCreate(upload)");
+    *out = s;
+    return PDV_OK;
+}
 
 pdv_status ensure_on_device(const pdv_cloud *c, int device) {
     std::lock_guard<std::mutex> lk(c->mu);
     if (c->d_blob && c->device == device) return PDV_OK;
     if (c->d_blob) return fail(PDV_E_INVALID, "cloud was uploaded to another CUDA device");
     const size_t cap = BlobCache::capacity_for(c->blob.size());
-    unsigned char *d = g_blob_cache.take(cap, device);
-    if (d) {
-        // the buffer belonged to a destroyed cloud: whatever may still read it (a run enqueued on a non-blocking stream)
-        // must be over before it is overwritten -- what cudaFree used to guarantee
-        CU(cudaDeviceSynchronize(), "cudaDeviceSynchronize(reuse of a cloud buffer)");
+    BlobCache::Entry e{nullptr, cap, device, nullptr, false};
+    if (g_blob_cache.take(cap, device, e)) {
+        // the buffer belonged to a destroyed cloud: the runs that may still read the old image (enqueued on any stream) must
+        // be over before it is overwritten -- they end at the buffer's last_read event; nothing else is waited for
+        if (e.read_pending) CU(cudaEventSynchronize(e.last_read), "cudaEventSynchronize(reuse of a cloud buffer)");
     } else {
-        CU(cudaMalloc(&d, cap), "cudaMalloc(cloud tables)");
+        CU(cudaMalloc(&e.p, cap), "cudaMalloc(cloud tables)");
+        cudaError_t ee = cudaEventCreateWithFlags(&e.last_read, cudaEventDisableTiming);
+        if (ee != cudaSuccess) { cudaFree(e.p); return cuda_fail(ee, "cudaEventCreate(cloud buffer)"); }
     }
+    auto give_back = [&]() { g_blob_cache.give(BlobCache::Entry{e.p, cap, device, e.last_read, false}); };
+    cudaStream_t up = nullptr;
+    pdv_status s = upload_stream(device, &up);
+    if (s != PDV_OK) { give_back(); return s; }
+    if (g_upload_stage.bytes < c->blob.size()) {
+        if (g_upload_stage.p) cudaFreeHost(g_upload_stage.p);
+        g_upload_stage.p = nullptr; g_upload_stage.bytes = 0;
+        const size_t want = std::max(BlobCache::capacity_for(c->blob.size()), (size_t)1 << 18);
+        cudaError_t ee = cudaMallocHost(&g_upload_stage.p, want);
+        if (ee != cudaSuccess) { give_back(); return cuda_fail(ee, "cudaMallocHost(upload staging)"); }
+        g_upload_stage.bytes = want;
+    }
+    std::memcpy(g_upload_stage.p, c->blob.data(), c->blob.size());
+    cudaError_t ee = cudaMemcpyAsync(e.p, g_upload_stage.p, c->blob.size(), cudaMemcpyHostToDevice, up);
+    if (ee == cudaSuccess) ee = cudaStreamSynchronize(up);    // the staging buffer is free again and the image is resident
+    if (ee != cudaSuccess) { give_back(); return cuda_fail(ee, "cudaMemcpyAsync(cloud tables)"); }
     c->d_bytes = cap;                                         // capacity of the buffer (the image fills blob.size() of it)
-    cudaError_t e = cudaMemcpy(d, c->blob.data(), c->blob.size(), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(cloud tables)"); }
-    c->d_blob = d;
+    c->d_blob = e.p;
+    c->last_read = e.last_read;
+    c->read_pending = false;
     c->device = device;
     return PDV_OK;
 }
@@ -358,7 +426,9 @@ pdv_status scratch_alloc(size_t bytes, int device, cudaStream_t st, StreamScratc
     return PDV_OK;
 }
 
-pdv_status ensure_events(int device) {
+pdv_status ensure_events(int device, cudaStream_t st) {
+    g_last_ptr = launch_slot(st, true);
+    g_last.used = ++g_launch_clock;
     if (g_ev.e0 && g_ev.device != device) {
         cudaEventDestroy(g_ev.e0); cudaEventDestroy(g_ev.e1);
         g_ev.e0 = g_ev.e1 = nullptr;
@@ -584,25 +654,50 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *
     if (any_gas) {
         if (!t_snap) return fail(PDV_E_UNSUPPORTED, "gas clouds need snapshot times (not available through pdv_mc_trace)");
         max_blob = 0;
-        // the units are independent: built on parallel host threads (0.4 ms each; a 20-snapshot spectrogram 7.6 -> ~1 ms)
-        std::vector<std::vector<unsigned char>> imgs((size_t)n_units);
+        // the units are independent: built on parallel host threads (0.4 ms each; a 20-snapshot spectrogram 7.6 -> ~1 ms), and
+        // kept with their cloud: the next run of the same cloud at the same snapshot times reuses them (pdv_cloud::gas_imgs)
+        std::vector<const std::vector<unsigned char> *> imgs((size_t)n_units, nullptr);
+        std::vector<std::unique_lock<std::mutex>> locks;      // the clouds' caches stay locked while this call reads them
+        std::vector<int> todo;                                // units whose image must be built
         {
+            std::vector<const pdv_cloud *> uniq(clouds, clouds + n_clouds);          // the same cloud may come twice in one launch
+            std::sort(uniq.begin(), uniq.end());                                       // one lock order for every caller
+            uniq.erase(std::unique(uniq.begin(), uniq.end()), uniq.end());
+            for (const pdv_cloud *c : uniq) locks.emplace_back(c->mu);
+            std::vector<const pdv_cloud *> seen;
+            for (int i = 0; i < n_clouds; ++i) {
+                const pdv_cloud *c = clouds[i];
+                if (std::find(seen.begin(), seen.end(), c) != seen.end()) continue;
+                seen.push_back(c);
+                const bool hit = c->gas_t.size() == (size_t)n_snap && std::equal(c->gas_t.begin(), c->gas_t.end(), t_snap) &&
+                                 c->gas_imgs.size() == (size_t)n_snap;
+                if (!hit) {
+                    c->gas_t.assign(t_snap, t_snap + n_snap);
+                    c->gas_imgs.assign((size_t)n_snap, std::vector<unsigned char>());
+                    for (int j = 0; j < n_snap; ++j) todo.push_back(i * n_snap + j);
+                }
+            }
+            for (int u = 0; u < n_units; ++u) imgs[(size_t)u] = &clouds[u / n_snap]->gas_imgs[(size_t)(u % n_snap)];
+        }
+        if (!todo.empty()) {
             std::atomic<int> next{0};
+            const int n_todo = (int)todo.size();
             auto work = [&]() {
-                for (int u = next.fetch_add(1); u < n_units; u = next.fetch_add(1)) {
+                for (int k = next.fetch_add(1); k < n_todo; k = next.fetch_add(1)) {
+                    const int u = todo[(size_t)k];
                     GasUnit gu;
                     build_gas_unit(clouds[u / n_snap]->host, t_snap[u % n_snap], gu);
-                    build_blob(clouds[u / n_snap]->host, imgs[(size_t)u], &gu);
+                    build_blob(clouds[u / n_snap]->host, clouds[u / n_snap]->gas_imgs[(size_t)(u % n_snap)], &gu);
                 }
             };
-            const int n_thr = std::min(n_units, (int)std::min(std::max(1u, std::thread::hardware_concurrency()), 16u));
+            const int n_thr = std::min(n_todo, (int)std::min(std::max(1u, std::thread::hardware_concurrency()), 16u));
             std::vector<std::thread> pool;
             for (int k = 1; k < n_thr; ++k) pool.emplace_back(work);
             work();
             for (auto &th : pool) th.join();
         }
         for (int u = 0; u < n_units; ++u) {
-            const std::vector<unsigned char> &img = imgs[(size_t)u];
+            const std::vector<unsigned char> &img = *imgs[(size_t)u];
             DevCloudHeader hd;
             std::memcpy(&hd, img.data(), sizeof(hd));
             if (hd.depth_bisect == 1u) return fail(PDV_E_UNSUPPORTED, "gas unit: depth table too irregular for the one-probe guide (use fewer n_depth_bins)");
@@ -636,7 +731,7 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *
     StreamScratch scratch;
     if ((s = scratch_alloc(off, device, st, scratch)) != PDV_OK) return s;
     unsigned char *ws = scratch.p;
-    if ((s = ensure_events(device)) != PDV_OK) return s;
+    if ((s = ensure_events(device, st)) != PDV_OK) return s;
 
     // ---- unit table: visiting order (descending estimated cost), where each block starts, guided chunk sizes per unit ----
     std::vector<unsigned char> table(table_bytes, 0);
@@ -708,6 +803,11 @@ pdv_status run_impl(const pdv_cloud *const *clouds, int n_clouds, const double *
     }
     CUX(cudaEventRecord(g_ev.e1, st), "cudaEventRecord");
     g_last.pending = true;               // elapsed time is read when the events have completed
+    if (n_photons > 0)                   // whoever reuses a cloud's buffer after its destruction waits for this launch (ensure_on_device)
+        for (int i = 0; i < n_clouds; ++i) {
+            std::lock_guard<std::mutex> lk(clouds[i]->mu);
+            if (clouds[i]->last_read && cudaEventRecord(clouds[i]->last_read, st) == cudaSuccess) clouds[i]->read_pending = true;
+        }
 
     const bool dev_out = o->output_on_device != 0;
     double *oh = dev_out ? hist : reinterpret_cast<double *>(ws + o_oh);
@@ -863,7 +963,13 @@ pdv_status run_static_impl(const pdv_cloud *const *clouds, int n_clouds, int n_s
     rp.hist2 = reinterpret_cast<unsigned long long *>(ws + o_hist2);
     rp.stats = reinterpret_cast<unsigned long long *>(ws + o_stats);
     rp.trace = nullptr;
-    if (n_photons > 0) CU(launch_transport(rp, plan.variant, plan.shape, st), "transport kernel launch");
+    if (n_photons > 0) {
+        CU(launch_transport(rp, plan.variant, plan.shape, st), "transport kernel launch");
+        for (int i = 0; i < n_clouds; ++i) {                  // recording an existing event allocates nothing
+            std::lock_guard<std::mutex> lk(clouds[i]->mu);
+            if (clouds[i]->last_read && cudaEventRecord(clouds[i]->last_read, st) == cudaSuccess) clouds[i]->read_pending = true;
+        }
+    }
     CU(launch_finalize(rp.hist, rp.hist2, rp.stats, (uint32_t)n_units, (uint32_t)nb, hist, hist2, stats, st), "finalize kernel launch");
     return PDV_OK;
 }
@@ -918,7 +1024,7 @@ pdv_status pdv_cloud_create(const pdv_cloud_params *params, pdv_cloud **out) {
 
 void pdv_cloud_destroy(pdv_cloud *c) {
     if (!c) return;
-    if (c->d_blob) g_blob_cache.give(c->d_blob, c->d_bytes, c->device);
+    if (c->d_blob) g_blob_cache.give(BlobCache::Entry{c->d_blob, c->d_bytes, c->device, c->last_read, c->read_pending});
     delete c;
 }
 
@@ -1258,22 +1364,34 @@ pdv_status pdv_issue_peaks(double millis, double *ffma, double *mufu, double *mh
     return PDV_OK;
 }
 
-pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes, int32_t *variant) {
-    if (g_last.pending && g_ev.e0 && g_ev.e1) {      // output_on_device run: wait for its transport kernel only
+static pdv_status launch_info_of(LastLaunch *l, int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes,
+                                 int32_t *variant) {
+    static const LastLaunch none;
+    if (!l) l = const_cast<LastLaunch *>(&none);
+    if (l->pending && l->e0 && l->e1) {          // output_on_device run: wait for that run's transport kernel only
         float ms = 0.f;
-        if (cudaEventSynchronize(g_ev.e1) == cudaSuccess && cudaEventElapsedTime(&ms, g_ev.e0, g_ev.e1) == cudaSuccess)
-            g_last.ms = ms;
+        if (cudaEventSynchronize(l->e1) == cudaSuccess && cudaEventElapsedTime(&ms, l->e0, l->e1) == cudaSuccess)
+            l->ms = ms;
         else
             cudaGetLastError();
-        g_last.pending = false;
+        l->pending = false;
     }
-    if (n_kernels) *n_kernels = g_last.n_kernels;
-    if (transport_ms) *transport_ms = g_last.ms;
-    if (grid) *grid = g_last.grid;
-    if (block) *block = g_last.block;
-    if (smem_bytes) *smem_bytes = g_last.smem;
-    if (variant) *variant = g_last.variant;
+    if (n_kernels) *n_kernels = l->n_kernels;
+    if (transport_ms) *transport_ms = l->ms;
+    if (grid) *grid = l->grid;
+    if (block) *block = l->block;
+    if (smem_bytes) *smem_bytes = l->smem;
+    if (variant) *variant = l->variant;
     return PDV_OK;
+}
+
+pdv_status pdv_last_launch_info(int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block, int32_t *smem_bytes, int32_t *variant) {
+    return launch_info_of(g_last_ptr, n_kernels, transport_ms, grid, block, smem_bytes, variant);
+}
+
+pdv_status pdv_launch_info_on_stream(void *cuda_stream, int32_t *n_kernels, float *transport_ms, int32_t *grid, int32_t *block,
+                                     int32_t *smem_bytes, int32_t *variant) {
+    return launch_info_of(launch_slot((cudaStream_t)cuda_stream, false), n_kernels, transport_ms, grid, block, smem_bytes, variant);
 }
 
 }  // extern "C"
