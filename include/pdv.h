@@ -78,7 +78,13 @@ typedef struct {
      * snapshot time: pdv_mc_run builds the depth tables of every (cloud, snapshot) unit at run time. */
     double gas_density;          /* rho_g, kg/m^3; 0: vacuum (the paper; every other field keeps its meaning and the run is bit-identical
                                     to one without these two fields) */
-    double drag_coefficient;     /* C_d > 0 when gas_density > 0 (0.5 is typical of spheres at high Reynolds number) */
+    double drag_coefficient;     /* C_d > 0 when gas_density > 0 (0.5 is typical of spheres at high Reynolds number).
+                                    Limit: a gas unit keeps one row of class thresholds PER DEPTH BIN in shared memory
+                                    (n_depth_bins x (2^ceil(log2 n_classes) + 1) words), so 16 classes with 1024-cell phase tables and
+                                    512 velocity bins run with at most about 790 depth bins: the row-f4 workload uses n_depth_bins
+                                    = 256, and 16 x 1024 is PDV_E_UNSUPPORTED.  256 bins are enough at the statistics this library is run at: two stored
+                                    oracle runs of that workload's last snapshot at 1e8 histories, 256 against 1024 bins, agree
+                                    bin by bin within their noise (tests/test_oracle_gas.py) */
 } pdv_cloud_params;
 
 #define PDV_MAX_CLASSES 32

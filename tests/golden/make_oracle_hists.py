@@ -44,6 +44,10 @@ JOBS = {
     # R38), so a spectrum is stored per snapshot: the first and the last of the 20.  ("gas", snapshot index, histories)
     "f4gas_snap00": ("gas", 0, 100_000_000),
     "f4gas_snap19": ("gas", 19, 100_000_000),
+    # the same last snapshot with 1024 depth bins instead of the workload's 256 (the product limit for 16 classes in a gas, pdv.h):
+    # oracle against oracle, the two stored runs bound the discretisation error of the 256 bins at 1e8 histories
+    # (tests/test_oracle_gas.py).  ("gas", snapshot index, histories, depth bins)
+    "f4gas_snap19_nd1024": ("gas", 19, 100_000_000, 1024),
 }
 for _i in range(48):
     if f"cfg4_cloud{_i:02d}" not in JOBS:
@@ -52,7 +56,8 @@ SMALL_CHUNK = 1_000_000     # chunk of the 2e7-history jobs: 20 chunks for the b
 
 
 def make(name: str) -> str:
-    idx, ci, n = JOBS[name]
+    idx, ci, n = JOBS[name][:3]
+    n_depth = JOBS[name][3] if len(JOBS[name]) > 3 else None
     chunk = CHUNK if n >= 100_000_000 else SMALL_CHUNK
     gas = None
     if idx == "gas":
@@ -60,7 +65,7 @@ def make(name: str) -> str:
         cfg, snap, ci = W.gas_spectrogram(), ci, 0
         par = cfg["clouds"][0]
         oc = ocloud.build_cloud(par)
-        gas = ogas.build_tables(oc, par, cfg["t_snap"][snap], par["n_depth_bins"])
+        gas = ogas.build_tables(oc, par, cfg["t_snap"][snap], n_depth or par["n_depth_bins"])
     else:
         cfg = W.config(idx)
         oc = ocloud.build_cloud(cfg["clouds"][ci])
@@ -80,7 +85,7 @@ def make(name: str) -> str:
         "what": "oracle/ (fp64 CPU Monte-Carlo) tallies; written by tests/golden/make_oracle_hists.py; no value comes from the CUDA path",
         "workload": cfg["name"], "config_index": idx, "cloud_index": ci, "t_snap": (gas["t"] if gas else None), "n_photons": n, "seed": SEED, "rng_mode": 0,
         "run": {k: run[k] for k in ("n_bins", "v_lo", "v_hi", "aperture_sr", "mode", "max_events", "roulette_survival")},
-        "tau_ext": oc.tau_ext, "seconds": round(time.time() - t0, 1), "threads": os.cpu_count(),
+        "n_depth_bins": (n_depth or cfg["clouds"][0].get("n_depth_bins")), "tau_ext": oc.tau_ext, "seconds": round(time.time() - t0, 1), "threads": os.cpu_count(),
         "stats": {k: (int(v) if isinstance(v, int) else float(v)) for k, v in stats.items()},
         "chunk": chunk, "chunk_stats": chunk_stats,
         "hist": [float(x) for x in hist], "hist2": [float(x) for x in hist2],

@@ -184,3 +184,22 @@ def test_spectrum_depends_on_time_in_gas_and_not_in_the_vacuum_limit(cfg3_gas):
         assert res["worst"] < 5.0 and res["chi2"] < res["ndf"] + 5 * math.sqrt(2 * res["ndf"])
     # the optical structure does not change with time: same number of events per history (mean path), gas or not
     assert a.stats["particle_events"] / n == pytest.approx(v.stats["particle_events"] / n, rel=0.01)
+
+
+def test_256_depth_bins_are_enough_for_the_gas_workload_at_1e8_histories():
+    """The product runs 16 size classes in a gas with at most 256 depth bins (per-bin class thresholds: 16 x 1024 would not fit
+    the shared memory of a block; include/pdv.h), where every vacuum workload uses 1024.  Two STORED oracle runs of the last
+    snapshot of the row-f4 workload, 1e8 histories each, one with the workload's 256 bins and one with 1024
+    (tests/golden/make_oracle_hists.py: f4gas_snap19, f4gas_snap19_nd1024; oracle against oracle, nothing of the CUDA path):
+    their spectra agree bin by bin within 5 sigma of their own noise and their integrated rates to 5 sigma -- the
+    discretisation error of 256 bins (reading R37) is below what 1e8 histories resolve."""
+    from histcmp import load_golden, per_history_variance
+    a, b = load_golden("f4gas_snap19"), load_golden("f4gas_snap19_nd1024")
+    assert a.n_photons == b.n_photons == 10 ** 8 and a.run == b.run and a.tau_ext == pytest.approx(b.tau_ext, rel=1e-12)
+    res = compare(a.hist, a.hist2, a.n_photons, b.hist, b.hist2, b.n_photons)
+    assert res["ndf"] >= 200 and res["worst"] < 5.0, res["worst"]
+    assert res["chi2"] < res["ndf"] + 6 * math.sqrt(2 * res["ndf"]) + 10, (res["chi2"], res["ndf"])
+    for key in ("detected", "escaped", "absorbed_particles", "absorbed_surface"):
+        x, y = a.stats[key] / a.n_photons, b.stats[key] / b.n_photons
+        assert abs(x - y) < 5 * math.sqrt(max(x, 1e-12) / a.n_photons + max(y, 1e-12) / b.n_photons), (key, x, y)
+    assert a.stats["particle_events"] / a.n_photons == pytest.approx(b.stats["particle_events"] / b.n_photons, rel=1e-3)
