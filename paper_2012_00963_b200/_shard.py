@@ -200,7 +200,7 @@ def _reduce_job_device(hist, hist2, stats_u8, unit_ids, n_units: int, group=None
     if n_local:
         wf.index_add_(0, idx, words[:, :N_STAT_FLOATS].view(torch.float64))
         wi.index_add_(0, idx, words[:, N_STAT_FLOATS:N_STAT_FLOATS + 3])
-        mx.index_reduce_(0, idx, words[:, N_STAT_WORDS - 1], "amax", include_self=True)
+        mx.index_copy_(0, idx, words[:, N_STAT_WORDS - 1].contiguous())      # a unit appears once per rank: a copy is the maximum
     if dist.is_initialized() and dist.get_world_size(group) > 1:
         dist.all_reduce(out, op=dist.ReduceOp.SUM, group=group)
         dist.all_reduce(wf, op=dist.ReduceOp.SUM, group=group)

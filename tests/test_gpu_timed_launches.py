@@ -236,3 +236,43 @@ def test_phase_table_error_at_spectrum_level_and_fig6_cases(P):
     r6 = P.pdv_mc_run([mie, iso], cfg["t_snap"], n6, 32, cfg["run"])
     res = compare(r6.hist[0, 0], r6.hist2[0, 0], n6, r6.hist[1, 0], r6.hist2[1, 0], n6)
     assert res["worst"] > 20.0 and res["chi2"] > 10 * res["ndf"], (res["worst"], res["chi2"], res["ndf"])
+
+
+@pytest.mark.parametrize("idx,n_snap,n_clouds", [(3, None, 7), (2, 5, None)])
+def test_cost_balanced_shares_of_a_job_reduce_to_the_one_call_job_bit_for_bit(P, idx, n_snap, n_clouds):
+    """Row f3 with the round-3 split (_shard.plan_balanced, what `bench.py --gpus N --scaling strong` runs for multi-unit jobs): the
+    job is cut into 3 stretches of equal estimated cost (the library's pdv_estimated_flights), units that straddle a rank boundary
+    split by photon id.  The three shares are run one after the other on this GPU, each segment one pdv_mc_run call with its units'
+    sub-streams of the whole job, and reduced with reduce_job on the raw statistics records (the device path): hist, hist2 and
+    every field of stats equal the one-call run of the job."""
+    import torch
+    from paper_2012_00963_b200 import _shard
+    cfg = W.scaled(W.config(idx), 150_001, n_snap=n_snap, n_clouds=n_clouds)
+    run, n, world = cfg["run"], cfg["run"]["n_photons"], 3
+    clouds = [P.pdv_cloud_create(c) for c in cfg["clouds"]]
+    nc, ns, nb = len(clouds), len(cfg["t_snap"]), run["n_bins"]
+    whole = P.pdv_mc_run(clouds, cfg["t_snap"], n, 23, run)
+    costs = [c.estimated_flights(run) for c in clouds for _ in cfg["t_snap"]]
+    acc_h = torch.zeros((nc * ns, nb), dtype=torch.float64)
+    acc_h2 = torch.zeros_like(acc_h)
+    acc_st = None
+    n_split_units = 0
+    for rank in range(world):
+        segs = _shard.plan_balanced(costs, nc, ns, n, rank, world)
+        assert 1 <= len(segs) <= 3 or ns > 1                  # a partial unit at each end and the whole units between them
+        rh, rh2, rs, ids = [], [], [], []
+        for sg in segs:
+            r = P.pdv_mc_run([clouds[i] for i in sg["clouds"]], [cfg["t_snap"][j] for j in sg["snaps"]], sg["n_photons"], 23,
+                             dict(run, first_photon_id=sg["first_photon_id"], unit_streams=sg["unit_ids"]))
+            rh.append(r.hist.reshape(-1, nb)); rh2.append(r.hist2.reshape(-1, nb)); rs.append(r.stats.reshape(-1)); ids += sg["unit_ids"]
+            n_split_units += sum(1 for _ in sg["unit_ids"]) if sg["n_photons"] < n else 0
+        st_u8 = torch.from_numpy(np.frombuffer(np.concatenate(rs).tobytes(), dtype=np.uint8).copy())
+        h, h2, st = _shard.reduce_job(torch.from_numpy(np.concatenate(rh)), torch.from_numpy(np.concatenate(rh2)), st_u8, ids, nc * ns)
+        acc_h += h
+        acc_h2 += h2
+        st = st.numpy().view(P.STATS_DTYPE)
+        acc_st = st if acc_st is None else _shard.merge_stats([acc_st, st])
+    assert n_split_units >= 2                                 # units were indeed cut by photon id
+    assert np.array_equal(acc_h.numpy(), whole.hist.reshape(-1, nb)) and np.array_equal(acc_h2.numpy(), whole.hist2.reshape(-1, nb))
+    for k in acc_st.dtype.names:
+        assert np.array_equal(acc_st[k], whole.stats.reshape(-1)[k]), k
